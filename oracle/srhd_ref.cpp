@@ -1,0 +1,640 @@
+// oracle/srhd_ref.cpp
+//
+// TEST INFRASTRUCTURE ONLY (see srhd_ref.hpp).  Plain fp64 CPU restatement of the GAMER-SR
+// (arXiv 2012.11130) per-patch-group SRHD update, written from the paper's equations in the paper's
+// order.  No blocking, no fusion, no reordering beyond what the cited passages / DESIGN.md
+// readings state.  Build: g++ -O2 -ffp-contract=off -fopenmp (see oracle/build.py); std::fma is
+// used only where DESIGN.md "canonical forms" says so.
+//
+// "P:n" = /root/reference/PAPER.md line n.  "S#"/"G#" = readings listed in DESIGN.md section 4.
+#include "srhd_ref.hpp"
+
+#include <algorithm>
+#include <cfloat>
+#include <cmath>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr double kEps = DBL_EPSILON;  // eps_machine of Eq. 30 for double precision
+
+// ---------------------------------------------------------------- O1: Taub-Mathews EoS ---------
+// P:185 Eq. 22: htilde = 2.5 T + 2.25 T^2 / (1 + sqrt(2.25 T^2 + 1))      (subtraction free)
+double htilde_of_T(double T) {
+  const double a = 2.25 * T * T;
+  return 2.5 * T + a / (1.0 + std::sqrt(a + 1.0));
+}
+// P:148 Eq. 16: T = (2 ht^2 + 4 ht) / (5 ht + 5 + sqrt(9 ht^2 + 18 ht + 25))
+double T_of_htilde(double ht) {
+  return (2.0 * ht * ht + 4.0 * ht) / (5.0 * ht + 5.0 + std::sqrt(9.0 * ht * ht + 18.0 * ht + 25.0));
+}
+// P:591 Eq. A2
+double dT_dhtilde(double ht) {
+  const double s = std::sqrt(9.0 * ht * ht + 18.0 * ht + 25.0);
+  const double den = 5.0 * ht + 5.0 + s;
+  return (4.0 * ht + 4.0) / den - (2.0 * ht * ht + 4.0 * ht) * ((9.0 * ht + 9.0) / s + 5.0) / (den * den);
+}
+// P:129 Eq. 14 squared, with h = 1 + htilde(T) (Eq. 10 == 1 + Eq. 22)
+double cs2_of_T(double T) {
+  const double h = 1.0 + htilde_of_T(T);
+  return (T / (3.0 * h)) * ((5.0 * h - 8.0 * T) / (h - T));
+}
+// P:140-144 Eq. 15, right-hand side f(htilde) with musq = (|M|/D)^2, T = T(htilde) by Eq. 16
+double f_eq15(double ht, double T, double musq) {
+  const double h = ht + 1.0;
+  return ht * ht + 2.0 * ht - 2.0 * T * h + (T * T) * (h * h) / (h * h + musq);
+}
+// P:587 Eq. A1
+double df_eqA1(double ht, double T, double dT, double musq) {
+  const double h = ht + 1.0;
+  const double den = h * h + musq;
+  const double h4 = (h * h) * (h * h);
+  return 2.0 * ht + 2.0 - 2.0 * T - 2.0 * h * dT +
+         (2.0 * T * h4 * dT + 2.0 * T * h * musq * (h * dT + T)) / (den * den);
+}
+// initial guess.  A7 threshold; A6 hot branch; A4 cold branch in the corrected form
+// (reading G2: the positive root of A3; the printed numerator sqrt(...) is a typo).
+double htilde_guess(double L, double musq) {
+  const double s = 1.0 + musq;
+  const double q = 43.0 * musq + 63.0;
+  const double r = 1800.0 * s / (437.0 * musq + 117.0);
+  if (L > r * r) return (4.0 / 3.0) * std::sqrt(L);                                   // A6
+  return 125.0 * s * L / (75.0 * s + std::sqrt(125.0 * s * q * L + 5625.0 * s * s));  // A4 (G2)
+}
+
+// ---------------------------------------------------------------- O2: prim -> cons --------------
+// P:641 Fig. 15 (right); Eq. 5a, 5b; Eq. 22, 23; Eq. 15 "with known |M|/D".
+void prim2cons(const double W[5], double U[5]) {
+  const double rho = W[0], Ux = W[1], Uy = W[2], Uz = W[3], p = W[4];
+  const double T = p / rho;                                   // Eq. 18
+  const double ht = htilde_of_T(T);                           // Eq. 22
+  const double Usq = Ux * Ux + Uy * Uy + Uz * Uz;
+  const double gamma = std::sqrt(1.0 + Usq);                  // Eq. 8
+  const double D = rho * gamma;                               // Eq. 5a
+  const double h = 1.0 + ht;
+  const double Dh = D * h;
+  const double musq = (h * h) * Usq;                          // (|M|/D)^2 from Eq. 5b
+  const double f = f_eq15(ht, T, musq);                       // Eq. 15
+  U[0] = D;
+  U[1] = Dh * Ux;                                             // Eq. 5b
+  U[2] = Dh * Uy;
+  U[3] = Dh * Uz;
+  U[4] = D * ((musq + f) / (1.0 + std::sqrt(1.0 + musq + f)));  // Eq. 23
+}
+
+// ---------------------------------------------------------------- O3: cons -> prim --------------
+// P:641 Fig. 15 (left); Eq. 15-18; App. A; Eq. 30.
+// Canonical IEEE sequence for L: division, sqrt and fma are
+// correctly rounded, so L is reproducible bit for bit by any IEEE implementation.
+// Returns true iff the input passes D>0, Etilde>0, L>eps (Eq. 30).  A failing state is evaluated
+// with L <- eps (reading S10) so the result is deterministic and finite.
+bool cons2prim(const double U[5], double W[5], double rtol, int max_iter, int* iters_out,
+               double* ht_out) {
+  const double D = U[0], Et = U[4];
+  bool phys = (D > 0.0) && (Et > 0.0);
+  // S10: a state without positive D is evaluated as vacuum at rest (D <- DBL_MIN, M <- 0, Etilde <- 0)
+  const bool dpos = D > DBL_MIN;
+  const double Dc = dpos ? D : DBL_MIN;
+  const double Mx = dpos ? U[1] : 0.0, My = dpos ? U[2] : 0.0, Mz = dpos ? U[3] : 0.0;
+  const double x = dpos ? Et / Dc : 0.0;
+  const double ux = Mx / Dc, uy = My / Dc, uz = Mz / Dc;
+  const double musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
+  double L = std::fma(x, x + 2.0, -musq);                     // left-hand side of Eq. 15 / Eq. 30
+  if (!(L > kEps)) {
+    phys = false;
+    L = kEps;
+  }
+  double ht = htilde_guess(L, musq);
+  int it = 0;
+  while (it < max_iter) {                                     // Newton-Raphson
+    const double T = T_of_htilde(ht);
+    const double dT = dT_dhtilde(ht);
+    const double delta = (f_eq15(ht, T, musq) - L) / df_eqA1(ht, T, dT, musq);
+    const double ht_new = ht - delta;
+    ++it;
+    const bool done = (ht_new == ht) || (std::fabs(delta) <= rtol * std::fabs(ht_new));  // S2
+    ht = ht_new;
+    if (done) break;
+  }
+  const double h = 1.0 + ht;
+  const double Ux = Mx / (Dc * h), Uy = My / (Dc * h), Uz = Mz / (Dc * h);        // Eq. 17
+  const double gamma = std::sqrt(1.0 + (Ux * Ux + Uy * Uy + Uz * Uz));            // Eq. 8
+  const double rho = Dc / gamma;                                                   // Eq. 5a
+  const double T = T_of_htilde(ht);                                                // Eq. 16
+  W[0] = rho;
+  W[1] = Ux;
+  W[2] = Uy;
+  W[3] = Uz;
+  W[4] = rho * T;                                                                  // Eq. 18
+  if (iters_out) *iters_out = it;
+  if (ht_out) *ht_out = ht;
+  return phys;
+}
+
+// Eq. 30 check alone, same canonical L (used on updated cells, O9)
+bool is_physical(const double U[5]) {
+  const double D = U[0], Et = U[4];
+  if (!(D > 0.0) || !(Et > 0.0)) return false;
+  const double x = Et / D;
+  const double ux = U[1] / D, uy = U[2] / D, uz = U[3] / D;
+  const double musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
+  const double L = std::fma(x, x + 2.0, -musq);
+  return L > kEps;
+}
+
+// ---------------------------------------------------------------- O4: signal speed --------------
+// P:241 Eq. 26 (reading G1: |U^x|+|U^y|+|U^z|), from primitives; T = p/rho (Eq. 18)
+double umax_of_prim(const double W[5]) {
+  const double T = W[4] / W[0];
+  const double cs2 = cs2_of_T(T);
+  const double Us2 = cs2 / (1.0 - cs2);                       // U_s = c_s/sqrt(1-c_s^2)
+  const double Us = std::sqrt(Us2);
+  const double gs = std::sqrt(1.0 + Us2);                     // gamma_s (reading G4)
+  const double gamma = std::sqrt(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+  return gs * (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + 3.0 * gamma * Us;
+}
+double smax_of_umax(double umax) { return umax / std::sqrt(1.0 + umax * umax); }  // P:247 Eq. 27
+
+// ---------------------------------------------------------------- fluxes ------------------------
+// P:61-65 Eq. 4a, 4b and P:83 Eq. 7 along direction d; v = U_d/gamma
+void phys_flux(int d, const double W[5], const double U[5], double F[5]) {
+  const double gamma = std::sqrt(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+  const double v = W[1 + d] / gamma;
+  F[0] = U[0] * v;
+  F[1] = U[1] * v;
+  F[2] = U[2] * v;
+  F[3] = U[3] * v;
+  F[1 + d] += W[4];
+  F[4] = (U[4] + W[4]) * v;
+}
+
+// One side of a Riemann problem in the rotated frame (n = normal, t1, t2 = tangential).
+struct Side {
+  double U[5];   // D, M_n, M_t1, M_t2, Etilde
+  double F[5];   // physical flux along n
+  double p, vn, lam_m, lam_p;
+};
+// Acoustic eigenvalues in 4-velocity form (reading S6):
+//   lambda_pm = (gamma U_n +- U_s Q) / (gamma^2 + U_s^2),  Q = sqrt(1 + U_t^2 + U_s^2)
+void side_setup(int d, const double W[5], const double U[5], Side& s) {
+  const int n = 1 + d, t1 = 1 + (d + 1) % 3, t2 = 1 + (d + 2) % 3;
+  const double rho = W[0], Un = W[n], Ut1 = W[t1], Ut2 = W[t2], p = W[4];
+  const double T = p / rho;
+  const double cs2 = cs2_of_T(T);                             // Eq. 14 (TM sound speed)
+  const double Us2 = cs2 / (1.0 - cs2);
+  const double Us = std::sqrt(Us2);
+  const double Utsq = Ut1 * Ut1 + Ut2 * Ut2;
+  const double g2 = 1.0 + (Un * Un + Utsq);
+  const double gamma = std::sqrt(g2);
+  const double Q = std::sqrt(1.0 + Utsq + Us2);
+  s.lam_p = (gamma * Un + Us * Q) / (g2 + Us2);
+  s.lam_m = (gamma * Un - Us * Q) / (g2 + Us2);
+  s.vn = Un / gamma;
+  s.p = p;
+  s.U[0] = U[0];
+  s.U[1] = U[n];
+  s.U[2] = U[t1];
+  s.U[3] = U[t2];
+  s.U[4] = U[4];
+  s.F[0] = s.U[0] * s.vn;
+  s.F[1] = s.U[1] * s.vn + p;
+  s.F[2] = s.U[2] * s.vn;
+  s.F[3] = s.U[3] * s.vn;
+  s.F[4] = (s.U[4] + p) * s.vn;
+}
+
+// HLLE (Mignone & Bodo 2005 form with the S6 speeds); rotated frame
+void hlle_rot(const Side& L, const Side& R, double F[5]) {
+  const double SL = std::min(L.lam_m, R.lam_m), SR = std::max(L.lam_p, R.lam_p);
+  if (SL >= 0.0) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
+  if (SR <= 0.0) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
+  for (int c = 0; c < 5; ++c)
+    F[c] = (SR * L.F[c] - SL * R.F[c] + SL * SR * (R.U[c] - L.U[c])) / (SR - SL);
+}
+// HLLC adapted to Etilde ("replacing E with Etilde + D c^2"; reading S7); rotated frame
+void hllc_rot(const Side& L, const Side& R, double F[5]) {
+  const double SL = std::min(L.lam_m, R.lam_m), SR = std::max(L.lam_p, R.lam_p);
+  if (SL >= 0.0) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
+  if (SR <= 0.0) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
+  double Uh[5], Fh[5];                                        // HLL state and flux
+  for (int c = 0; c < 5; ++c) {
+    Uh[c] = (SR * R.U[c] - SL * L.U[c] + L.F[c] - R.F[c]) / (SR - SL);
+    Fh[c] = (SR * L.F[c] - SL * R.F[c] + SL * SR * (R.U[c] - L.U[c])) / (SR - SL);
+  }
+  const double Eh = Uh[4] + Uh[0];                            // E = Etilde + D   (sums only)
+  const double FEh = Fh[4] + Fh[0];
+  const double a = FEh, b = Eh + Fh[1], m = Uh[1];
+  // contact speed: root of a lam^2 - b lam + m = 0 in (-1,1), rationalised (safe for a -> 0)
+  const double lam = 2.0 * m / (b + std::sqrt(b * b - 4.0 * a * m));
+  const double ps = Fh[1] - lam * FEh;                        // p*
+  const Side& K = (lam >= 0.0) ? L : R;
+  const double S = (lam >= 0.0) ? SL : SR;
+  const double A = S - K.vn;
+  const double den = S - lam;
+  double Us[5];
+  Us[0] = K.U[0] * A / den;
+  Us[1] = (K.U[1] * A + ps - K.p) / den;
+  Us[2] = K.U[2] * A / den;
+  Us[3] = K.U[3] * A / den;
+  Us[4] = (K.U[4] * A + ps * lam - K.p * K.vn) / den;         // linear in E: no D is subtracted
+  for (int c = 0; c < 5; ++c) F[c] = K.F[c] + S * (Us[c] - K.U[c]);
+}
+void riemann_flux(int riemann, int d, const double WL[5], const double UL[5], const double WR[5],
+                  const double UR[5], double F[5]) {
+  Side L, R;
+  side_setup(d, WL, UL, L);
+  side_setup(d, WR, UR, R);
+  double Fr[5];
+  if (riemann == 0) hlle_rot(L, R, Fr); else hllc_rot(L, R, Fr);
+  const int n = 1 + d, t1 = 1 + (d + 1) % 3, t2 = 1 + (d + 2) % 3;
+  F[0] = Fr[0];
+  F[n] = Fr[1];
+  F[t1] = Fr[2];
+  F[t2] = Fr[3];
+  F[4] = Fr[4];
+}
+
+// ---------------------------------------------------------------- reconstruction ----------------
+// reading S3: van Leer harmonic mean capped by generalised minmod with coefficient beta
+double limited_slope(double sL, double sR, double beta) {
+  if (sL * sR <= 0.0) return 0.0;
+  const double vl = 2.0 * std::fabs(sL * sR) / std::fabs(sL + sR);
+  const double mm = beta * std::min(std::fabs(sL), std::fabs(sR));
+  const double mag = std::min(vl, mm);
+  return (sL > 0.0) ? mag : -mag;
+}
+// a[0..4] = a_{i-2..i+2}; returns the left/right edge values of cell i.
+// PLM: a -+ d/2.  PPM (reading S4): Colella & Woodward 1984 on a uniform grid.
+void recon_1d(int recon, const double a[5], double beta, double beta0, double& am, double& ap) {
+  const double ai = a[2];
+  if (recon == 0) {
+    const double d = limited_slope(ai - a[1], a[3] - ai, beta);
+    am = ai - 0.5 * d;
+    ap = ai + 0.5 * d;
+    return;
+  }
+  const double dm = limited_slope(a[1] - a[0], a[2] - a[1], beta);   // d_{i-1}
+  const double d0 = limited_slope(a[2] - a[1], a[3] - a[2], beta);   // d_i
+  const double dp = limited_slope(a[3] - a[2], a[4] - a[3], beta);   // d_{i+1}
+  am = 0.5 * (a[1] + a[2]) - (d0 - dm) / 6.0;                         // face i-1/2
+  ap = 0.5 * (a[2] + a[3]) - (dp - d0) / 6.0;                         // face i+1/2
+  if ((ap - ai) * (ai - am) <= 0.0) {                                 // CW84 Eq. 1.10
+    am = ai;
+    ap = ai;
+  } else {
+    const double dd = ap - am;
+    const double c6 = 6.0 * (ai - 0.5 * (am + ap));
+    if (dd * c6 > dd * dd) am = 3.0 * ai - 2.0 * ap;
+    else if (-(dd * dd) > dd * c6) ap = 3.0 * ai - 2.0 * am;
+  }
+  if (beta != beta0) {                                                // retry blend (reading S4)
+    const double w = beta / beta0;
+    am = ai + w * (am - ai);
+    ap = ai + w * (ap - ai);
+  }
+}
+
+// ---------------------------------------------------------------- O5-O9: one box ----------------
+struct Box {
+  int nx, ny, nz, g;
+  int sx, sy, sz;   // padded extents
+  size_t cstride;   // padded cells per component
+  size_t at(int i, int j, int k) const {   // i,j,k in [-g, n+g)
+    return (size_t)(k + g) * sy * sx + (size_t)(j + g) * sx + (size_t)(i + g);
+  }
+};
+
+int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt, double dh,
+             const srhd_ref_params& par, srhd_ref_stats& st) {
+  const int g = par.ghost;
+  Box b{nx, ny, nz, g, nx + 2 * g, ny + 2 * g, nz + 2 * g, 0};
+  b.cstride = (size_t)b.sx * b.sy * b.sz;
+  const size_t np = b.cstride;
+  const int ext[3] = {nx, ny, nz};
+  const int stp[3] = {1, b.sx, b.sx * b.sy};
+
+  // O5a: W = C2P(U) for every tile cell (incl. ghosts); pass independent
+  std::vector<double> Wc(5 * np);
+  double umax = 0.0;
+  for (int k = -g; k < nz + g; ++k)
+    for (int j = -g; j < ny + g; ++j)
+      for (int i = -g; i < nx + g; ++i) {
+        const size_t c = b.at(i, j, k);
+        double U[5], W[5];
+        for (int q = 0; q < 5; ++q) U[q] = cons_in[q * np + c];
+        int it = 0;
+        const bool phys = cons2prim(U, W, par.newton_rtol, par.newton_max_iter, &it, nullptr);
+        st.newton_iters += (unsigned long long)it;
+        for (int q = 0; q < 5; ++q) Wc[q * np + c] = W[q];
+        const bool interior = i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz;
+        if (interior) {
+          if (!phys) ++st.n_c2p_fail;
+          umax = std::max(umax, umax_of_prim(W));             // A2 / O4 on the input interior
+        }
+      }
+  st.max_speed = std::max(st.max_speed, smax_of_umax(umax));
+
+  // face states of the cells that are face-adjacent to the interior (at most one index outside)
+  std::vector<double> Um(3 * 5 * np), Up(3 * 5 * np);         // [dir][comp][cell] evolved cons
+  std::vector<double> Fx(5 * np);                             // scratch for one direction's fluxes
+  std::vector<double> Flux(3 * 5 * np);                       // [dir][comp][cell c] = F at c+1/2 n
+  const int K = par.max_retry;
+  double beta = par.minmod_coeff;
+  unsigned long long face_fail = 0, cell_fail = 0;
+  int pass = 0;
+  for (;; ++pass) {
+    if (pass > 0) beta = (pass <= K) ? beta * 0.75 : 0.0;     // P:273, reading S9
+    face_fail = 0;
+    cell_fail = 0;
+    // O5b + O6
+    for (int k = -1; k <= nz; ++k)
+      for (int j = -1; j <= ny; ++j)
+        for (int i = -1; i <= nx; ++i) {
+          const int nout = (i < 0 || i >= nx) + (j < 0 || j >= ny) + (k < 0 || k >= nz);
+          if (nout > 1) continue;
+          const size_t c = b.at(i, j, k);
+          double Wm[3][5], Wp[3][5];
+          for (int d = 0; d < 3; ++d)
+            for (int q = 0; q < 5; ++q) {
+              double a[5];
+              for (int m = -2; m <= 2; ++m) {
+                // PLM touches only m = -1..1; guard the read for PLM's narrower ghost zone
+                a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0
+                                                                     : Wc[q * np + c + (ptrdiff_t)m * stp[d]];
+              }
+              recon_1d(par.recon, a, beta, par.minmod_coeff, Wm[d][q], Wp[d][q]);
+            }
+          // O6: MUSCL-Hancock half step (reading S5), 3-D unsplit
+          double Ucm[3][5], Ucp[3][5], dU[5];
+          double dF[3][5];
+          for (int d = 0; d < 3; ++d) {
+            double Fm[5], Fp[5];
+            prim2cons(Wm[d], Ucm[d]);
+            prim2cons(Wp[d], Ucp[d]);
+            phys_flux(d, Wm[d], Ucm[d], Fm);
+            phys_flux(d, Wp[d], Ucp[d], Fp);
+            for (int q = 0; q < 5; ++q) dF[d][q] = Fp[q] - Fm[q];
+          }
+          const double hdt = dt / (2.0 * dh);
+          for (int q = 0; q < 5; ++q) dU[q] = -hdt * ((dF[0][q] + dF[1][q]) + dF[2][q]);
+          for (int d = 0; d < 3; ++d)
+            for (int q = 0; q < 5; ++q) {
+              Um[(d * 5 + q) * np + c] = Ucm[d][q] + dU[q];
+              Up[(d * 5 + q) * np + c] = Ucp[d][q] + dU[q];
+            }
+        }
+    // O7: one Riemann problem per face that touches an interior cell
+    for (int d = 0; d < 3; ++d) {
+      int lo[3] = {0, 0, 0}, hi[3] = {nx - 1, ny - 1, nz - 1};
+      lo[d] = -1;                                             // left cell index along d: -1..n-1
+      for (int k = lo[2]; k <= hi[2]; ++k)
+        for (int j = lo[1]; j <= hi[1]; ++j)
+          for (int i = lo[0]; i <= hi[0]; ++i) {
+            const size_t c = b.at(i, j, k), cr = c + stp[d];
+            double UL[5], UR[5], WL[5], WR[5], F[5];
+            for (int q = 0; q < 5; ++q) {
+              UL[q] = Up[(d * 5 + q) * np + c];
+              UR[q] = Um[(d * 5 + q) * np + cr];
+            }
+            int it = 0;
+            if (!cons2prim(UL, WL, par.newton_rtol, par.newton_max_iter, &it, nullptr)) ++face_fail;  // S15
+            st.newton_iters += (unsigned long long)it;
+            if (!cons2prim(UR, WR, par.newton_rtol, par.newton_max_iter, &it, nullptr)) ++face_fail;
+            st.newton_iters += (unsigned long long)it;
+            riemann_flux(par.riemann, d, WL, UL, WR, UR, F);
+            for (int q = 0; q < 5; ++q) Flux[(d * 5 + q) * np + c] = F[q];
+          }
+    }
+    // O8: update (reading S12: ((x)+(y))+(z), each (F+ - F-) first)
+    const double dtdh = dt / dh;
+    const size_t no = (size_t)nx * ny * nz;
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          const size_t c = b.at(i, j, k);
+          double Un[5];
+          for (int q = 0; q < 5; ++q) {
+            const double dfx = Flux[(0 * 5 + q) * np + c] - Flux[(0 * 5 + q) * np + c - stp[0]];
+            const double dfy = Flux[(1 * 5 + q) * np + c] - Flux[(1 * 5 + q) * np + c - stp[1]];
+            const double dfz = Flux[(2 * 5 + q) * np + c] - Flux[(2 * 5 + q) * np + c - stp[2]];
+            Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);
+            cons_out[q * no + ((size_t)k * ny + j) * nx + i] = Un[q];
+          }
+          if (!is_physical(Un)) ++cell_fail;                  // O9: Eq. 30 on the updated cell
+        }
+    (void)ext;
+    if ((face_fail == 0 && cell_fail == 0) || beta == 0.0) break;   // S9, S10
+  }
+  if (pass > 0) ++st.n_retry_pg;
+  st.n_c2p_fail += face_fail;        // only non-zero in an accepted beta = 0 pass (S15)
+  st.n_unphys_final += cell_fail;
+  return pass + 1;
+}
+
+// index of the source cell for ghost index i under a boundary type (reading S11)
+inline int map_index(int i, int n, int bc_lo, int bc_hi) {
+  if (i < 0) return (bc_lo == 0) ? ((i % n) + n) % n : 0;
+  if (i >= n) return (bc_hi == 0) ? (i % n) : n - 1;
+  return i;
+}
+
+}  // namespace
+
+// =================================================================== C entry points ============
+extern "C" {
+
+double srhd_ref_htilde_of_T(double T) { return htilde_of_T(T); }
+double srhd_ref_T_of_htilde(double ht) { return T_of_htilde(ht); }
+double srhd_ref_dT_dhtilde(double ht) { return dT_dhtilde(ht); }
+double srhd_ref_cs2_of_T(double T) { return cs2_of_T(T); }
+double srhd_ref_f_eq15(double ht, double musq) { return f_eq15(ht, T_of_htilde(ht), musq); }
+double srhd_ref_df_eqA1(double ht, double musq) {
+  return df_eqA1(ht, T_of_htilde(ht), dT_dhtilde(ht), musq);
+}
+double srhd_ref_htilde_guess(double L, double musq) { return htilde_guess(L, musq); }
+double srhd_ref_umax_of_prim(const double W[5]) { return umax_of_prim(W); }
+double srhd_ref_smax_of_umax(double umax) { return smax_of_umax(umax); }
+double srhd_ref_limited_slope(double sL, double sR, double beta) { return limited_slope(sL, sR, beta); }
+void srhd_ref_recon_1d(int recon, const double* a, double beta, double beta0, double* am, double* ap) {
+  recon_1d(recon, a, beta, beta0, *am, *ap);
+}
+void srhd_ref_phys_flux(int dir, const double* W, const double* U, double* F) { phys_flux(dir, W, U, F); }
+void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL, const double* WR,
+                           const double* UR, double* F) {
+  riemann_flux(riemann, dir, WL, UL, WR, UR, F);
+}
+
+void srhd_ref_prim2cons(const double* prim, double* cons, size_t n, size_t stride) {
+#pragma omp parallel for schedule(static)
+  for (long long i = 0; i < (long long)n; ++i) {
+    double W[5], U[5];
+    for (int q = 0; q < 5; ++q) W[q] = prim[q * stride + i];
+    prim2cons(W, U);
+    for (int q = 0; q < 5; ++q) cons[q * stride + i] = U[q];
+  }
+}
+
+void srhd_ref_cons2prim_diag(const double* cons, double* prim, size_t n, size_t stride,
+                             const srhd_ref_params* par, double* htilde, int* iters,
+                             unsigned char* unphys) {
+#pragma omp parallel for schedule(static)
+  for (long long i = 0; i < (long long)n; ++i) {
+    double W[5], U[5], ht;
+    int it;
+    for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
+    const bool phys = cons2prim(U, W, par->newton_rtol, par->newton_max_iter, &it, &ht);
+    for (int q = 0; q < 5; ++q) prim[q * stride + i] = W[q];
+    if (htilde) htilde[i] = ht;
+    if (iters) iters[i] = it;
+    if (unphys) unphys[i] = phys ? 0 : 1;
+  }
+}
+
+void srhd_ref_cons2prim(const double* cons, double* prim, size_t n, size_t stride,
+                        const srhd_ref_params* par, srhd_ref_stats* stats) {
+  unsigned long long nfail = 0, niter = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nfail, niter)
+  for (long long i = 0; i < (long long)n; ++i) {
+    double W[5], U[5];
+    int it;
+    for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
+    if (!cons2prim(U, W, par->newton_rtol, par->newton_max_iter, &it, nullptr)) ++nfail;
+    niter += (unsigned long long)it;
+    for (int q = 0; q < 5; ++q) prim[q * stride + i] = W[q];
+  }
+  if (stats) {
+    std::memset(stats, 0, sizeof(*stats));
+    stats->n_c2p_fail = nfail;
+    stats->newton_iters = niter;
+  }
+}
+
+void srhd_ref_max_signal_speed(const double* cons, size_t n, size_t stride,
+                               const srhd_ref_params* par, double* max_speed) {
+  double umax = 0.0;
+#pragma omp parallel for schedule(static) reduction(max : umax)
+  for (long long i = 0; i < (long long)n; ++i) {
+    double W[5], U[5];
+    for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
+    cons2prim(U, W, par->newton_rtol, par->newton_max_iter, nullptr, nullptr);
+    umax = std::max(umax, umax_of_prim(W));
+  }
+  *max_speed = smax_of_umax(umax);                            // monotone: convert once (O4)
+}
+
+int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt,
+                      double dh, const srhd_ref_params* par, srhd_ref_stats* stats) {
+  srhd_ref_stats st;
+  std::memset(&st, 0, sizeof(st));
+  const int passes = step_box(cons_in, cons_out, nx, ny, nz, dt, dh, *par, st);
+  if (stats) *stats = st;
+  return passes;
+}
+
+void srhd_ref_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+                         const srhd_ref_params* par, srhd_ref_stats* stats, int nthreads) {
+  const int nxt = 16 + 2 * par->ghost;
+  const size_t in_pg = (size_t)5 * nxt * nxt * nxt, out_pg = (size_t)8 * 5 * 512;
+  unsigned long long f1 = 0, f2 = 0, f3 = 0, f4 = 0;
+  double ms = 0.0;
+#ifdef _OPENMP
+  if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+  nthreads = 1;
+#endif
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : f1, f2, f3, f4) reduction(max : ms)
+  for (int pg = 0; pg < npg; ++pg) {
+    srhd_ref_stats st;
+    std::memset(&st, 0, sizeof(st));
+    std::vector<double> box((size_t)5 * 4096);
+    step_box(cons_in + pg * in_pg, box.data(), 16, 16, 16, dt, dh, *par, st);
+    double* out = cons_out + pg * out_pg;
+    for (int q = 0; q < 5; ++q)
+      for (int k = 0; k < 16; ++k)
+        for (int j = 0; j < 16; ++j)
+          for (int i = 0; i < 16; ++i) {
+            const int p = (i >> 3) + 2 * (j >> 3) + 4 * (k >> 3);          // S13
+            out[((size_t)p * 5 + q) * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7)] =
+                box[(size_t)q * 4096 + (k * 16 + j) * 16 + i];
+          }
+    f1 += st.n_c2p_fail;
+    f2 += st.n_retry_pg;
+    f3 += st.n_unphys_final;
+    f4 += st.newton_iters;
+    ms = std::max(ms, st.max_speed);
+  }
+  if (stats) {
+    stats->n_c2p_fail = f1;
+    stats->n_retry_pg = f2;
+    stats->n_unphys_final = f3;
+    stats->newton_iters = f4;
+    stats->max_speed = ms;
+  }
+}
+
+void srhd_ref_grid_pad(const double* grid, double* padded, int nx, int ny, int nz, int g,
+                       const int* bc, const unsigned char* inflow_mask, const double* inflow_cons) {
+  const int sx = nx + 2 * g, sy = ny + 2 * g, sz = nz + 2 * g;
+  const size_t n = (size_t)nx * ny * nz, np = (size_t)sx * sy * sz;
+  for (int k = -g; k < nz + g; ++k)
+    for (int j = -g; j < ny + g; ++j)
+      for (int i = -g; i < nx + g; ++i) {
+        const int si = map_index(i, nx, bc[0], bc[1]);
+        const int sj = map_index(j, ny, bc[2], bc[3]);
+        const int sk = map_index(k, nz, bc[4], bc[5]);
+        const size_t dst = ((size_t)(k + g) * sy + (j + g)) * sx + (i + g);
+        const bool inflow = inflow_mask && k < 0 && inflow_mask[(size_t)sj * nx + si];
+        for (int q = 0; q < 5; ++q)
+          padded[q * np + dst] = inflow ? inflow_cons[q] : grid[q * n + ((size_t)sk * ny + sj) * nx + si];
+      }
+}
+
+void srhd_ref_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int g,
+                          const int* bc, const unsigned char* inflow_mask,
+                          const double* inflow_cons) {
+  const int nxt = 16 + 2 * g;
+  const int px = nx / 16, py = ny / 16, pz = nz / 16;
+  const size_t n = (size_t)nx * ny * nz, t3 = (size_t)nxt * nxt * nxt;
+#pragma omp parallel for schedule(static)
+  for (int pg = 0; pg < px * py * pz; ++pg) {
+    const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+    double* tile = cons_in + (size_t)pg * 5 * t3;
+    for (int k = 0; k < nxt; ++k)
+      for (int j = 0; j < nxt; ++j)
+        for (int i = 0; i < nxt; ++i) {
+          const int kk = gz * 16 + k - g;
+          const int si = map_index(gx * 16 + i - g, nx, bc[0], bc[1]);
+          const int sj = map_index(gy * 16 + j - g, ny, bc[2], bc[3]);
+          const int sk = map_index(kk, nz, bc[4], bc[5]);
+          const bool inflow = inflow_mask && kk < 0 && inflow_mask[(size_t)sj * nx + si];
+          for (int q = 0; q < 5; ++q)
+            tile[q * t3 + ((size_t)k * nxt + j) * nxt + i] =
+                inflow ? inflow_cons[q] : grid[q * n + ((size_t)sk * ny + sj) * nx + si];
+        }
+  }
+}
+
+void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz) {
+  const int px = nx / 16, py = ny / 16, pz = nz / 16;
+  const size_t n = (size_t)nx * ny * nz;
+#pragma omp parallel for schedule(static)
+  for (int pg = 0; pg < px * py * pz; ++pg) {
+    const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+    const double* src = cons_out + (size_t)pg * 8 * 5 * 512;
+    for (int p = 0; p < 8; ++p)
+      for (int q = 0; q < 5; ++q)
+        for (int k = 0; k < 8; ++k)
+          for (int j = 0; j < 8; ++j)
+            for (int i = 0; i < 8; ++i) {
+              const int I = gx * 16 + (p & 1) * 8 + i, J = gy * 16 + ((p >> 1) & 1) * 8 + j,
+                        Kk = gz * 16 + (p >> 2) * 8 + k;
+              grid[q * n + ((size_t)Kk * ny + J) * nx + I] = src[((size_t)p * 5 + q) * 512 + k * 64 + j * 8 + i];
+            }
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,99 @@
+// oracle/srhd_ref.hpp
+//
+// TEST INFRASTRUCTURE ONLY.  Plain, slow, fp64 CPU oracle for the GAMER-SR hot path
+// (arXiv 2012.11130).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may build, link, import or call anything in oracle/.  It shares no code,
+// header, table or helper with the CUDA path in paper_2012_11130_b200/csrc.
+//
+// Citations: "P:n" = /root/reference/PAPER.md line n; "S#/G#" = reading listed in DESIGN.md.
+// Units c = k_B = m = 1.  T == Theta == p/rho (Eq. 18).
+//
+// State vectors:
+//   primitive W = (rho, U^x, U^y, U^z, p)   -- FOUR-velocity (Eq. 8)
+//   conserved U = (D, M^x, M^y, M^z, Etilde) -- REDUCED energy Etilde = E - D (Eq. 6)
+// SoA convention of the C entry points: component c of state i at ptr[c*stride + i].
+//
+// Pin status (see tests/test_oracle_*.py and DESIGN.md "Oracle pins"):
+//   EoS, prim2cons, cons2prim, max speed, HLLE/HLLC, PLM/PPM, fluid step: pinned.
+//   Retry ladder (K, beta0, granularity = patch group; S3/S9) and the PPM/limiter details (S3/S4):
+//   "parity unpinned" against the paper -- the paper is silent; pinned only by textbook properties.
+#pragma once
+#include <cstddef>
+
+extern "C" {
+
+struct srhd_ref_params {
+  int    recon;            // 0 PLM, 1 PPM                           (PPM per BASELINE.json)
+  int    riemann;          // 0 HLLE, 1 HLLC
+  double minmod_coeff;     // beta0 in [1,2]                         (value: reading S3)
+  int    max_retry;        // K reductions by 0.75, then beta = 0    (K: reading S9)
+  double newton_rtol;      // stop when |delta| <= rtol*|htilde|     (reading S2)
+  int    newton_max_iter;  // iteration cap                          (reading S2)
+  int    ghost;            // 2 (PLM) or 3 (PPM)
+};
+
+struct srhd_ref_stats {
+  unsigned long long n_c2p_fail;      // Eq. 30 violations on input to a conversion
+  unsigned long long n_retry_pg;      // patch groups that needed >= 1 retry
+  unsigned long long n_unphys_final;  // output cells still violating Eq. 30 in the accepted pass
+  unsigned long long newton_iters;    // total Newton iterations (informational)
+  double             max_speed;       // max S_max (Eq. 27) over the input interior cells
+};
+
+// --- O1 EoS (Eq. 10, Eq. 22, Eq. 16, Eq. 14) --------------------------
+double srhd_ref_htilde_of_T(double T);
+double srhd_ref_T_of_htilde(double ht);
+double srhd_ref_dT_dhtilde(double ht);                       // P:591 Eq. A2
+double srhd_ref_cs2_of_T(double T);                          // P:129 Eq. 14 (squared)
+double srhd_ref_f_eq15(double ht, double musq);              // P:140-144 Eq. 15 right-hand side
+double srhd_ref_df_eqA1(double ht, double musq);             // P:587 Eq. A1
+double srhd_ref_htilde_guess(double L, double musq);         // P:602-618 Eq. A4 (reading G2), A6, A7
+
+// --- O2/O3 conversions on n SoA states; all pointers are HOST pointers --------------------------
+void srhd_ref_prim2cons(const double* prim, double* cons, size_t n, size_t stride);
+void srhd_ref_cons2prim(const double* cons, double* prim, size_t n, size_t stride,
+                        const srhd_ref_params* par, srhd_ref_stats* stats);
+// optional diagnostics: per-state root htilde, iteration count and Eq.-30 flag (may be null)
+void srhd_ref_cons2prim_diag(const double* cons, double* prim, size_t n, size_t stride,
+                             const srhd_ref_params* par, double* htilde, int* iters,
+                             unsigned char* unphys);
+
+// --- O4 time step (Eq. 26-28) -------------------------------------------------------
+// per-state U_max (Eq. 26, reading G1) from PRIMITIVES, and S_max = U_max/sqrt(1+U_max^2) (Eq. 27)
+double srhd_ref_umax_of_prim(const double W[5]);
+double srhd_ref_smax_of_umax(double umax);
+void   srhd_ref_max_signal_speed(const double* cons, size_t n, size_t stride,
+                                 const srhd_ref_params* par, double* max_speed);
+
+// --- O5-O9 one fluid step ---------------------------------------------------------------------
+// Box form: cons_in [5][nz+2g][ny+2g][nx+2g] (x fastest) -> cons_out [5][nz][ny][nx].
+// Retry granularity = the whole box.  Returns the number of passes used (1 = no retry).
+int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz,
+                      double dt, double dh, const srhd_ref_params* par, srhd_ref_stats* stats);
+// Patch-group form (the C-ABI shape of SURVEY.md 8b):
+//   cons_in  [npg][5][nxt][nxt][nxt], nxt = 16 + 2*ghost
+//   cons_out [npg][8][5][8][8][8],    patch p = ix + 2*iy + 4*iz   (reading S13)
+void srhd_ref_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+                         const srhd_ref_params* par, srhd_ref_stats* stats, int nthreads);
+
+// single Riemann flux along direction dir (0,1,2), for tests: WL/UL/WR/UR are 5-vectors
+void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL,
+                           const double* WR, const double* UR, double* F);
+// physical flux along dir (Eq. 4a, 4b; Eq. 7)
+void srhd_ref_phys_flux(int dir, const double* W, const double* U, double* F);
+// limited slope (reading S3) and 1-D face reconstruction of one component for tests:
+double srhd_ref_limited_slope(double sL, double sR, double beta);
+void   srhd_ref_recon_1d(int recon, const double* a /*5 values: i-2..i+2*/, double beta,
+                         double beta0, double* am, double* ap);
+
+// --- O10 uniform-grid helpers -------------------------------------------------------------------
+// grid [5][nz][ny][nx].  bc[6] = {x_lo,x_hi,y_lo,y_hi,z_lo,z_hi}: 0 periodic, 1 outflow (copy).
+// inflow_mask (may be null): [ny][nx] bytes; ghost cells with k<0 whose (wrapped/clamped) (i,j)
+// has mask!=0 hold inflow_cons[5] (fixed inflow at the z_lo face), outflow elsewhere.
+void srhd_ref_grid_pad(const double* grid, double* padded, int nx, int ny, int nz, int g,
+                       const int* bc, const unsigned char* inflow_mask, const double* inflow_cons);
+void srhd_ref_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int g,
+                          const int* bc, const unsigned char* inflow_mask,
+                          const double* inflow_cons);
+void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz);
+}
