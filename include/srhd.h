@@ -1,0 +1,134 @@
+/* include/srhd.h -- C ABI of the B200-native GAMER-SR hot path (arXiv 2012.11130).
+ *
+ * One data-parallel path of the paper: the per-patch-group special-relativistic hydrodynamics
+ * update with the Taub-Mathews equation of state, in fp64, as hand-written CUDA for sm_100a.
+ *
+ * Citations: "P:n" = line n of the paper text; "S#"/"G#" = readings listed in
+ * DESIGN.md section 4.  Units c = k_B = m = 1.
+ *
+ * State vectors (Eq. 5-8, "equations actually solved"):
+ *   primitive  W = (rho, U^x, U^y, U^z, p)       -- U^i is the FOUR-velocity (Eq. 8)
+ *   conserved  U = (D, M^x, M^y, M^z, Etilde)    -- Etilde = E - D, the REDUCED energy (Eq. 6)
+ *
+ * Conventions common to every call
+ *   - every data pointer is a DEVICE pointer owned by the caller (allocate / free is the caller's
+ *     job; the library keeps no state between calls).  `const srhd_params*` is a HOST pointer and is
+ *     read before the call returns.  `srhd_stats*` / `double* d_max_speed` are DEVICE pointers.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream); every call is
+ *     asynchronous on that stream and returns after the launch.
+ *   - SoA state lists: component c of state i lives at ptr[c*stride + i], stride >= n (in doubles).
+ *   - return value: 0 = OK; negative = bad argument (SRHD_ERR_*); positive = a cudaError_t raised by
+ *     the launch.  UNPHYSICAL STATES ARE NOT ERRORS: they are counted in srhd_stats and evaluated
+ *     by the deterministic rules S9/S10/S15 so that results are reproducible.
+ *   - n == 0 / npg == 0 is a no-op that returns 0 (stats are still zeroed).
+ *   - there is no CPU fallback: without a CUDA device every compute call returns a cudaError_t.
+ */
+#ifndef SRHD_H_
+#define SRHD_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SRHD_OK                 0
+#define SRHD_ERR_NULL_POINTER  (-1)
+#define SRHD_ERR_BAD_PARAMS    (-2)   /* recon/riemann out of range, ghost != 2 (PLM) / 3 (PPM), ... */
+#define SRHD_ERR_BAD_SIZE      (-3)   /* stride < n, negative npg, grid extent not a multiple of 16 */
+#define SRHD_ERR_BAD_STEP      (-4)   /* dt <= 0 or dh <= 0 (or not finite)                         */
+#define SRHD_ERR_ALIAS         (-5)   /* cons_in and cons_out overlap                               */
+#define SRHD_ERR_BAD_ALIGN     (-6)   /* cons_in not 16-byte aligned (TMA bulk copies need it)      */
+
+#define SRHD_RECON_PLM   0
+#define SRHD_RECON_PPM   1
+#define SRHD_RIEMANN_HLLE 0
+#define SRHD_RIEMANN_HLLC 1
+
+#define SRHD_BC_PERIODIC 0
+#define SRHD_BC_OUTFLOW  1
+
+/* Run-time parameters of the solver (values the paper leaves open are the
+ * readings S2, S3, S9 of DESIGN.md). */
+typedef struct {
+  int    recon;            /* SRHD_RECON_PLM or SRHD_RECON_PPM (BASELINE.json configs 3, 5)   */
+  int    riemann;          /* SRHD_RIEMANN_HLLE or SRHD_RIEMANN_HLLC                          */
+  double minmod_coeff;     /* beta0 in [1,2], "original minmod coefficient"; default 1.5 (S3) */
+  int    max_retry;        /* K reductions of beta by 0.75, then beta = 0; default 8 (S9)     */
+  double newton_rtol;      /* Newton-Raphson stop: |delta| <= rtol*|htilde|; default 1e-15 (S2)       */
+  int    newton_max_iter;  /* iteration cap; default 20 (S2)                                          */
+  int    ghost;            /* ghost width of cons_in: must be 2 for PLM, 3 for PPM                    */
+} srhd_params;
+
+/* Per-call counters, DEVICE resident, zeroed by the callee at call start (on the stream). */
+typedef struct {
+  unsigned long long n_c2p_fail;      /* states violating Eq. 30 on input to a conversion:
+                                         srhd_cons2prim: every failing state; srhd_fluid_step: failing
+                                         input interior cells + failing half-step face states of the
+                                         accepted beta = 0 pass (S15)                                 */
+  unsigned long long n_retry_pg;      /* patch groups that needed >= 1 retry pass         */
+  unsigned long long n_unphys_final;  /* updated cells still violating Eq. 30 after beta = 0 (S10)    */
+  unsigned long long newton_iters;    /* total Newton-Raphson iterations (for the flop model)         */
+  double             max_speed;       /* max S_max (Eq. 27) over the INPUT interior cells       */
+} srhd_stats;
+
+/* Fill *p with the defaults above for the given recon / riemann choice (host pointer). */
+void srhd_default_params(srhd_params* p, int recon, int riemann);
+
+/* prim -> cons for n independent states (Fig. 15 right; Eq. 5a-b; Eq. 22-23).
+ * prim, cons: device, SoA with `stride`; the two arrays must not overlap. */
+int srhd_prim2cons(const double* prim, double* cons, size_t n, size_t stride, void* stream);
+
+/* cons -> prim for n independent states (Fig. 15 left; Eq. 15-18; App. A):
+ * Newton-Raphson on htilde = h - 1 from the two-branch guess A4/A6, canonical left-hand side
+ * L = fma(x, x+2, -mu^2).  A state that fails Eq. 30 is counted in
+ * stats->n_c2p_fail and evaluated with L <- eps_machine (S10).  stats may be NULL. */
+int srhd_cons2prim(const double* cons, double* prim, size_t n, size_t stride,
+                   const srhd_params* params, srhd_stats* stats, void* stream);
+
+/* CFL signal speed (Eq. 24-28; G1): *d_max_speed = S_max(max_i U_max,i) with
+ * U_max = gamma_s (|U^x|+|U^y|+|U^z|) + 3 gamma U_s from cons2prim of each state.  The time step is
+ * dt = C_CFL * dh / *d_max_speed (Eq. 28), formed by the caller.  n == 0 gives 0. */
+int srhd_max_signal_speed(const double* cons, size_t n, size_t stride,
+                          const srhd_params* params, double* d_max_speed, void* stream);
+
+/* One MUSCL-Hancock step (readings S3-S7, S9-S15) of npg patch groups.
+ *   cons_in : [npg][5][nxt][nxt][nxt] doubles, nxt = 16 + 2*ghost, x fastest: the 16^3 interior
+ *             cells of the patch group (2^3 patches of 8^3 cells) plus `ghost` layers of
+ *             ghost zones on every side, already filled by the caller (srhd_grid_gather below, or
+ *             an AMR driver -- P:219).
+ *   cons_out: [npg][8][5][8][8][8] doubles: patch p = ix + 2*iy + 4*iz (S13), component, z, y, x.
+ *   dt, dh  : time step and cell size.
+ * Per patch group: cons2prim of every tile cell -> PLM/PPM edge values on primitives -> Hancock
+ * half step -> cons2prim of both states at every face -> HLLE/HLLC flux -> flux-difference update
+ * -> Eq. 30 check; if any interior cell or face state of the group fails, the whole group is redone
+ * with beta <- 0.75 beta, after max_retry reductions with beta = 0, whose result is accepted.
+ * cons_in and cons_out must not overlap.  stats may be NULL. */
+int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+                    const srhd_params* params, srhd_stats* stats, void* stream);
+
+/* Bytes of caller-provided scratch srhd_fluid_step needs: 0, the step is fully fused. */
+size_t srhd_workspace_bytes(int npg, const srhd_params* params);
+
+/* Harness helpers for a uniform grid (reading S11, S13; NOT part of the paper's solver: they stand in
+ * for the AMR driver's ghost-zone fill).  grid: [5][nz][ny][nx] conserved, extents multiples
+ * of 16.  bc[6] (HOST pointer) = {x-lo, x-hi, y-lo, y-hi, z-lo, z-hi}, each SRHD_BC_PERIODIC (wrap)
+ * or SRHD_BC_OUTFLOW (copy the nearest interior cell).  inflow_mask (device, [ny][nx] bytes, may be
+ * NULL): ghost cells below z = 0 whose column is marked hold inflow_cons[5] (HOST pointer) instead.
+ * Patch group pg = gx + (nx/16)*(gy + (ny/16)*gz). */
+int srhd_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int ghost,
+                     const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
+                     void* stream);
+int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz, void* stream);
+
+/* Human-readable text for a return code of this library (negative) or of CUDA (positive). */
+const char* srhd_error_string(int code);
+
+/* 1 if this build reproduces the reference operation order without fused multiply-add contraction
+ * (libsrhd_b200_exact.so, used by the bit-parity tests), 0 for the production build. */
+int srhd_build_is_exact(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SRHD_H_ */

@@ -1,0 +1,214 @@
+"""Thin Python binding of the C-ABI library (include/srhd.h): argument marshalling only.
+
+Every function here has the name of the C entry point it calls and does nothing but check tensor
+dtype/device/contiguity, allocate the output with torch, and pass raw device pointers plus the
+current CUDA stream.  All arithmetic runs in the CUDA kernels of libsrhd_b200.so.  There is no CPU
+fallback: if the library is missing or no CUDA device is present, the calls raise.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+_D = C.c_double
+_VP = C.c_void_p
+
+RECON = {"plm": 0, "ppm": 1}
+RIEMANN = {"hlle": 0, "hllc": 1}
+BC = {"periodic": 0, "outflow": 1}
+
+
+class Params(C.Structure):
+    """srhd_params (include/srhd.h)."""
+    _fields_ = [("recon", C.c_int), ("riemann", C.c_int), ("minmod_coeff", C.c_double),
+                ("max_retry", C.c_int), ("newton_rtol", C.c_double), ("newton_max_iter", C.c_int),
+                ("ghost", C.c_int)]
+
+
+class Stats(C.Structure):
+    """srhd_stats (include/srhd.h); lives in device memory, read back with stats_to_host()."""
+    _fields_ = [("n_c2p_fail", C.c_ulonglong), ("n_retry_pg", C.c_ulonglong),
+                ("n_unphys_final", C.c_ulonglong), ("newton_iters", C.c_ulonglong),
+                ("max_speed", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
+           "srhd_fluid_step", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
+           "srhd_error_string", "srhd_build_is_exact"]
+
+_LIBS = {}
+
+
+class SrhdError(RuntimeError):
+    pass
+
+
+def load_library(exact=False):
+    """dlopen libsrhd_b200[_exact].so (built in-tree by paper_2012_11130_b200.build)."""
+    if exact in _LIBS:
+        return _LIBS[exact]
+    path = _build.lib_path(exact)
+    if not os.path.exists(path):
+        raise SrhdError(f"{path} is missing: run `python -m paper_2012_11130_b200.build` "
+                        "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    L.srhd_default_params.restype = None
+    L.srhd_default_params.argtypes = [C.POINTER(Params), C.c_int, C.c_int]
+    L.srhd_prim2cons.restype = C.c_int
+    L.srhd_prim2cons.argtypes = [_VP, _VP, C.c_size_t, C.c_size_t, _VP]
+    L.srhd_cons2prim.restype = C.c_int
+    L.srhd_cons2prim.argtypes = [_VP, _VP, C.c_size_t, C.c_size_t, C.POINTER(Params), _VP, _VP]
+    L.srhd_max_signal_speed.restype = C.c_int
+    L.srhd_max_signal_speed.argtypes = [_VP, C.c_size_t, C.c_size_t, C.POINTER(Params), _VP, _VP]
+    L.srhd_fluid_step.restype = C.c_int
+    L.srhd_fluid_step.argtypes = [_VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
+    L.srhd_workspace_bytes.restype = C.c_size_t
+    L.srhd_workspace_bytes.argtypes = [C.c_int, C.POINTER(Params)]
+    L.srhd_grid_gather.restype = C.c_int
+    L.srhd_grid_gather.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), _VP,
+                                   C.POINTER(C.c_double), _VP]
+    L.srhd_grid_scatter.restype = C.c_int
+    L.srhd_grid_scatter.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, _VP]
+    L.srhd_error_string.restype = C.c_char_p
+    L.srhd_error_string.argtypes = [C.c_int]
+    L.srhd_build_is_exact.restype = C.c_int
+    L.srhd_build_is_exact.argtypes = []
+    _LIBS[exact] = L
+    return L
+
+
+def params(recon="plm", riemann="hllc", minmod_coeff=None, max_retry=None, newton_rtol=None,
+           newton_max_iter=None, exact=False):
+    """srhd_default_params + overrides."""
+    p = Params()
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    s = RIEMANN[riemann] if isinstance(riemann, str) else int(riemann)
+    load_library(exact).srhd_default_params(C.byref(p), r, s)
+    if minmod_coeff is not None:
+        p.minmod_coeff = minmod_coeff
+    if max_retry is not None:
+        p.max_retry = max_retry
+    if newton_rtol is not None:
+        p.newton_rtol = newton_rtol
+    if newton_max_iter is not None:
+        p.newton_max_iter = newton_max_iter
+    return p
+
+
+def _check(code, L):
+    if code != 0:
+        raise SrhdError(f"srhd error {code}: {L.srhd_error_string(code).decode()}")
+
+
+def _dev(t, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise SrhdError(f"{name} must be a contiguous float64 CUDA tensor (no CPU fallback)")
+    return t
+
+
+def _stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+def new_stats(device="cuda"):
+    """Device buffer holding one srhd_stats (40 bytes)."""
+    return torch.zeros(C.sizeof(Stats), dtype=torch.uint8, device=device)
+
+
+def stats_to_host(stats_buf):
+    """One small device->host copy; returns a Stats struct."""
+    raw = stats_buf.cpu().numpy().tobytes()
+    return Stats.from_buffer_copy(raw)
+
+
+def prim2cons(prim, cons=None, exact=False):
+    """srhd_prim2cons on a (5, n) SoA tensor."""
+    L = load_library(exact)
+    prim = _dev(prim, "prim")
+    n = prim.shape[1]
+    cons = torch.empty_like(prim) if cons is None else _dev(cons, "cons")
+    _check(L.srhd_prim2cons(prim.data_ptr(), cons.data_ptr(), n, prim.stride(0) if n else 0, _stream()), L)
+    return cons
+
+
+def cons2prim(cons, par=None, prim=None, stats=None, exact=False):
+    """srhd_cons2prim on a (5, n) SoA tensor; returns (prim, stats device buffer)."""
+    L = load_library(exact)
+    cons = _dev(cons, "cons")
+    par = par or params(exact=exact)
+    n = cons.shape[1]
+    prim = torch.empty_like(cons) if prim is None else _dev(prim, "prim")
+    stats = new_stats(cons.device) if stats is None else stats
+    _check(L.srhd_cons2prim(cons.data_ptr(), prim.data_ptr(), n, cons.stride(0) if n else 0, C.byref(par),
+                            stats.data_ptr(), _stream()), L)
+    return prim, stats
+
+
+def max_signal_speed(cons, par=None, out=None, exact=False):
+    """srhd_max_signal_speed on a (5, n) SoA tensor; returns a 1-element device tensor."""
+    L = load_library(exact)
+    cons = _dev(cons, "cons")
+    par = par or params(exact=exact)
+    n = cons.shape[1]
+    out = torch.empty(1, dtype=torch.float64, device=cons.device) if out is None else out
+    _check(L.srhd_max_signal_speed(cons.data_ptr(), n, cons.stride(0) if n else 0, C.byref(par),
+                                   out.data_ptr(), _stream()), L)
+    return out
+
+
+def fluid_step(cons_in, dt, dh, par, cons_out=None, stats=None, exact=False):
+    """srhd_fluid_step: cons_in (npg,5,nxt,nxt,nxt) -> cons_out (npg,8,5,8,8,8); returns (cons_out, stats)."""
+    L = load_library(exact)
+    cons_in = _dev(cons_in, "cons_in")
+    npg = cons_in.shape[0]
+    nxt = 16 + 2 * par.ghost
+    if tuple(cons_in.shape) != (npg, 5, nxt, nxt, nxt):
+        raise SrhdError(f"cons_in must have shape (npg,5,{nxt},{nxt},{nxt})")
+    if cons_out is None:
+        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=torch.float64, device=cons_in.device)
+    stats = new_stats(cons_in.device) if stats is None else stats
+    _check(L.srhd_fluid_step(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(), npg, float(dt),
+                             float(dh), C.byref(par), stats.data_ptr(), _stream()), L)
+    return cons_out, stats
+
+
+def _bc(bc):
+    return (C.c_int * 6)(*[BC[b] if isinstance(b, str) else int(b) for b in bc])
+
+
+def grid_gather(grid, ghost, bc, inflow=None, cons_in=None, exact=False):
+    """srhd_grid_gather: grid (5,nz,ny,nx) -> cons_in (npg,5,nxt,nxt,nxt).
+    inflow = (mask uint8 CUDA tensor (ny,nx), cons 5 floats) or None."""
+    L = load_library(exact)
+    grid = _dev(grid, "grid")
+    _, nz, ny, nx = grid.shape
+    npg = (nx // 16) * (ny // 16) * (nz // 16)
+    nxt = 16 + 2 * ghost
+    if cons_in is None:
+        cons_in = torch.empty((npg, 5, nxt, nxt, nxt), dtype=torch.float64, device=grid.device)
+    mask_ptr, icons = None, None
+    if inflow is not None:
+        mask, vals = inflow
+        if not (mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous()):
+            raise SrhdError("inflow mask must be a contiguous uint8 CUDA tensor")
+        mask_ptr = mask.data_ptr()
+        icons = (C.c_double * 5)(*[float(v) for v in vals])
+    _check(L.srhd_grid_gather(grid.data_ptr(), cons_in.data_ptr(), nx, ny, nz, ghost, _bc(bc), mask_ptr,
+                              icons, _stream()), L)
+    return cons_in
+
+
+def grid_scatter(cons_out, shape, grid=None, exact=False):
+    """srhd_grid_scatter: cons_out (npg,8,5,8,8,8) -> grid (5,nz,ny,nx)."""
+    L = load_library(exact)
+    cons_out = _dev(cons_out, "cons_out")
+    nz, ny, nx = shape
+    if grid is None:
+        grid = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=cons_out.device)
+    _check(L.srhd_grid_scatter(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, _stream()), L)
+    return grid

@@ -1,0 +1,461 @@
+// srhd_fluid.cu -- srhd_fluid_step: one fused kernel per batch of patch groups.
+//
+// One CTA advances one patch group (16^3 interior cells + ghost zones) and marches through
+// its z planes, keeping all three directional sweeps on chip:
+//   phase 1  plane s of the conserved tile arrives in shared memory by TMA bulk copies
+//            (cp.async.bulk + mbarrier) and is converted IN PLACE to primitives (cons2prim, Eq. 15-18);
+//            input-interior cells also feed the CFL reduction (Eq. 26) and the Eq. 30 counter;
+//   phase 2  plane kh = s - 2g + 1: PLM/PPM edge values in x, y (same plane) and z (ring of 2g-1
+//            primitive planes), prim2cons + physical fluxes of the six edge states, the common
+//            Hancock increment, evolved edge states to shared memory;
+//   phase 3  one Riemann problem per face of plane kh (x: 17x16, y: 16x17) and per z face between
+//            kh-1 and kh (16x16): cons2prim of both sides (two Newton chains per lane), HLLE/HLLC;
+//            the thread that owns column (i,j) then updates cell (i,j,kh-1), checks Eq. 30 and stores.
+// If any face state or updated cell of the group fails Eq. 30 the CTA repeats the march with
+// beta <- 0.75 beta, finally with beta = 0.  Each cell's state crosses HBM once on the way
+// in (plus ghost layers) and once on the way out; the update re-reads its own cell through L2.
+#include "srhd_common.cuh"
+
+namespace srhd {
+
+constexpr int kFluidThreads = 512;   // 16 warps, <= 128 registers per thread, one CTA per SM
+
+// ---- TMA bulk copy + mbarrier (PTX; SASS: UBLKCP / SYNCS) -------------------------------------
+SRHD_DEV uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+SRHD_DEV void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+SRHD_DEV void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+SRHD_DEV bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+SRHD_DEV void mbar_wait(uint64_t* bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {
+  }
+}
+SRHD_DEV void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+SRHD_DEV void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ---- shared-memory plan -----------------------------------------------------------------------
+template <int G>
+struct Plan {
+  static constexpr int NXT = 16 + 2 * G;      // tile extent
+  static constexpr int PL = NXT * NXT;        // cells per tile plane
+  static constexpr int T3 = PL * NXT;         // cells per tile component
+  static constexpr int R = 2 * G - 1;         // primitive planes kept (z stencil of the reconstruction)
+  static constexpr int XS = 16 * 18;          // x edge states: row j in 0..15, cell i in -1..16
+  static constexpr int YS = 18 * 16;          // y edge states: cell j in -1..16, column i in 0..15
+  static constexpr int ZS = 256;              // z edge states: interior columns
+  static constexpr int NFXY = 272;            // faces per plane along x (17x16) and along y (16x17)
+  // offsets in doubles
+  static constexpr int oW = 0;
+  static constexpr int oXSm = oW + R * 5 * PL;
+  static constexpr int oXSp = oXSm + 5 * XS;
+  static constexpr int oYSm = oXSp + 5 * XS;
+  static constexpr int oYSp = oYSm + 5 * YS;
+  static constexpr int oZSm = oYSp + 5 * YS;
+  static constexpr int oZSp = oZSm + 5 * ZS;          // two buffers (plane parity)
+  static constexpr int oFX = oZSp + 2 * 5 * ZS;
+  static constexpr int oFY = oFX + 5 * NFXY;
+  static constexpr int oCtl = oFY + 5 * NFXY;         // control block: 8 x 8 bytes
+  static constexpr int nDoubles = oCtl + 8;
+  static constexpr size_t bytes = (size_t)nDoubles * sizeof(double);
+};
+
+struct Ctl {                       // lives in shared memory
+  uint64_t mbar;
+  unsigned long long newton;
+  unsigned long long umax_bits;
+  unsigned int face_fail, cell_fail, in_fail, pad;
+};
+
+// Edge states of one cell along direction d: reconstruction of the five primitives, prim2cons of
+// both edges, physical fluxes; returns dF = F(W+) - F(W-) and the un-evolved conserved edge states.
+template <int G, int d>
+SRHD_DEV void hancock_dir(const double* __restrict__ Wr, int tk, int cidx, double beta, double beta0,
+                          double um[5], double up[5], double dF[5]) {
+  using P = Plan<G>;
+  double wm[5], wp[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    double a[2 * G - 1];
+#pragma unroll
+    for (int m = -(G - 1); m <= G - 1; ++m) {
+      int off;
+      if (d == 0) off = ((tk % P::R) * 5 + q) * P::PL + cidx + m;
+      else if (d == 1) off = ((tk % P::R) * 5 + q) * P::PL + cidx + m * P::NXT;
+      else off = (((tk + m) % P::R) * 5 + q) * P::PL + cidx;
+      a[m + G - 1] = Wr[off];
+    }
+    if (G == 2) recon_plm(a, beta, wm[q], wp[q]);
+    else recon_ppm(a, beta, beta0, wm[q], wp[q]);
+  }
+  double Fm[5], Fp[5];
+  prim2cons(wm, um);
+  prim2cons(wp, up);
+  phys_flux<d>(wm, um, Fm);
+  phys_flux<d>(wp, up, Fp);
+#pragma unroll
+  for (int q = 0; q < 5; ++q) dF[q] = Fp[q] - Fm[q];
+}
+
+template <int G, int RS>
+__global__ void __launch_bounds__(kFluidThreads, 1)
+fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out, double dt, double dh,
+                  double beta0, int max_retry, double rtol, int max_iter, srhd_stats* __restrict__ stats) {
+  using P = Plan<G>;
+  constexpr int NT = kFluidThreads;
+  constexpr int NXT = P::NXT, PL = P::PL, T3 = P::T3, R = P::R;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* sm = reinterpret_cast<double*>(smem_raw);
+  double* Wr = sm + P::oW;
+  double* XSm = sm + P::oXSm;
+  double* XSp = sm + P::oXSp;
+  double* YSm = sm + P::oYSm;
+  double* YSp = sm + P::oYSp;
+  double* ZSm = sm + P::oZSm;
+  double* ZSp = sm + P::oZSp;
+  double* FX = sm + P::oFX;
+  double* FY = sm + P::oFY;
+  Ctl* ctl = reinterpret_cast<Ctl*>(sm + P::oCtl);
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const double* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
+  double* __restrict__ out = cons_out + (size_t)blockIdx.x * 8 * 5 * 512;
+
+  if (tid == 0) {
+    mbar_init(&ctl->mbar, 1);
+    ctl->newton = 0ull;
+    ctl->umax_bits = 0ull;
+    ctl->face_fail = ctl->cell_fail = ctl->in_fail = 0u;
+    fence_proxy_async();
+  }
+  __syncthreads();
+
+  const double hdt = dt / (2.0 * dh);
+  const double dtdh = dt / dh;
+  uint32_t parity = 0;
+  unsigned long long my_iters = 0;
+  unsigned my_in_fail = 0;
+  double my_umax = 0.0;
+  double beta = beta0;
+  int pass = 0;
+  unsigned n_face_fail = 0, n_cell_fail = 0;
+
+  for (;; ++pass) {
+    if (pass > 0) beta = (pass <= max_retry) ? beta * 0.75 : 0.0;
+    if (tid == 0) {
+      ctl->face_fail = 0u;
+      ctl->cell_fail = 0u;
+      fence_proxy_async();
+      mbar_expect_tx(&ctl->mbar, 5u * PL * 8u);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) bulk_g2s(Wr + q * PL, tile + (size_t)q * T3, PL * 8u, &ctl->mbar);
+    }
+    unsigned my_face_fail = 0, my_cell_fail = 0;
+    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // (Fx+ - Fx-) + (Fy+ - Fy-) of this thread's column cell
+    double fzp[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // z flux through the lower face of that cell
+
+    for (int s = 0; s < NXT; ++s) {
+      const int kh = s - 2 * G + 1;               // physical plane handled by phases 2 and 3
+
+      // ---- phase 1a: in-plane flux differences of plane kh-1 (fluxes written in the previous step)
+      if (tid < 256 && kh - 1 >= 0 && kh - 1 <= 15) {
+        const int i = tid & 15, j = tid >> 4;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          const double dfx = FX[q * P::NFXY + j * 17 + i + 1] - FX[q * P::NFXY + j * 17 + i];
+          const double dfy = FY[q * P::NFXY + (j + 1) * 16 + i] - FY[q * P::NFXY + j * 16 + i];
+          part[q] = dfx + dfy;
+        }
+      }
+
+      // ---- phase 1b: plane s has landed; conserved -> primitive in place
+      mbar_wait(&ctl->mbar, parity);
+      parity ^= 1u;
+      {
+        double* Ws = Wr + (s % R) * 5 * PL;
+        for (int base = warp * 32; base < PL; base += NT) {
+          const int item = base + lane;
+          const bool valid = item < PL;
+          const int c = valid ? item : PL - 1;
+          double U[1][5], W[1][5];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) U[0][q] = Ws[q * PL + c];
+          bool phys[1];
+          int it[1];
+          cons2prim_multi<1>(U, W, rtol, max_iter, phys, it);
+          if (valid) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) Ws[q * PL + c] = W[0][q];
+            if (pass == 0) {
+              my_iters += (unsigned)it[0];
+              const int ti = c % NXT, tj = c / NXT;
+              const bool interior = (ti >= G) && (ti < G + 16) && (tj >= G) && (tj < G + 16) && (s >= G) &&
+                                    (s < G + 16);
+              if (interior) {
+                if (!phys[0]) ++my_in_fail;
+                my_umax = fmax(my_umax, umax_of_prim(W[0]));
+              }
+            }
+          }
+        }
+      }
+      __syncthreads();
+
+      // ---- phase 2: edge states + Hancock half step of plane kh (S3-S5)
+      if (kh >= -1 && kh <= 16) {
+        const bool inplane = (kh >= 0) && (kh <= 15);
+        const int nh = inplane ? 320 : 256;
+        const int tk = kh + G;
+        const int zb = (kh + 2) & 1;
+        for (int item = tid; item < nh; item += NT) {
+          int i, j;
+          if (item < 256) {
+            i = item & 15;
+            j = item >> 4;
+          } else {
+            const int e = item - 256, side = e >> 4, t = e & 15;
+            i = (side == 0) ? -1 : ((side == 1) ? 16 : t);
+            j = (side == 2) ? -1 : ((side == 3) ? 16 : t);
+          }
+          const int cidx = (j + G) * NXT + (i + G);
+          const bool hasx = inplane && (j >= 0) && (j <= 15);
+          const bool hasy = inplane && (i >= 0) && (i <= 15);
+          const bool hasz = (item < 256);
+          const int ix = j * 18 + (i + 1);
+          const int iy = (j + 1) * 16 + i;
+          const int iz = item;            // j*16 + i when item < 256
+          double acc[5], um[5], up[5], dF[5];
+          hancock_dir<G, 0>(Wr, tk, cidx, beta, beta0, um, up, dF);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) acc[q] = dF[q];
+          if (hasx) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              XSm[q * P::XS + ix] = um[q];
+              XSp[q * P::XS + ix] = up[q];
+            }
+          }
+          hancock_dir<G, 1>(Wr, tk, cidx, beta, beta0, um, up, dF);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) acc[q] = acc[q] + dF[q];
+          if (hasy) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              YSm[q * P::YS + iy] = um[q];
+              YSp[q * P::YS + iy] = up[q];
+            }
+          }
+          hancock_dir<G, 2>(Wr, tk, cidx, beta, beta0, um, up, dF);
+          double dU[5];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dU[q] = -hdt * (acc[q] + dF[q]);
+          if (hasz) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              ZSm[q * P::ZS + iz] = um[q] + dU[q];
+              ZSp[(zb * 5 + q) * P::ZS + iz] = up[q] + dU[q];
+            }
+          }
+          if (hasx) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              XSm[q * P::XS + ix] = XSm[q * P::XS + ix] + dU[q];
+              XSp[q * P::XS + ix] = XSp[q * P::XS + ix] + dU[q];
+            }
+          }
+          if (hasy) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              YSm[q * P::YS + iy] = YSm[q * P::YS + iy] + dU[q];
+              YSp[q * P::YS + iy] = YSp[q * P::YS + iy] + dU[q];
+            }
+          }
+        }
+      }
+      __syncthreads();
+
+      // the oldest primitive plane is free now: prefetch conserved plane s+1 into its slot
+      if (tid == 0 && s + 1 < NXT) {
+        fence_proxy_async();
+        mbar_expect_tx(&ctl->mbar, 5u * PL * 8u);
+        double* dst = Wr + ((s + 1) % R) * 5 * PL;
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          bulk_g2s(dst + q * PL, tile + (size_t)q * T3 + (size_t)(s + 1) * PL, PL * 8u, &ctl->mbar);
+      }
+
+      // ---- phase 3: Riemann problems of plane kh, then the update of plane kh-1
+      if (kh >= 0 && kh <= 16) {
+        const int nf = (kh <= 15) ? (256 + 2 * P::NFXY) : 256;
+        const int zbl = (kh + 1) & 1;             // buffer of plane kh-1
+        for (int base = warp * 32; base < nf; base += NT) {
+          const int item = base + lane;
+          const bool valid = item < nf;
+          const int idx = valid ? item : nf - 1;
+          int d, qs;
+          const double *pL, *pR;
+          if (idx < 256) {
+            d = 2;
+            qs = P::ZS;
+            pL = ZSp + zbl * 5 * P::ZS + idx;
+            pR = ZSm + idx;
+          } else if (idx < 256 + P::NFXY) {
+            const int f = idx - 256, jj = f / 17, fi = f - jj * 17;
+            d = 0;
+            qs = P::XS;
+            pL = XSp + jj * 18 + fi;
+            pR = XSm + jj * 18 + fi + 1;
+          } else {
+            const int f = idx - 256 - P::NFXY;
+            d = 1;
+            qs = P::YS;
+            pL = YSp + f;
+            pR = YSm + f + 16;
+          }
+          double U[2][5], W[2][5], F[5];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            U[0][q] = pL[q * qs];
+            U[1][q] = pR[q * qs];
+          }
+          bool phys[2];
+          int it[2];
+          cons2prim_multi<2>(U, W, rtol, max_iter, phys, it);
+          riemann_flux<RS>(d, W[0], U[0], W[1], U[1], F);
+          if (valid) {
+            my_iters += (unsigned)(it[0] + it[1]);
+            my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
+            if (idx < 256) {
+              if (kh >= 1) {                        // update cell (i, j, kh-1): Eq. 4a, 4b, 7; S12
+                const int ku = kh - 1, i = idx & 15, j = idx >> 4;
+                const double* uin = tile + ((size_t)(ku + G) * NXT + (j + G)) * NXT + (i + G);
+                const int p = (i >> 3) + 2 * (j >> 3) + 4 * (ku >> 3);   // S13
+                double* o = out + (size_t)p * 5 * 512 + (ku & 7) * 64 + (j & 7) * 8 + (i & 7);
+                double Un[5];
+#pragma unroll
+                for (int q = 0; q < 5; ++q) {
+                  const double dfz = F[q] - fzp[q];
+                  Un[q] = __ldg(uin + (size_t)q * T3) - dtdh * (part[q] + dfz);
+                  o[q * 512] = Un[q];
+                }
+                if (!is_physical(Un)) ++my_cell_fail;                      // Eq. 30
+              }
+#pragma unroll
+              for (int q = 0; q < 5; ++q) fzp[q] = F[q];
+            } else if (idx < 256 + P::NFXY) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) FX[q * P::NFXY + (idx - 256)] = F[q];
+            } else {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) FY[q * P::NFXY + (idx - 256 - P::NFXY)] = F[q];
+            }
+          }
+        }
+      }
+      __syncthreads();
+    }
+
+    // ---- verdict of this pass for the whole patch group (S9, S10, S15)
+    my_face_fail = (unsigned)warp_sum(my_face_fail);
+    my_cell_fail = (unsigned)warp_sum(my_cell_fail);
+    if (lane == 0) {
+      if (my_face_fail) atomicAdd(&ctl->face_fail, my_face_fail);
+      if (my_cell_fail) atomicAdd(&ctl->cell_fail, my_cell_fail);
+    }
+    __syncthreads();
+    n_face_fail = ctl->face_fail;
+    n_cell_fail = ctl->cell_fail;
+    __syncthreads();
+    if ((n_face_fail == 0 && n_cell_fail == 0) || beta == 0.0) break;
+  }
+
+  // ---- per-call counters
+  my_iters = warp_sum(my_iters);
+  my_in_fail = (unsigned)warp_sum(my_in_fail);
+  my_umax = warp_max(my_umax);
+  if (lane == 0) {
+    atomicAdd(&ctl->newton, my_iters);
+    if (my_in_fail) atomicAdd(&ctl->in_fail, my_in_fail);
+    atomicMax(&ctl->umax_bits, (unsigned long long)__double_as_longlong(my_umax));
+  }
+  __syncthreads();
+  if (tid == 0 && stats) {
+    atomicAdd(&stats->newton_iters, ctl->newton);
+    const unsigned long long nf = (unsigned long long)ctl->in_fail + n_face_fail;
+    if (nf) atomicAdd(&stats->n_c2p_fail, nf);
+    if (n_cell_fail) atomicAdd(&stats->n_unphys_final, (unsigned long long)n_cell_fail);
+    if (pass > 0) atomicAdd(&stats->n_retry_pg, 1ull);
+    const double umax = __longlong_as_double((long long)ctl->umax_bits);
+    atomic_max_nonneg(&stats->max_speed, smax_of_umax(umax));      // Eq. 27 per group, then max
+  }
+}
+
+template <int G, int RS>
+int launch_fluid(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+                 const srhd_params* p, srhd_stats* stats, cudaStream_t st) {
+  auto kern = fluid_step_kernel<G, RS>;
+  const size_t smem = Plan<G>::bytes;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return (int)e;
+  kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, dt, dh, p->minmod_coeff, p->max_retry,
+                                         p->newton_rtol, p->newton_max_iter, stats);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace srhd
+
+using namespace srhd;
+
+extern "C" size_t srhd_workspace_bytes(int, const srhd_params*) { return 0; }
+
+extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+                               const srhd_params* params, srhd_stats* stats, void* stream) {
+  if (!cons_in || !cons_out) return SRHD_ERR_NULL_POINTER;
+  const int pc = check_params(params);
+  if (pc) return pc;
+  if (npg < 0) return SRHD_ERR_BAD_SIZE;
+  if (!(dt > 0.0) || !(dh > 0.0) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
+  if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & 7u))
+    return SRHD_ERR_BAD_ALIGN;
+  const int nxt = 16 + 2 * params->ghost;
+  const size_t in_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(double);
+  const size_t out_bytes = (size_t)npg * 8 * 5 * 512 * sizeof(double);
+  const uintptr_t a = reinterpret_cast<uintptr_t>(cons_in), b = reinterpret_cast<uintptr_t>(cons_out);
+  if (a < b + out_bytes && b < a + in_bytes) return SRHD_ERR_ALIAS;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (stats) {
+    const cudaError_t e = cudaMemsetAsync(stats, 0, sizeof(srhd_stats), st);
+    if (e != cudaSuccess) return (int)e;
+  }
+  if (npg == 0) return SRHD_OK;
+  if (params->recon == SRHD_RECON_PLM) {
+    return params->riemann == SRHD_RIEMANN_HLLE
+               ? launch_fluid<2, 0>(cons_in, cons_out, npg, dt, dh, params, stats, st)
+               : launch_fluid<2, 1>(cons_in, cons_out, npg, dt, dh, params, stats, st);
+  }
+  return params->riemann == SRHD_RIEMANN_HLLE
+             ? launch_fluid<3, 0>(cons_in, cons_out, npg, dt, dh, params, stats, st)
+             : launch_fluid<3, 1>(cons_in, cons_out, npg, dt, dh, params, stats, st);
+}

@@ -1,0 +1,127 @@
+// srhd_grid.cu -- uniform-grid harness helpers (S11, S13): ghost-zone fill into patch-group tiles and
+// the scatter of updated patches back to the grid.  They stand in for the AMR driver's ghost-zone
+// preparation, are pure data movement (no arithmetic) and are timed as part of a step.
+#include "srhd_common.cuh"
+
+namespace srhd {
+
+struct GridBC {
+  int bc[6];
+  double inflow[5];
+  int has_inflow;
+};
+
+// source index of ghost index i along an axis of n cells (S11): periodic wraps, outflow clamps
+SRHD_DEV int map_index(int i, int n, int bc_lo, int bc_hi) {
+  if (i < 0) return (bc_lo == SRHD_BC_PERIODIC) ? ((i % n) + n) % n : 0;
+  if (i >= n) return (bc_hi == SRHD_BC_PERIODIC) ? (i % n) : n - 1;
+  return i;
+}
+
+// one CTA per (patch group, component): rows of nxt doubles, reads coalesced along x
+__global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restrict__ grid,
+                                                          double* __restrict__ cons_in, int nx, int ny,
+                                                          int nz, int g, GridBC b,
+                                                          const unsigned char* __restrict__ mask) {
+  const int nxt = 16 + 2 * g, t3 = nxt * nxt * nxt;
+  const int px = nx / 16, py = ny / 16;
+  const int pg = blockIdx.x, q = blockIdx.y;
+  const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+  const size_t n = (size_t)nx * ny * nz;
+  const double* __restrict__ src = grid + (size_t)q * n;
+  double* __restrict__ dst = cons_in + ((size_t)pg * 5 + q) * t3;
+  for (int c = threadIdx.x; c < t3; c += blockDim.x) {
+    const int i = c % nxt, j = (c / nxt) % nxt, k = c / (nxt * nxt);
+    const int kk = gz * 16 + k - g;
+    const int si = map_index(gx * 16 + i - g, nx, b.bc[0], b.bc[1]);
+    const int sj = map_index(gy * 16 + j - g, ny, b.bc[2], b.bc[3]);
+    const int sk = map_index(kk, nz, b.bc[4], b.bc[5]);
+    const bool inflow = b.has_inflow && kk < 0 && mask[(size_t)sj * nx + si];
+    dst[c] = inflow ? b.inflow[q] : __ldg(src + ((size_t)sk * ny + sj) * nx + si);
+  }
+}
+
+// one CTA per (patch group, component): 4096 cells, writes coalesced along x in 16-cell rows
+__global__ void __launch_bounds__(256) grid_scatter_kernel(const double* __restrict__ cons_out,
+                                                           double* __restrict__ grid, int nx, int ny,
+                                                           int nz) {
+  const int px = nx / 16, py = ny / 16;
+  const int pg = blockIdx.x, q = blockIdx.y;
+  const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+  const size_t n = (size_t)nx * ny * nz;
+  const double* __restrict__ src = cons_out + (size_t)pg * 8 * 5 * 512;
+  double* __restrict__ dst = grid + (size_t)q * n;
+  for (int c = threadIdx.x; c < 4096; c += blockDim.x) {
+    const int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
+    const int p = (i >> 3) + 2 * (j >> 3) + 4 * (k >> 3);
+    const double v = __ldg(src + ((size_t)p * 5 + q) * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7));
+    dst[((size_t)(gz * 16 + k) * ny + (gy * 16 + j)) * nx + (gx * 16 + i)] = v;
+  }
+}
+
+}  // namespace srhd
+
+using namespace srhd;
+
+static int check_extents(int nx, int ny, int nz) {
+  if (nx <= 0 || ny <= 0 || nz <= 0 || nx % 16 || ny % 16 || nz % 16) return SRHD_ERR_BAD_SIZE;
+  return SRHD_OK;
+}
+
+extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int ghost,
+                                const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
+                                void* stream) {
+  if (!grid || !cons_in || !bc) return SRHD_ERR_NULL_POINTER;
+  if (ghost != 2 && ghost != 3) return SRHD_ERR_BAD_PARAMS;
+  const int ce = check_extents(nx, ny, nz);
+  if (ce) return ce;
+  GridBC b;
+  for (int i = 0; i < 6; ++i) {
+    if (bc[i] != SRHD_BC_PERIODIC && bc[i] != SRHD_BC_OUTFLOW) return SRHD_ERR_BAD_PARAMS;
+    b.bc[i] = bc[i];
+  }
+  b.has_inflow = (inflow_mask != nullptr);
+  if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
+  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
+  const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  grid_gather_kernel<<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
+                                                                                   ghost, b, inflow_mask);
+  return (int)cudaGetLastError();
+}
+
+extern "C" int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz, void* stream) {
+  if (!cons_out || !grid) return SRHD_ERR_NULL_POINTER;
+  const int ce = check_extents(nx, ny, nz);
+  if (ce) return ce;
+  const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  grid_scatter_kernel<<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(cons_out, grid, nx, ny, nz);
+  return (int)cudaGetLastError();
+}
+
+extern "C" void srhd_default_params(srhd_params* p, int recon, int riemann) {
+  if (!p) return;
+  p->recon = recon;
+  p->riemann = riemann;
+  p->minmod_coeff = 1.5;
+  p->max_retry = 8;
+  p->newton_rtol = 1e-15;
+  p->newton_max_iter = 20;
+  p->ghost = (recon == SRHD_RECON_PLM) ? 2 : 3;
+}
+
+extern "C" const char* srhd_error_string(int code) {
+  switch (code) {
+    case SRHD_OK: return "ok";
+    case SRHD_ERR_NULL_POINTER: return "null pointer argument";
+    case SRHD_ERR_BAD_PARAMS: return "bad srhd_params (recon / riemann / ghost / coefficients)";
+    case SRHD_ERR_BAD_SIZE: return "bad size (stride < n, negative count, extent not a multiple of 16)";
+    case SRHD_ERR_BAD_STEP: return "dt and dh must be positive and finite";
+    case SRHD_ERR_ALIAS: return "cons_in and cons_out overlap";
+    case SRHD_ERR_BAD_ALIGN: return "cons_in must be 16-byte aligned";
+    default: break;
+  }
+  if (code > 0) return cudaGetErrorString(static_cast<cudaError_t>(code));
+  return "unknown srhd error code";
+}
+
+extern "C" int srhd_build_is_exact(void) { return SRHD_EXACT; }

@@ -1,0 +1,126 @@
+"""-m gpu parity: srhd_fluid_step (and the grid helpers) vs the CPU oracle on seeded patch groups.
+
+exact build: bit-identical output and identical counters (same IEEE operations, same decisions);
+production build: per-cell error (norm S14) <= 1e-11 after one step (north_star).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2012_11130_b200 import binding as B
+from paper_2012_11130_b200 import workloads as wl
+from tests.gpu_util import step_err
+
+pytestmark = pytest.mark.gpu
+TOL_STEP = 1e-11   # BASELINE.json north_star: relative error per cell after one step
+
+COMBOS = [("plm", "hlle"), ("plm", "hllc"), ("ppm", "hlle"), ("ppm", "hllc")]
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_tiles(ref, npg, ghost, seed, **kw):
+    prim = wl.random_patch_groups(npg, ghost, seed=seed, **kw)
+    nxt = 16 + 2 * ghost
+    cons = ref.prim2cons(prim.transpose(1, 0, 2, 3, 4).reshape(5, -1))
+    return np.ascontiguousarray(cons.reshape(5, npg, nxt, nxt, nxt).transpose(1, 0, 2, 3, 4))
+
+
+def cfl_dt(ref, tiles, dh, cfl=0.4):
+    return cfl * dh / ref.max_signal_speed(tiles.transpose(1, 0, 2, 3, 4).reshape(5, -1))
+
+
+@pytest.mark.parametrize("recon,riemann", COMBOS)
+def test_one_step_parity(ref, recon, riemann):
+    po = ref.params(recon, riemann)
+    npg, dh = 5, 1.0 / 64
+    tiles = make_tiles(ref, npg, po.ghost, seed=11 + po.ghost)
+    dt = cfl_dt(ref, tiles, dh)
+    want, st = ref.fluid_step(tiles, dt, dh, po)
+    # exact build: bit for bit, counters included
+    pe = B.params(recon, riemann, exact=True)
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, pe, exact=True)
+    s = B.stats_to_host(sbuf)
+    got = got.cpu().numpy()
+    assert np.array_equal(got, want), float(np.nanmax(step_err(got, want, 2)))
+    assert s.as_dict() == st.as_dict()
+    # production build: tolerance
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, B.params(recon, riemann))
+    s = B.stats_to_host(sbuf)
+    got = got.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    err = step_err(got, want, 2)
+    assert err.max() <= TOL_STEP, err.max()
+    assert (s.n_retry_pg, s.n_unphys_final, s.n_c2p_fail) == (st.n_retry_pg, st.n_unphys_final, st.n_c2p_fail)
+    assert abs(s.max_speed - st.max_speed) <= 1e-13 * st.max_speed
+
+
+@pytest.mark.parametrize("recon,riemann", [("plm", "hllc"), ("ppm", "hllc")])
+def test_retry_ladder_parity(ref, recon, riemann):
+    """A time step far above the CFL limit on rough, fast data forces Eq. 30 failures: the retry
+    decisions (per patch group, beta *= 0.75 ... then 0) must match the oracle's exactly."""
+    po = ref.params(recon, riemann, max_retry=3)
+    npg, dh = 4, 1.0 / 64
+    tiles = make_tiles(ref, npg, po.ghost, seed=5, umax=30.0, rough=3.0, log_theta=(-8.0, 2.0))
+    dt = 4.0 * cfl_dt(ref, tiles, dh)
+    want, st = ref.fluid_step(tiles, dt, dh, po)
+    assert st.n_retry_pg > 0, "test input must trigger the retry ladder"
+    pe = B.params(recon, riemann, max_retry=3, exact=True)
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, pe, exact=True)
+    s = B.stats_to_host(sbuf)
+    assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+    assert s.as_dict() == st.as_dict()
+
+
+def test_uniform_state_is_a_fixed_point(ref):
+    """All flux differences are x - x: bit-exact fixed point for any gamma, T (SURVEY 8c pin)."""
+    for recon in ("plm", "ppm"):
+        p = B.params(recon, "hllc")
+        nxt = 16 + 2 * p.ghost
+        W = np.array([0.7, 3.0e2, -1.0e2, 5.0e1, 1e-4])
+        prim = np.broadcast_to(W[:, None], (5, 2 * nxt ** 3)).copy()
+        cons = B.prim2cons(dev(prim))
+        tiles = cons.reshape(5, 2, nxt, nxt, nxt).permute(1, 0, 2, 3, 4).contiguous()
+        out, sbuf = B.fluid_step(tiles, 1e-3, 1e-2, p)
+        out = out.cpu().numpy()
+        c0 = cons[:, 0].cpu().numpy()
+        assert np.array_equal(out, np.broadcast_to(c0[None, None, :, None, None, None], out.shape))
+        assert B.stats_to_host(sbuf).n_retry_pg == 0
+
+
+def test_npg_zero_and_many(ref):
+    p = B.params("plm", "hlle")
+    e = torch.empty((0, 5, 20, 20, 20), dtype=torch.float64, device="cuda")
+    out, sbuf = B.fluid_step(e, 0.1, 1.0, p)
+    assert out.shape[0] == 0 and B.stats_to_host(sbuf).newton_iters == 0
+    # more patch groups than SMs (several waves, ragged last wave): sampled parity
+    po = ref.params("plm", "hlle")
+    base = make_tiles(ref, 3, 2, seed=3)
+    npg = 2 * 148 + 5
+    tiles = np.ascontiguousarray(base[np.arange(npg) % 3])
+    dt = cfl_dt(ref, base, 1.0 / 64)
+    want, _ = ref.fluid_step(base, dt, 1.0 / 64, po)
+    got, _ = B.fluid_step(dev(tiles), dt, 1.0 / 64, B.params("plm", "hlle", exact=True), exact=True)
+    got = got.cpu().numpy()
+    for pg in (0, 1, 2, 147, 148, 149, npg - 2, npg - 1):
+        assert np.array_equal(got[pg], want[pg % 3])
+
+
+@pytest.mark.parametrize("ghost", [2, 3])
+def test_grid_gather_scatter_bit_exact(ref, ghost):
+    rng = np.random.default_rng(ghost)
+    grid = rng.standard_normal((5, 32, 16, 48))
+    mask = (rng.random((16, 48)) < 0.2).astype(np.uint8)
+    vals = np.arange(5) + 0.5
+    for bc in (["periodic"] * 6, ["outflow"] * 6, ["outflow", "periodic", "periodic", "outflow", "outflow", "outflow"]):
+        for inflow in (None, (mask, vals)):
+            want = ref.grid_gather(grid, ghost, bc, inflow)
+            di = None if inflow is None else (dev(mask), vals)
+            got = B.grid_gather(dev(grid), ghost, bc, di).cpu().numpy()
+            assert np.array_equal(got, want)
+    out = rng.standard_normal((6, 8, 5, 8, 8, 8))
+    want = ref.grid_scatter(out, (32, 16, 48))
+    got = B.grid_scatter(dev(out), (32, 16, 48)).cpu().numpy()
+    assert np.array_equal(got, want)
