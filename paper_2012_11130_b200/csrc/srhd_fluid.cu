@@ -432,7 +432,7 @@ extern "C" size_t srhd_workspace_bytes(int, const srhd_params*) { return 0; }
 
 extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
                                const srhd_params* params, srhd_stats* stats, void* stream) {
-  if (!cons_in || !cons_out) return SRHD_ERR_NULL_POINTER;
+  if (npg > 0 && (!cons_in || !cons_out)) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
   if (npg < 0) return SRHD_ERR_BAD_SIZE;
