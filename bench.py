@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole SRHD hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload blast256|random512|jet|tube|conv]
+                    [--impl ours|reference] [--no-e2e] [--no-cpu-baseline]
+
+A "step" is one pass of the whole hot path over the grid (driver.GridStepper.step): the CFL
+reduction (srhd_max_signal_speed), ghost-zone gather, srhd_fluid_step, scatter.  Default workload:
+BASELINE.json configs[2] (256^3 spherical blast, PPM+HLLC, CFL 0.4) -- the 3-D fluid step the
+metric "fp64 SRHD cell updates/s" is quoted on.  N > 1 runs N independent
+replicas (the path does not shard on this tier: DESIGN.md section 8); value = all ranks' cell
+updates / max-over-ranks device time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload on the host cores; see DESIGN.md section 7.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 SRHD cell updates/sec"
+UNIT = "cell updates/s"
+
+# name -> (recon, riemann, cfl, paper-config description)
+WORKLOADS = {
+    "blast256": ("ppm", "hllc", 0.4, "BASELINE.json configs[2]: 256^3 spherical blast, periodic, PPM+HLLC, CFL 0.4"),
+    "random512": ("plm", "hlle", 0.4, "BASELINE.json configs[3]: 512^3 k^-2 Gaussian random field, periodic, PLM+HLLE, CFL 0.4"),
+    "jet": ("ppm", "hllc", 0.4, "BASELINE.json configs[4]: 512x512x1024 relativistic jet, outflow + fixed inflow, PPM+HLLC, CFL 0.4"),
+    "tube": ("plm", "hllc", 0.5, "BASELINE.json configs[0]: 256x16x16 TM shock tube, PLM+HLLC, CFL 0.5"),
+}
+
+
+def make_workload(name, scale=1):
+    """Seeded synthetic input of a config (primitives on the host): (prim, dh, bc, inflow_prim)."""
+    from paper_2012_11130_b200 import workloads as wl
+    if name == "blast256":
+        prim, dh, bc = wl.blast_wave(n=256 // scale)
+        return prim, dh, bc, None
+    if name == "random512":
+        prim, dh, bc = wl.random_field(n=512 // scale)
+        return prim, dh, bc, None
+    if name == "jet":
+        prim, dh, bc, inflow = wl.jet(nx=512 // scale, ny=512 // scale, nz=1024 // scale,
+                                      radius=0.02 * (scale if scale > 1 else 1))
+        return prim, dh, bc, inflow
+    if name == "tube":
+        prim, dh, bc = wl.shock_tube()
+        return prim, dh, bc, None
+    raise SystemExit(f"unknown workload {name}")
+
+
+# ------------------------------------------------------------------ clocks during the timed region
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if mask & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def result(self):
+        self.stop_flag = True
+        if self.nv is None or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+def oracle_sample_input(name):
+    """Bounded sample of a workload for the oracle: a 64^3 block (64 patch groups) cut from the part
+    of the 1/4-scale initial condition that holds its structure (blast surface / nozzle / centre),
+    made periodic; the tube is small enough to be taken whole.  Built with oracle/ calls only."""
+    from oracle import ref
+    recon, riemann, cfl, _ = WORKLOADS[name]
+    prim, dh, bc, _ = make_workload(name, scale=1 if name == "tube" else 4)
+    if name == "tube":
+        what = "the full 256x16x16 tube (16 patch groups)"
+    else:
+        nz, ny, nx = prim.shape[1:]
+        z0 = 0 if name == "jet" else (nz - 64) // 2
+        prim = np.ascontiguousarray(prim[:, z0:z0 + 64, (ny - 64) // 2:(ny + 64) // 2, (nx - 64) // 2:(nx + 64) // 2])
+        bc = [0] * 6
+        what = f"a periodic 64^3 block (64 patch groups) cut from the 1/4-scale {name} initial condition"
+    par = ref.params(recon, riemann)
+    cons = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    return ref, cons, dh, bc, par, cfl, what
+
+
+def oracle_steps(ref, cons, dh, bc, par, cfl, nsteps=None, budget_s=None):
+    """Advance the sample with the oracle (CFL reduction + tiled step); returns (cons, steps, seconds)."""
+    done, t0 = 0, time.perf_counter()
+    while True:
+        cons, _ = ref.grid_step_tiled(cons, ref.cfl_dt(cons, cfl, dh, par), dh, par, bc)
+        done += 1
+        el = time.perf_counter() - t0
+        if (nsteps is not None and done >= nsteps) or (budget_s is not None and el >= budget_s):
+            return cons, done, el
+
+
+def cpu_baseline(name, budget_s=12.0):
+    ref, cons, dh, bc, par, cfl, what = oracle_sample_input(name)
+    _, done, el = oracle_steps(ref, cons, dh, bc, par, cfl, nsteps=60, budget_s=budget_s)
+    return {"value": cons[0].size * done / el, "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle",
+            "sample": f"{what}; {done} steps in {el:.1f} s, OpenMP over patch groups"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; a step = one pass over the sample."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    recon, riemann, cfl, desc = WORKLOADS[args.workload]
+    ref, cons, dh, bc, par, cfl, what = oracle_sample_input(args.workload)
+    steps, warm = min(args.steps, 40), min(args.warmup, 3)     # bounded: ends within a few minutes
+    cons, _, _ = oracle_steps(ref, cons, dh, bc, par, cfl, nsteps=warm) if warm else (cons, 0, 0)
+    cons, steps, el = oracle_steps(ref, cons, dh, bc, par, cfl, nsteps=steps)
+    value = cons[0].size * steps / el
+    cores = os.cpu_count() or 1
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": 1e3 * el / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "scheme": f"{recon}+{riemann}", "cfl": cfl, "what": desc,
+                   "sample": what},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------ GPU legs
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE fluid_step_kernel launch, from the ncu --set full
+# capture named beside each entry (profiles/); None until a capture of that workload exists.
+NCU_TRAFFIC_BYTES = {"blast256": 2.4638e9}   # profiles/r1a_fluid_step_ppm_hllc.md (1.758 GB read + 0.705 GB written)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2012_11130_b200 import binding as B
+    from paper_2012_11130_b200 import build as cuda_build
+    from paper_2012_11130_b200 import flopmodel as fm
+    from paper_2012_11130_b200.driver import GridStepper
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        cuda_build.build()
+    if world > 1:
+        dist.barrier()
+    B.load_library()
+
+    recon, riemann, cfl, desc = WORKLOADS[args.workload]
+    prim, dh, bc, inflow = make_workload(args.workload, scale=args.scale)
+    shape = prim.shape[1:]
+    st = GridStepper(shape, dh, bc, recon, riemann, cfl=cfl)
+    if inflow is not None:
+        mask, prim_jet = inflow
+        cj = B.prim2cons(torch.from_numpy(prim_jet.reshape(5, 1).copy()).cuda()).cpu().numpy().ravel()
+        st = GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=(mask, cj))
+    st.set_prim(prim)
+    del prim
+    ncell = st.ncell
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        st.step()
+    barrier()
+
+    # ---- device-resident timing: K steps, CUDA events on the launching (current) stream
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kev, iters, retries = [], 0, 0
+    ev0.record()
+    for _ in range(args.steps):
+        st.step(kernel_events=kev)
+    ev1.record()
+    barrier()
+    clocks = sampler.result()
+    ms = ev0.elapsed_time(ev1)
+    k_ms = sum(a.elapsed_time(b) for a, b in kev) / len(kev)
+    s = st.last_stats()
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.cpu())
+    value = world * ncell * args.steps / (ms_max * 1e-3)
+
+    # ---- end to end: host (pinned) -> device, one step, device -> host, every step
+    e2e = None
+    if not args.no_e2e:
+        h_a = torch.empty(st.grid.shape, dtype=torch.float64, pin_memory=True)
+        h_b = torch.empty_like(h_a, pin_memory=True)
+        h_a.copy_(st.grid)
+        n_e2e = max(1, min(args.steps, 10))
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n_e2e):
+            st.grid.copy_(h_a, non_blocking=True)
+            st.step()
+            h_b.copy_(st.grid, non_blocking=True)
+            h_a, h_b = h_b, h_a
+        e1.record()
+        barrier()
+        t2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        nbytes = st.grid.numel() * 8
+        e2e = {"value": world * ncell * n_e2e / (float(t2.cpu()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 8, "steps": n_e2e}
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel (fluid_step_kernel): ALU bound
+    nxt = 16 + 2 * st.par.ghost
+    nconv = st.npg * (nxt ** 3 + 2 * 3 * 17 * 256)
+    k_mean = s.newton_iters / nconv
+    flops = ncell * fm.fluid_step_flops_per_cell(recon, riemann, k_mean)
+    peak = fm.fp64_peak_tflops(clocks["sm_max_mhz"] or 1965.0)
+    ach = flops / (k_ms * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    hbm_ach = ncell * fm.FLUID_STEP_BYTES_PER_CELL / (k_ms * 1e-3) / 1e9
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "what": desc, "grid": list(shape), "patch_groups": st.npg,
+                   "scheme": f"{recon}+{riemann}", "cfl": cfl, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": f"inputs larger than L2 ({st.grid.numel() * 8 / 1e6:.0f} MB state, {st.tiles.numel() * 8 / 1e6:.0f} MB tiles)"
+                         if st.grid.numel() * 8 > 126e6 else "state fits L2 (small case)",
+                   "newton_iters_per_conversion": k_mean, "retry_patch_groups_last_step": s.n_retry_pg,
+                   "unphysical_cells_last_step": s.n_unphys_final},
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "fluid_step_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                     "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                     "peak_source": "148 SMs x 64 fp64 lanes x 2 x max SM clock (unit counts; DESIGN.md section 6)",
+                     "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (ms / args.steps),
+                     "flops_per_cell": flops / ncell,
+                     "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
+                             "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"}},
+        "gpu_launches": st.launches_per_step * args.steps,
+    }
+    if e2e:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        out["cpu_baseline"] = cpu_baseline(args.workload)
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="blast256", choices=sorted(WORKLOADS))
+    ap.add_argument("--scale", type=int, default=1, help="divide the grid extents (debugging only; 1 = the config)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
