@@ -169,6 +169,23 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------ GPU legs
+def max_over_ranks(x, world, device):
+    """MAX all-reduce of one float over the ranks (the only cross-rank exchange: replicas only,
+    DESIGN.md section 8).  Works on any backend (nccl on the GPU box, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.cpu())
+
+
+def aggregate_value(ncell_per_rank, steps, ms_local, world, device):
+    """Whole-job throughput: the units all ranks processed / the slowest rank's device time."""
+    ms_max = max_over_ranks(ms_local, world, device)
+    return world * ncell_per_rank * steps / (ms_max * 1e-3), ms_max
+
+
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE fluid_step_kernel launch, from the ncu --set full
 # capture named beside each entry (profiles/); None until a capture of that workload exists.
 NCU_TRAFFIC_BYTES = {"blast256": 2.4638e9}   # profiles/r1a_fluid_step_ppm_hllc.md (1.758 GB read + 0.705 GB written)
@@ -233,11 +250,7 @@ def run_ours(args):
     ms = ev0.elapsed_time(ev1)
     k_ms = sum(a.elapsed_time(b) for a, b in kev) / len(kev)
     s = st.last_stats()
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.cpu())
-    value = world * ncell * args.steps / (ms_max * 1e-3)
+    value, ms_max = aggregate_value(ncell, args.steps, ms, world, "cuda")
 
     # ---- end to end: host (pinned) -> device, one step, device -> host, every step
     e2e = None
@@ -256,11 +269,9 @@ def run_ours(args):
             h_a, h_b = h_b, h_a
         e1.record()
         barrier()
-        t2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        e2e_value, _ = aggregate_value(ncell, n_e2e, e0.elapsed_time(e1), world, "cuda")
         nbytes = st.grid.numel() * 8
-        e2e = {"value": world * ncell * n_e2e / (float(t2.cpu()) * 1e-3), "unit": UNIT,
+        e2e = {"value": e2e_value, "unit": UNIT,
                "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 8, "steps": n_e2e}
 
     if rank != 0:
