@@ -235,6 +235,8 @@ def run_ours(args):
     for _ in range(args.warmup):
         st.step()
     barrier()
+    peak_meas = B.fp64_peak_probe() if rank == 0 else None     # measured DFMA roof (outside the timed region)
+    barrier()
 
     # ---- device-resident timing: K steps, CUDA events on the launching (current) stream
     sampler = ClockSampler(local)
@@ -304,6 +306,8 @@ def run_ours(args):
         "roofline": {"bound": "alu", "kernel": "fluid_step_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                      "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
                      "peak_source": "148 SMs x 64 fp64 lanes x 2 x max SM clock (unit counts; DESIGN.md section 6)",
+                     "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
+                     "peak_measured_source": "srhd_fp64_peak_probe (register-only DFMA loop) in this run",
                      "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (ms / args.steps),
                      "flops_per_cell": flops / ncell,
                      "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,

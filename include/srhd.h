@@ -121,6 +121,13 @@ int srhd_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz
                      void* stream);
 int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz, void* stream);
 
+/* Measurement helper (not part of the solver): launches a register-only DFMA loop that fills every
+ * fp64 lane of the GPU (148 x 8 CTAs x 256 threads, 32*iters dependent-chain DFMA per thread in 8
+ * independent chains) on `stream`; *flops (HOST pointer, may be NULL) receives the flop count of the
+ * launch (2 per DFMA).  The caller times it with events.  d_sink: device, >= 1 double, never written
+ * in practice.  bench.py uses it for the measured fp64 ALU roof. */
+int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, void* stream);
+
 /* Human-readable text for a return code of this library (negative) or of CUDA (positive). */
 const char* srhd_error_string(int code);
 

@@ -39,7 +39,7 @@ class Stats(C.Structure):
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
            "srhd_fluid_step", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
-           "srhd_error_string", "srhd_build_is_exact"]
+           "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
 
@@ -74,6 +74,8 @@ def load_library(exact=False):
                                    C.POINTER(C.c_double), _VP]
     L.srhd_grid_scatter.restype = C.c_int
     L.srhd_grid_scatter.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, _VP]
+    L.srhd_fp64_peak_probe.restype = C.c_int
+    L.srhd_fp64_peak_probe.argtypes = [_VP, C.c_int, C.POINTER(C.c_ulonglong), _VP]
     L.srhd_error_string.restype = C.c_char_p
     L.srhd_error_string.argtypes = [C.c_int]
     L.srhd_build_is_exact.restype = C.c_int
@@ -212,3 +214,20 @@ def grid_scatter(cons_out, shape, grid=None, exact=False):
         grid = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=cons_out.device)
     _check(L.srhd_grid_scatter(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, _stream()), L)
     return grid
+
+
+def fp64_peak_probe(iters=4096, reps=5):
+    """srhd_fp64_peak_probe timed with CUDA events on the current stream: measured DFMA TFLOP/s."""
+    L = load_library(False)
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    flops = C.c_ulonglong(0)
+    best = 0.0
+    for r in range(reps + 1):                       # first launch is warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(L.srhd_fp64_peak_probe(sink.data_ptr(), iters, C.byref(flops), _stream()), L)
+        e1.record()
+        e1.synchronize()
+        if r:
+            best = max(best, flops.value / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+    return best

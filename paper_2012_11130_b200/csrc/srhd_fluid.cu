@@ -111,10 +111,11 @@ SRHD_DEV void hancock_dir(const double* __restrict__ Wr, int tk, int cidx, doubl
     else recon_ppm(a, beta, beta0, wm[q], wp[q]);
   }
   double Fm[5], Fp[5];
-  prim2cons(wm, um);
-  prim2cons(wp, up);
-  phys_flux<d>(wm, um, Fm);
-  phys_flux<d>(wp, up, Fp);
+  Aux am, ap;
+  prim2cons_aux(wm, um, am);
+  prim2cons_aux(wp, up, ap);
+  phys_flux<d>(wm, um, am, Fm);
+  phys_flux<d>(wp, up, ap, Fp);
 #pragma unroll
   for (int q = 0; q < 5; ++q) dF[q] = Fp[q] - Fm[q];
 }
@@ -204,7 +205,8 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           for (int q = 0; q < 5; ++q) U[0][q] = Ws[q * PL + c];
           bool phys[1];
           int it[1];
-          cons2prim_multi<1>(U, W, rtol, max_iter, phys, it);
+          Aux aux[1];
+          cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
           if (valid) {
 #pragma unroll
             for (int q = 0; q < 5; ++q) Ws[q * PL + c] = W[0][q];
@@ -215,7 +217,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
                                     (s < G + 16);
               if (interior) {
                 if (!phys[0]) ++my_in_fail;
-                my_umax = fmax(my_umax, umax_of_prim(W[0]));
+                my_umax = fmax(my_umax, umax_of_prim(W[0], aux[0]));
               }
             }
           }
@@ -342,8 +344,9 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           }
           bool phys[2];
           int it[2];
-          cons2prim_multi<2>(U, W, rtol, max_iter, phys, it);
-          riemann_flux<RS>(d, W[0], U[0], W[1], U[1], F);
+          Aux aux[2];
+          cons2prim_multi<2>(U, W, aux, rtol, max_iter, phys, it);
+          riemann_flux<RS>(d, W[0], U[0], aux[0], W[1], U[1], aux[1], F);
           if (valid) {
             my_iters += (unsigned)(it[0] + it[1]);
             my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
@@ -420,7 +423,7 @@ int launch_fluid(const double* cons_in, double* cons_out, int npg, double dt, do
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
   kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, dt, dh, p->minmod_coeff, p->max_retry,
-                                         p->newton_rtol, p->newton_max_iter, stats);
+                                         newton_stop_rtol(p->newton_rtol), p->newton_max_iter, stats);
   return (int)cudaGetLastError();
 }
 

@@ -125,3 +125,33 @@ extern "C" const char* srhd_error_string(int code) {
 }
 
 extern "C" int srhd_build_is_exact(void) { return SRHD_EXACT; }
+
+// ---- fp64 ALU roof: register-only DFMA loop, 8 independent chains per thread, 8 CTAs x 256 threads
+// per SM (full occupancy).  Used by bench.py for the MEASURED denominator of the "alu" roofline.
+namespace srhd {
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double* __restrict__ sink, int iters, double a, double b) {
+  double x[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = 1.0 + 1e-3 * (threadIdx.x + k);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(x[k], a, b);
+    }
+  }
+  double acc = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc += x[k];
+  if (acc == 12345.678) sink[0] = acc;    // never true: keeps the chains alive without a store
+}
+}  // namespace srhd
+
+extern "C" int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, void* stream) {
+  if (!d_sink) return SRHD_ERR_NULL_POINTER;
+  if (iters < 1) return SRHD_ERR_BAD_SIZE;
+  const int grid = srhd::kNumSMs * 8, block = 256;
+  srhd::fp64_peak_kernel<<<grid, block, 0, static_cast<cudaStream_t>(stream)>>>(d_sink, iters, 0.999999, 1e-6);
+  if (flops) *flops = 2ull * 32ull * (unsigned long long)iters * (unsigned long long)grid * block;
+  return (int)cudaGetLastError();
+}

@@ -63,7 +63,9 @@ def test_cons2prim_production_within_tolerance(ref, states):
     got = got.cpu().numpy()
     s = B.stats_to_host(sbuf)
     assert s.n_c2p_fail == int(bad.sum())                 # identical Eq. 30 verdicts (canonical L)
-    assert abs(int(s.newton_iters) - int(it.sum())) <= 0.01 * it.sum()
+    # production stop rule: the oracle's final, confirming iteration is skipped
+    n = states.shape[1]
+    assert it.sum() - 1.05 * n <= s.newton_iters <= it.sum()
     # conditioning of the inversion: (1 + Mach^2) eps with Mach = |U| / U_s
     T = states[4] / states[0]
     cs2 = ref.cs2_of_T(T)
