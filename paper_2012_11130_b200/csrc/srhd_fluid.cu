@@ -1,16 +1,20 @@
 // srhd_fluid.cu -- srhd_fluid_step: one fused kernel per batch of patch groups.
 //
 // One CTA advances one patch group (16^3 interior cells + ghost zones) and marches through
-// its z planes, keeping all three directional sweeps on chip:
-//   phase 1  plane s of the conserved tile arrives in shared memory by TMA bulk copies
-//            (cp.async.bulk + mbarrier) and is converted IN PLACE to primitives (cons2prim, Eq. 15-18);
-//            input-interior cells also feed the CFL reduction (Eq. 26) and the Eq. 30 counter;
-//   phase 2  plane kh = s - 2g + 1: PLM/PPM edge values in x, y (same plane) and z (ring of 2g-1
-//            primitive planes), prim2cons + physical fluxes of the six edge states, the common
-//            Hancock increment, evolved edge states to shared memory;
-//   phase 3  one Riemann problem per face of plane kh (x: 17x16, y: 16x17) and per z face between
-//            kh-1 and kh (16x16): cons2prim of both sides (two Newton chains per lane), HLLE/HLLC;
-//            the thread that owns column (i,j) then updates cell (i,j,kh-1), checks Eq. 30 and stores.
+// its z planes, keeping all three directional sweeps on chip.  Two barrier intervals per plane s:
+//   interval Y  (plane kh = s - 2g + 1)  Hancock stage: one LANE per (cell, direction) -- 10 cells x
+//               3 directions per warp -- does the PLM/PPM edge values of the five primitives along its
+//               direction, prim2cons + physical flux of both edge states; the three flux differences
+//               of a cell are combined with warp shuffles in the fixed order (x + y) + z, and every
+//               lane stores its two evolved edge states to shared memory (S3-S5);
+//   interval X  a CTA-wide work queue of 32-item chunks: (i) one Riemann problem per face of plane kh
+//               (z faces below it: 16x16, bound to the thread that owns the column and therefore
+//               updates cell (i,j,kh-1), checks Eq. 30 and stores it; x: 17x16, y: 16x17): cons2prim
+//               of both sides as two interleaved Newton chains per lane, HLLE/HLLC; (ii) cons2prim of
+//               the NEXT tile plane s+1 (staged by TMA bulk copies, cp.async.bulk + mbarrier, one plane
+//               ahead) into the ring of 2g-1 primitive planes; interior cells feed the CFL reduction
+//               (Eq. 26) and the Eq. 30 counter.  Mixing the two kinds of chunk fills the ragged tail of
+//               the face list.
 // If any face state or updated cell of the group fails Eq. 30 the CTA repeats the march with
 // beta <- 0.75 beta, finally with beta = 0.  Each cell's state crosses HBM once on the way
 // in (plus ghost layers) and once on the way out; the update re-reads its own cell through L2.
@@ -56,6 +60,7 @@ SRHD_DEV void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar
 }
 SRHD_DEV void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+
 // ---- shared-memory plan -----------------------------------------------------------------------
 template <int G>
 struct Plan {
@@ -69,7 +74,8 @@ struct Plan {
   static constexpr int NFXY = 272;            // faces per plane along x (17x16) and along y (16x17)
   // offsets in doubles
   static constexpr int oW = 0;
-  static constexpr int oXSm = oW + R * 5 * PL;
+  static constexpr int oStg = oW + R * 5 * PL;        // conserved plane staged by TMA, one plane ahead
+  static constexpr int oXSm = oStg + 5 * PL;
   static constexpr int oXSp = oXSm + 5 * XS;
   static constexpr int oYSm = oXSp + 5 * XS;
   static constexpr int oYSp = oYSm + 5 * YS;
@@ -86,27 +92,23 @@ struct Ctl {                       // lives in shared memory
   uint64_t mbar;
   unsigned long long newton;
   unsigned long long umax_bits;
-  unsigned int face_fail, cell_fail, in_fail, pad;
+  unsigned int face_fail, cell_fail, in_fail;
+  int queue;                       // next chunk of interval X
 };
 
-// Edge states of one cell along direction d: reconstruction of the five primitives, prim2cons of
-// both edges, physical fluxes; returns dF = F(W+) - F(W-) and the un-evolved conserved edge states.
-template <int G, int d>
-SRHD_DEV void hancock_dir(const double* __restrict__ Wr, int tk, int cidx, double beta, double beta0,
-                          double um[5], double up[5], double dF[5]) {
+// Hancock stage of one (cell, direction) lane: PLM/PPM edge values of the five primitives along d
+// (stencil offsets o[] into the primitive ring, component stride PL), prim2cons and physical flux
+// of both edge states; returns the un-evolved conserved edge states and dF = F(W+) - F(W-).
+template <int G>
+SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 * G - 1], double beta,
+                           double beta0, double um[5], double up[5], double dF[5]) {
   using P = Plan<G>;
   double wm[5], wp[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
     double a[2 * G - 1];
 #pragma unroll
-    for (int m = -(G - 1); m <= G - 1; ++m) {
-      int off;
-      if (d == 0) off = ((tk % P::R) * 5 + q) * P::PL + cidx + m;
-      else if (d == 1) off = ((tk % P::R) * 5 + q) * P::PL + cidx + m * P::NXT;
-      else off = (((tk + m) % P::R) * 5 + q) * P::PL + cidx;
-      a[m + G - 1] = Wr[off];
-    }
+    for (int m = 0; m < 2 * G - 1; ++m) a[m] = Wr[o[m] + q * P::PL];
     if (G == 2) recon_plm(a, beta, wm[q], wp[q]);
     else recon_ppm(a, beta, beta0, wm[q], wp[q]);
   }
@@ -114,8 +116,8 @@ SRHD_DEV void hancock_dir(const double* __restrict__ Wr, int tk, int cidx, doubl
   Aux am, ap;
   prim2cons_aux(wm, um, am);
   prim2cons_aux(wp, up, ap);
-  phys_flux<d>(wm, um, am, Fm);
-  phys_flux<d>(wp, up, ap, Fp);
+  phys_flux_rt(d, wm, um, am, Fm);
+  phys_flux_rt(d, wp, up, ap, Fp);
 #pragma unroll
   for (int q = 0; q < 5; ++q) dF[q] = Fp[q] - Fm[q];
 }
@@ -125,11 +127,15 @@ __global__ void __launch_bounds__(kFluidThreads, 1)
 fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out, double dt, double dh,
                   double beta0, int max_retry, double rtol, int max_iter, srhd_stats* __restrict__ stats) {
   using P = Plan<G>;
-  constexpr int NT = kFluidThreads;
+  constexpr int NT = kFluidThreads, NW = NT / 32;
   constexpr int NXT = P::NXT, PL = P::PL, T3 = P::T3, R = P::R;
+  constexpr int NP1 = (PL + 31) / 32;           // cons2prim chunks per tile plane
+  constexpr int NXY = 2 * P::NFXY / 32;         // x and y face chunks per plane (544 faces = 17 x 32)
+  static_assert(2 * P::NFXY % 32 == 0 && NW >= 8, "face list must be whole warps; z faces need 8 warps");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);
   double* Wr = sm + P::oW;
+  double* Stg = sm + P::oStg;
   double* XSm = sm + P::oXSm;
   double* XSp = sm + P::oXSp;
   double* YSm = sm + P::oYSm;
@@ -149,13 +155,18 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     ctl->newton = 0ull;
     ctl->umax_bits = 0ull;
     ctl->face_fail = ctl->cell_fail = ctl->in_fail = 0u;
+    ctl->queue = 0;
     fence_proxy_async();
   }
   __syncthreads();
 
+  // Hancock stage: lane -> (cell of the warp's ten, direction); lanes 30, 31 shadow lane 29
+  const int hd = (lane < 30) ? lane % 3 : 2;
+  const int hc = (lane < 30) ? lane / 3 : 9;
+  const int hbase = 3 * hc;
+
   const double hdt = dt / (2.0 * dh);
   const double dtdh = dt / dh;
-  uint32_t parity = 0;
   unsigned long long my_iters = 0;
   unsigned my_in_fail = 0;
   double my_umax = 0.0;
@@ -163,24 +174,65 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   int pass = 0;
   unsigned n_face_fail = 0, n_cell_fail = 0;
 
+  // TMA: conserved tile plane pl -> staging buffer (thread 0 only)
+  auto issue_plane = [&](int pl) {
+    fence_proxy_async();
+    mbar_expect_tx(&ctl->mbar, 5u * PL * 8u);
+#pragma unroll
+    for (int q = 0; q < 5; ++q)
+      bulk_g2s(Stg + q * PL, tile + (size_t)q * T3 + (size_t)pl * PL, PL * 8u, &ctl->mbar);
+  };
+  // cons2prim of 32 cells of the staged plane pl into its ring slot (Eq. 15-18); pass 0 also feeds
+  // the CFL reduction (Eq. 26) and the Eq. 30 counter from the input-interior cells
+  auto convert_chunk = [&](int pl, int chunk) {
+    mbar_wait(&ctl->mbar, (uint32_t)(pl & 1));     // NXT is even: plane parity is the same in every pass
+    double* Ws = Wr + (pl % R) * 5 * PL;
+    const int item = chunk * 32 + lane;
+    const bool valid = item < PL;
+    const int c = valid ? item : PL - 1;
+    double U[1][5], W[1][5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) U[0][q] = Stg[q * PL + c];
+    bool phys[1];
+    int it[1];
+    Aux aux[1];
+    cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
+    if (valid) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Ws[q * PL + c] = W[0][q];
+      if (pass == 0) {
+        my_iters += (unsigned)it[0];
+        const int ti = c % NXT, tj = c / NXT;
+        const bool interior = (ti >= G) && (ti < G + 16) && (tj >= G) && (tj < G + 16) && (pl >= G) &&
+                              (pl < G + 16);
+        if (interior) {
+          if (!phys[0]) ++my_in_fail;
+          my_umax = fmax(my_umax, umax_of_prim(W[0], aux[0]));
+        }
+      }
+    }
+  };
+
   for (;; ++pass) {
     if (pass > 0) beta = (pass <= max_retry) ? beta * 0.75 : 0.0;
     if (tid == 0) {
       ctl->face_fail = 0u;
       ctl->cell_fail = 0u;
-      fence_proxy_async();
-      mbar_expect_tx(&ctl->mbar, 5u * PL * 8u);
-#pragma unroll
-      for (int q = 0; q < 5; ++q) bulk_g2s(Wr + q * PL, tile + (size_t)q * T3, PL * 8u, &ctl->mbar);
+      issue_plane(0);
     }
     unsigned my_face_fail = 0, my_cell_fail = 0;
     double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // (Fx+ - Fx-) + (Fy+ - Fy-) of this thread's column cell
     double fzp[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // z flux through the lower face of that cell
 
-    for (int s = 0; s < NXT; ++s) {
-      const int kh = s - 2 * G + 1;               // physical plane handled by phases 2 and 3
+    // ---- prologue: tile plane 0 -> primitives; stage plane 1
+    for (int chunk = warp; chunk < NP1; chunk += NW) convert_chunk(0, chunk);
+    __syncthreads();
+    if (tid == 0) issue_plane(1);
 
-      // ---- phase 1a: in-plane flux differences of plane kh-1 (fluxes written in the previous step)
+    for (int s = 0; s < NXT; ++s) {
+      const int kh = s - 2 * G + 1;               // physical plane of the Hancock stage and the faces
+
+      // ---- in-plane flux differences of plane kh-1 (fluxes written in the previous interval X)
       if (tid < 256 && kh - 1 >= 0 && kh - 1 <= 15) {
         const int i = tid & 15, j = tid >> 4;
 #pragma unroll
@@ -191,131 +243,93 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
         }
       }
 
-      // ---- phase 1b: plane s has landed; conserved -> primitive in place
-      mbar_wait(&ctl->mbar, parity);
-      parity ^= 1u;
-      {
-        double* Ws = Wr + (s % R) * 5 * PL;
-        for (int base = warp * 32; base < PL; base += NT) {
-          const int item = base + lane;
-          const bool valid = item < PL;
-          const int c = valid ? item : PL - 1;
-          double U[1][5], W[1][5];
-#pragma unroll
-          for (int q = 0; q < 5; ++q) U[0][q] = Ws[q * PL + c];
-          bool phys[1];
-          int it[1];
-          Aux aux[1];
-          cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
-          if (valid) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) Ws[q * PL + c] = W[0][q];
-            if (pass == 0) {
-              my_iters += (unsigned)it[0];
-              const int ti = c % NXT, tj = c / NXT;
-              const bool interior = (ti >= G) && (ti < G + 16) && (tj >= G) && (tj < G + 16) && (s >= G) &&
-                                    (s < G + 16);
-              if (interior) {
-                if (!phys[0]) ++my_in_fail;
-                my_umax = fmax(my_umax, umax_of_prim(W[0], aux[0]));
-              }
-            }
-          }
-        }
-      }
-      __syncthreads();
-
-      // ---- phase 2: edge states + Hancock half step of plane kh (S3-S5)
+      // ---- interval Y: edge states + Hancock half step of plane kh (S3-S5)
       if (kh >= -1 && kh <= 16) {
         const bool inplane = (kh >= 0) && (kh <= 15);
-        const int nh = inplane ? 320 : 256;
+        const int nh = inplane ? 320 : 256;       // interior columns + the ring of cells around them
+        const int nchunk = (nh + 9) / 10;
         const int tk = kh + G;
         const int zb = (kh + 2) & 1;
-        for (int item = tid; item < nh; item += NT) {
+        for (int chunk = warp; chunk < nchunk; chunk += NW) {
+          int cell = chunk * 10 + hc;
+          const bool valid = (lane < 30) && (cell < nh);
+          if (cell >= nh) cell = nh - 1;
           int i, j;
-          if (item < 256) {
-            i = item & 15;
-            j = item >> 4;
+          if (cell < 256) {
+            i = cell & 15;
+            j = cell >> 4;
           } else {
-            const int e = item - 256, side = e >> 4, t = e & 15;
+            const int e = cell - 256, side = e >> 4, t = e & 15;
             i = (side == 0) ? -1 : ((side == 1) ? 16 : t);
             j = (side == 2) ? -1 : ((side == 3) ? 16 : t);
           }
           const int cidx = (j + G) * NXT + (i + G);
-          const bool hasx = inplane && (j >= 0) && (j <= 15);
-          const bool hasy = inplane && (i >= 0) && (i <= 15);
-          const bool hasz = (item < 256);
-          const int ix = j * 18 + (i + 1);
-          const int iy = (j + 1) * 16 + i;
-          const int iz = item;            // j*16 + i when item < 256
-          double acc[5], um[5], up[5], dF[5];
-          hancock_dir<G, 0>(Wr, tk, cidx, beta, beta0, um, up, dF);
+          int o[2 * G - 1];
 #pragma unroll
-          for (int q = 0; q < 5; ++q) acc[q] = dF[q];
-          if (hasx) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              XSm[q * P::XS + ix] = um[q];
-              XSp[q * P::XS + ix] = up[q];
-            }
+          for (int m = -(G - 1); m <= G - 1; ++m)
+            o[m + G - 1] = (hd == 2) ? (((tk + m) % R) * 5 * PL + cidx)
+                                     : ((tk % R) * 5 * PL + cidx + m * ((hd == 0) ? 1 : NXT));
+          double um[5], up[5], dF[5];
+          hancock_lane<G>(Wr, hd, o, beta, beta0, um, up, dF);
+          double* pm;
+          double* pp;
+          int qs;
+          bool has;
+          if (hd == 0) {
+            pm = XSm + j * 18 + (i + 1);
+            pp = XSp + j * 18 + (i + 1);
+            qs = P::XS;
+            has = inplane && (j >= 0) && (j <= 15);
+          } else if (hd == 1) {
+            pm = YSm + (j + 1) * 16 + i;
+            pp = YSp + (j + 1) * 16 + i;
+            qs = P::YS;
+            has = inplane && (i >= 0) && (i <= 15);
+          } else {
+            pm = ZSm + cell;
+            pp = ZSp + zb * 5 * P::ZS + cell;
+            qs = P::ZS;
+            has = cell < 256;
           }
-          hancock_dir<G, 1>(Wr, tk, cidx, beta, beta0, um, up, dF);
+          has = has && valid;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) acc[q] = acc[q] + dF[q];
-          if (hasy) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              YSm[q * P::YS + iy] = um[q];
-              YSp[q * P::YS + iy] = up[q];
-            }
-          }
-          hancock_dir<G, 2>(Wr, tk, cidx, beta, beta0, um, up, dF);
-          double dU[5];
-#pragma unroll
-          for (int q = 0; q < 5; ++q) dU[q] = -hdt * (acc[q] + dF[q]);
-          if (hasz) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              ZSm[q * P::ZS + iz] = um[q] + dU[q];
-              ZSp[(zb * 5 + q) * P::ZS + iz] = up[q] + dU[q];
-            }
-          }
-          if (hasx) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              XSm[q * P::XS + ix] = XSm[q * P::XS + ix] + dU[q];
-              XSp[q * P::XS + ix] = XSp[q * P::XS + ix] + dU[q];
-            }
-          }
-          if (hasy) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              YSm[q * P::YS + iy] = YSm[q * P::YS + iy] + dU[q];
-              YSp[q * P::YS + iy] = YSp[q * P::YS + iy] + dU[q];
+          for (int q = 0; q < 5; ++q) {
+            const double fx = __shfl_sync(0xffffffffu, dF[q], hbase);
+            const double fy = __shfl_sync(0xffffffffu, dF[q], hbase + 1);
+            const double fz = __shfl_sync(0xffffffffu, dF[q], hbase + 2);
+            const double dU = -hdt * ((fx + fy) + fz);
+            if (has) {
+              pm[q * qs] = um[q] + dU;
+              pp[q * qs] = up[q] + dU;
             }
           }
         }
       }
+      if (tid == 0) ctl->queue = 0;
       __syncthreads();
 
-      // the oldest primitive plane is free now: prefetch conserved plane s+1 into its slot
-      if (tid == 0 && s + 1 < NXT) {
-        fence_proxy_async();
-        mbar_expect_tx(&ctl->mbar, 5u * PL * 8u);
-        double* dst = Wr + ((s + 1) % R) * 5 * PL;
-#pragma unroll
-        for (int q = 0; q < 5; ++q)
-          bulk_g2s(dst + q * PL, tile + (size_t)q * T3 + (size_t)(s + 1) * PL, PL * 8u, &ctl->mbar);
-      }
-
-      // ---- phase 3: Riemann problems of plane kh, then the update of plane kh-1
-      if (kh >= 0 && kh <= 16) {
-        const int nf = (kh <= 15) ? (256 + 2 * P::NFXY) : 256;
+      // ---- interval X: Riemann problems of plane kh + update of plane kh-1; cons2prim of plane s+1
+      {
+        const int nxy = (kh >= 0 && kh <= 15) ? NXY : 0;
+        const int np1 = (s + 1 < NXT) ? NP1 : 0;
         const int zbl = (kh + 1) & 1;             // buffer of plane kh-1
-        for (int base = warp * 32; base < nf; base += NT) {
-          const int item = base + lane;
-          const bool valid = item < nf;
-          const int idx = valid ? item : nf - 1;
+        bool zfirst = (kh >= 0) && (kh <= 16) && (warp < 8);
+        for (;;) {
+          int idx;                                // face index, or -1 - chunk for a cons2prim chunk
+          if (zfirst) {
+            zfirst = false;
+            idx = tid;
+          } else {
+            int c = 0;
+            if (lane == 0) c = atomicAdd(&ctl->queue, 1);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c >= nxy + np1) break;
+            idx = (c < nxy) ? 256 + c * 32 + lane : -1 - (c - nxy);
+          }
+          if (idx < 0) {
+            convert_chunk(s + 1, -1 - idx);
+            continue;
+          }
           int d, qs;
           const double *pL, *pR;
           if (idx < 256) {
@@ -347,37 +361,37 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           Aux aux[2];
           cons2prim_multi<2>(U, W, aux, rtol, max_iter, phys, it);
           riemann_flux<RS>(d, W[0], U[0], aux[0], W[1], U[1], aux[1], F);
-          if (valid) {
-            my_iters += (unsigned)(it[0] + it[1]);
-            my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
-            if (idx < 256) {
-              if (kh >= 1) {                        // update cell (i, j, kh-1): Eq. 4a, 4b, 7; S12
-                const int ku = kh - 1, i = idx & 15, j = idx >> 4;
-                const double* uin = tile + ((size_t)(ku + G) * NXT + (j + G)) * NXT + (i + G);
-                const int p = (i >> 3) + 2 * (j >> 3) + 4 * (ku >> 3);   // S13
-                double* o = out + (size_t)p * 5 * 512 + (ku & 7) * 64 + (j & 7) * 8 + (i & 7);
-                double Un[5];
+          my_iters += (unsigned)(it[0] + it[1]);
+          my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
+          if (idx < 256) {
+            if (kh >= 1) {                          // update cell (i, j, kh-1): Eq. 4a, 4b, 7; S12
+              const int ku = kh - 1, i = idx & 15, j = idx >> 4;
+              const double* uin = tile + ((size_t)(ku + G) * NXT + (j + G)) * NXT + (i + G);
+              const int p = (i >> 3) + 2 * (j >> 3) + 4 * (ku >> 3);   // S13
+              double* o = out + (size_t)p * 5 * 512 + (ku & 7) * 64 + (j & 7) * 8 + (i & 7);
+              double Un[5];
 #pragma unroll
-                for (int q = 0; q < 5; ++q) {
-                  const double dfz = F[q] - fzp[q];
-                  Un[q] = __ldg(uin + (size_t)q * T3) - dtdh * (part[q] + dfz);
-                  o[q * 512] = Un[q];
-                }
-                if (!is_physical(Un)) ++my_cell_fail;                      // Eq. 30
+              for (int q = 0; q < 5; ++q) {
+                const double dfz = F[q] - fzp[q];
+                Un[q] = __ldg(uin + (size_t)q * T3) - dtdh * (part[q] + dfz);
+                o[q * 512] = Un[q];
               }
-#pragma unroll
-              for (int q = 0; q < 5; ++q) fzp[q] = F[q];
-            } else if (idx < 256 + P::NFXY) {
-#pragma unroll
-              for (int q = 0; q < 5; ++q) FX[q * P::NFXY + (idx - 256)] = F[q];
-            } else {
-#pragma unroll
-              for (int q = 0; q < 5; ++q) FY[q * P::NFXY + (idx - 256 - P::NFXY)] = F[q];
+              if (!is_physical(Un)) ++my_cell_fail;                      // Eq. 30
             }
+#pragma unroll
+            for (int q = 0; q < 5; ++q) fzp[q] = F[q];
+          } else if (idx < 256 + P::NFXY) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) FX[q * P::NFXY + (idx - 256)] = F[q];
+          } else {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) FY[q * P::NFXY + (idx - 256 - P::NFXY)] = F[q];
           }
         }
       }
       __syncthreads();
+      // the staging buffer is free again: stage conserved plane s+2
+      if (tid == 0 && s + 2 < NXT) issue_plane(s + 2);
     }
 
     // ---- verdict of this pass for the whole patch group (S9, S10, S15)
