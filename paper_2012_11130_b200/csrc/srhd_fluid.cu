@@ -22,7 +22,10 @@
 
 namespace srhd {
 
-constexpr int kFluidThreads = 512;   // 16 warps, <= 128 registers per thread, one CTA per SM
+#ifndef SRHD_FLUID_THREADS
+#define SRHD_FLUID_THREADS 512
+#endif
+constexpr int kFluidThreads = SRHD_FLUID_THREADS;   // 16 warps, <= 128 registers per thread, one CTA per SM
 
 // ---- TMA bulk copy + mbarrier (PTX; SASS: UBLKCP / SYNCS) -------------------------------------
 SRHD_DEV uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -83,7 +86,8 @@ struct Plan {
   static constexpr int oZSp = oZSm + 5 * ZS;          // two buffers (plane parity)
   static constexpr int oFX = oZSp + 2 * 5 * ZS;
   static constexpr int oFY = oFX + 5 * NFXY;
-  static constexpr int oCtl = oFY + 5 * NFXY;         // control block: 8 x 8 bytes
+  static constexpr int oFZ = oFY + 5 * NFXY;          // z flux through the lower face of each column's cell
+  static constexpr int oCtl = oFZ + 5 * ZS;           // control block: 8 x 8 bytes
   static constexpr int nDoubles = oCtl + 8;
   static constexpr size_t bytes = (size_t)nDoubles * sizeof(double);
 };
@@ -144,6 +148,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   double* ZSp = sm + P::oZSp;
   double* FX = sm + P::oFX;
   double* FY = sm + P::oFY;
+  double* FZ = sm + P::oFZ;     // written and read by the thread that owns the column: no barrier needed
   Ctl* ctl = reinterpret_cast<Ctl*>(sm + P::oCtl);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -222,7 +227,6 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     }
     unsigned my_face_fail = 0, my_cell_fail = 0;
     double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // (Fx+ - Fx-) + (Fy+ - Fy-) of this thread's column cell
-    double fzp[5] = {0.0, 0.0, 0.0, 0.0, 0.0};    // z flux through the lower face of that cell
 
     // ---- prologue: tile plane 0 -> primitives; stage plane 1
     for (int chunk = warp; chunk < NP1; chunk += NW) convert_chunk(0, chunk);
@@ -372,14 +376,14 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
               double Un[5];
 #pragma unroll
               for (int q = 0; q < 5; ++q) {
-                const double dfz = F[q] - fzp[q];
+                const double dfz = F[q] - FZ[q * P::ZS + idx];
                 Un[q] = __ldg(uin + (size_t)q * T3) - dtdh * (part[q] + dfz);
                 o[q * 512] = Un[q];
               }
               if (!is_physical(Un)) ++my_cell_fail;                      // Eq. 30
             }
 #pragma unroll
-            for (int q = 0; q < 5; ++q) fzp[q] = F[q];
+            for (int q = 0; q < 5; ++q) FZ[q * P::ZS + idx] = F[q];
           } else if (idx < 256 + P::NFXY) {
 #pragma unroll
             for (int q = 0; q < 5; ++q) FX[q * P::NFXY + (idx - 256)] = F[q];
