@@ -11,33 +11,46 @@ struct GridBC {
   int has_inflow;
 };
 
-// source index of ghost index i along an axis of n cells (S11): periodic wraps, outflow clamps
+// source index of ghost index i along an axis of n cells (S11): periodic wraps, outflow clamps.
+// |ghost offset| <= 3 < 16 <= n, so one conditional add replaces the modulo.
 SRHD_DEV int map_index(int i, int n, int bc_lo, int bc_hi) {
-  if (i < 0) return (bc_lo == SRHD_BC_PERIODIC) ? ((i % n) + n) % n : 0;
-  if (i >= n) return (bc_hi == SRHD_BC_PERIODIC) ? (i % n) : n - 1;
+  if (i < 0) return (bc_lo == SRHD_BC_PERIODIC) ? i + n : 0;
+  if (i >= n) return (bc_hi == SRHD_BC_PERIODIC) ? i - n : n - 1;
   return i;
 }
 
-// one CTA per (patch group, component): rows of nxt doubles, reads coalesced along x
+// one CTA per (patch group, component); a warp copies whole tile rows (lane = x index, so the x
+// mapping is computed once per thread), four rows in flight per warp
+template <int G>
 __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restrict__ grid,
                                                           double* __restrict__ cons_in, int nx, int ny,
-                                                          int nz, int g, GridBC b,
+                                                          int nz, GridBC b,
                                                           const unsigned char* __restrict__ mask) {
-  const int nxt = 16 + 2 * g, t3 = nxt * nxt * nxt;
+  constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
   const int px = nx / 16, py = ny / 16;
   const int pg = blockIdx.x, q = blockIdx.y;
   const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
   const size_t n = (size_t)nx * ny * nz;
   const double* __restrict__ src = grid + (size_t)q * n;
   double* __restrict__ dst = cons_in + ((size_t)pg * 5 + q) * t3;
-  for (int c = threadIdx.x; c < t3; c += blockDim.x) {
-    const int i = c % nxt, j = (c / nxt) % nxt, k = c / (nxt * nxt);
-    const int kk = gz * 16 + k - g;
-    const int si = map_index(gx * 16 + i - g, nx, b.bc[0], b.bc[1]);
-    const int sj = map_index(gy * 16 + j - g, ny, b.bc[2], b.bc[3]);
-    const int sk = map_index(kk, nz, b.bc[4], b.bc[5]);
-    const bool inflow = b.has_inflow && kk < 0 && mask[(size_t)sj * nx + si];
-    dst[c] = inflow ? b.inflow[q] : __ldg(src + ((size_t)sk * ny + sj) * nx + si);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane >= nxt) return;
+  const int si = map_index(gx * 16 + lane - G, nx, b.bc[0], b.bc[1]);
+  const double inflow_q = b.inflow[q];
+  for (int r0 = warp * 4; r0 < nrow; r0 += 32) {
+    double v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int r = r0 + u;                       // nrow is a multiple of 4
+      const int k = r / nxt, j = r - k * nxt;
+      const int kk = gz * 16 + k - G;
+      const int sj = map_index(gy * 16 + j - G, ny, b.bc[2], b.bc[3]);
+      const int sk = map_index(kk, nz, b.bc[4], b.bc[5]);
+      const bool inflow = b.has_inflow && kk < 0 && mask[(size_t)sj * nx + si];
+      v[u] = inflow ? inflow_q : __ldg(src + ((size_t)sk * ny + sj) * nx + si);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) dst[(r0 + u) * nxt + lane] = v[u];
   }
 }
 
@@ -84,8 +97,12 @@ extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int
   if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
   for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
-  grid_gather_kernel<<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
-                                                                                   ghost, b, inflow_mask);
+  if (ghost == 2)
+    grid_gather_kernel<2><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
+                                                                                        b, inflow_mask);
+  else
+    grid_gather_kernel<3><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
+                                                                                        b, inflow_mask);
   return (int)cudaGetLastError();
 }
 
