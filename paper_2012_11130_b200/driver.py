@@ -40,6 +40,12 @@ class GridStepper:
             mask, cons = inflow
             self.inflow = (torch.as_tensor(np.ascontiguousarray(mask, dtype=np.uint8)).to(device),
                            [float(v) for v in cons])
+        # the fixed-inflow ghost cells take part in the update, so their signal speed bounds dt too
+        # (Eq. 28 over every state of the stencil); one srhd_max_signal_speed call on that one state
+        self.smax_inflow = 0.0
+        if self.inflow is not None:
+            c = torch.tensor(self.inflow[1], **f64).reshape(5, 1).contiguous()
+            self.smax_inflow = float(B.max_signal_speed(c, self.par, exact=exact).cpu())
         self.t = 0.0
         self.nstep = 0
         self.launches_per_step = 5   # c2p-max, smax finish, gather, fluid step, scatter
@@ -65,7 +71,7 @@ class GridStepper:
     # ---- one step -------------------------------------------------------------------------------
     def signal_speed(self):
         B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
-        return float(self.smax.cpu())          # the one device->host double per step
+        return max(float(self.smax.cpu()), self.smax_inflow)   # the one device->host double per step
 
     def advance(self, dt, kernel_events=None):
         """gather -> fluid_step -> scatter with a given dt (asynchronous on the current stream).

@@ -118,7 +118,7 @@ def _grf(rng, n, dtype=np.float64):
     k2[0, 0, 0] = 1.0
     fk /= np.sqrt(k2)
     fk[0, 0, 0] = 0.0
-    f = np.fft.irfftn(fk, s=(n, n, n))
+    f = np.fft.irfftn(fk, s=(n, n, n), axes=(0, 1, 2))
     f -= f.mean()
     f /= f.std()
     return f
