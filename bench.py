@@ -191,7 +191,99 @@ def aggregate_value(ncell_per_rank, steps, ms_local, world, device):
 NCU_TRAFFIC_BYTES = {"blast256": 2.4638e9}   # profiles/r1a_fluid_step_ppm_hllc.md (1.758 GB read + 0.705 GB written)
 
 
+def run_conv(args):
+    """--workload conv: BASELINE.json configs[1], 2^24 states, prim -> cons -> prim per step."""
+    import torch
+    from paper_2012_11130_b200 import binding as B
+    from paper_2012_11130_b200 import build as cuda_build
+    from paper_2012_11130_b200 import flopmodel as fm
+    from paper_2012_11130_b200 import workloads as wl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    cuda_build.build()
+    n = (1 << 24) // args.scale
+    prim_h = torch.from_numpy(wl.conversion_states(n=n)).pin_memory()
+    prim = prim_h.cuda()
+    cons, back = torch.empty_like(prim), torch.empty_like(prim)
+    par, stats = B.params(), B.new_stats()
+
+    def step():
+        B.prim2cons(prim, cons=cons)
+        B.cons2prim(cons, par, prim=back, stats=stats)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    peak_meas = B.fp64_peak_probe()
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    t_p2c = t_c2p = 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ev[0].record()
+        B.prim2cons(prim, cons=cons)
+        ev[1].record()
+        B.cons2prim(cons, par, prim=back, stats=stats)
+        ev[2].record()
+        ev[2].synchronize()
+        t_p2c += ev[0].elapsed_time(ev[1])
+        t_c2p += ev[1].elapsed_time(ev[2])
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.result()
+    ms = e0.elapsed_time(e1)
+    s = B.stats_to_host(stats)
+    # end to end: states from pinned host memory, primitives back to the host
+    back_h = torch.empty_like(prim_h).pin_memory()
+    n_e2e = max(1, min(args.steps, 10))
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n_e2e):
+        prim.copy_(prim_h, non_blocking=True)
+        step()
+        back_h.copy_(back, non_blocking=True)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_e2e = e0.elapsed_time(e1)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    k_mean = s.newton_iters / n
+    c2p_ms, p2c_ms = t_c2p / args.steps, t_p2c / args.steps
+    ach = n * fm.c2p(k_mean) / (c2p_ms * 1e-3) / 1e12
+    peak = fm.fp64_peak_tflops(clocks["sm_max_mhz"] or 1965.0)
+    out = {
+        "metric": "fp64 SRHD prim->cons->prim round trips/sec", "value": n * args.steps / (ms * 1e-3),
+        "unit": "states/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "conv", "what": "BASELINE.json configs[1]: 2^24 states, log-uniform rho, Theta, Lorentz factor",
+                   "states": n, "l2": "inputs larger than L2 (671 MB per 5-array)", "newton_iters_per_conversion": k_mean,
+                   "eq30_failures": s.n_c2p_fail},
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "cons2prim_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                     "frac": ach / peak, "traffic": None, "kernel_ms": c2p_ms, "peak_measured": peak_meas,
+                     "flops_per_state": fm.c2p(k_mean),
+                     "hbm": {"achieved": n * 80 / (c2p_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": n * 80 / (c2p_ms * 1e-3) / 1e9 / hbm_peak},
+                     "prim2cons": {"bound": "hbm", "kernel_ms": p2c_ms, "achieved": n * 80 / (p2c_ms * 1e-3) / 1e9,
+                                   "peak": hbm_peak, "unit": "GB/s", "frac": n * 80 / (p2c_ms * 1e-3) / 1e9 / hbm_peak}},
+        "gpu_launches": 2 * args.steps,
+        "e2e": {"value": n * n_e2e / (ms_e2e * 1e-3), "unit": "states/s", "h2d_bytes_per_step": n * 40,
+                "d2h_bytes_per_step": n * 40, "steps": n_e2e},
+    }
+    print(json.dumps(out))
+
+
 def run_ours(args):
+    if args.workload == "conv":
+        return run_conv(args)
     import torch
     import torch.distributed as dist
     from paper_2012_11130_b200 import binding as B
@@ -343,13 +435,15 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="blast256", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="blast256", choices=sorted(WORKLOADS) + ["conv"])
     ap.add_argument("--scale", type=int, default=1, help="divide the grid extents (debugging only; 1 = the config)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":
+        if args.workload == "conv":
+            raise SystemExit("--impl reference times the fluid-step workloads only")
         run_reference(args)
     else:
         run_ours(args)
