@@ -107,6 +107,19 @@ int srhd_max_signal_speed(const double* cons, size_t n, size_t stride,
 int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
                     const srhd_params* params, srhd_stats* stats, void* stream);
 
+/* The same step, additionally returning the fluxes through the six boundary faces of every 8^3 patch
+ * -- what the AMR driver's flux-correction step at coarse-fine interfaces consumes (P:285 section
+ * 3.3(4); the solver runs on the GPU, the correction on the host side).
+ *   flux_out: device, [npg][8][6][5][8][8] doubles: patch p (S13), face (0 x-lo, 1 x-hi, 2 y-lo, 3 y-hi,
+ *             4 z-lo, 5 z-hi), component (D, M^x, M^y, M^z, Etilde), then the two in-face cell
+ *             coordinates, slower one first: (z,y) on x faces, (z,x) on y faces, (y,x) on z faces.
+ *             Values are the HLLE/HLLC fluxes of the ACCEPTED pass, positive along +axis; the face shared
+ *             by two patches of the group is written to both.  NULL = srhd_fluid_step.
+ * Must not overlap cons_in / cons_out.  Same errors and asynchrony as srhd_fluid_step. */
+int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+                           double dt, double dh, const srhd_params* params, srhd_stats* stats,
+                           void* stream);
+
 /* Bytes of caller-provided scratch srhd_fluid_step needs: 0, the step is fully fused. */
 size_t srhd_workspace_bytes(int npg, const srhd_params* params);
 

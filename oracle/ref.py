@@ -176,6 +176,18 @@ def fluid_step(cons_in, dt, dh, par, nthreads=0):
     return out, st
 
 
+def fluid_step_fluxes(cons_in, dt, dh, par, nthreads=0):
+    """As fluid_step, plus the patch-boundary fluxes (npg,8,6,5,8,8) of the accepted pass."""
+    cons_in = _f64(cons_in)
+    npg = cons_in.shape[0]
+    out = np.empty((npg, 8, 5, 8, 8, 8))
+    flux = np.empty((npg, 8, 6, 5, 8, 8))
+    st = Stats()
+    lib().srhd_ref_fluid_step_fluxes(_p(cons_in), _p(out), _p(flux), C.c_int(npg), _D(dt), _D(dh),
+                                     C.byref(par), C.byref(st), C.c_int(nthreads))
+    return out, flux, st
+
+
 def _bc(bc):
     m = {"periodic": 0, "outflow": 1}
     return (C.c_int * 6)(*[m[b] if isinstance(b, str) else int(b) for b in bc])

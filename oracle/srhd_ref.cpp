@@ -308,8 +308,10 @@ struct Box {
   }
 };
 
+// flux_keep (optional, 3*5*padded cells): receives the Riemann fluxes of the ACCEPTED pass,
+// [dir][comp][cell c] = flux through the face between c and c + 1 along dir
 int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt, double dh,
-             const srhd_ref_params& par, srhd_ref_stats& st) {
+             const srhd_ref_params& par, srhd_ref_stats& st, double* flux_keep = nullptr) {
   const int g = par.ghost;
   Box b{nx, ny, nz, g, nx + 2 * g, ny + 2 * g, nz + 2 * g, 0};
   b.cstride = (size_t)b.sx * b.sy * b.sz;
@@ -429,6 +431,7 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
     (void)ext;
     if ((face_fail == 0 && cell_fail == 0) || beta == 0.0) break;   // S9, S10
   }
+  if (flux_keep) std::copy(Flux.begin(), Flux.end(), flux_keep);
   if (pass > 0) ++st.n_retry_pg;
   st.n_c2p_fail += face_fail;        // only non-zero in an accepted beta = 0 pass (S15)
   st.n_unphys_final += cell_fail;
@@ -535,8 +538,20 @@ int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, i
   return passes;
 }
 
+// P:285 section 3.3(4): the fluxes through the six boundary faces of every 8^3 patch are what
+// the AMR driver's flux-correction step consumes.  flux_out (may be null): [npg][8][6][5][8][8],
+// patch p (S13), face 0 x-lo, 1 x-hi, 2 y-lo, 3 y-hi, 4 z-lo, 5 z-hi, component, then the two in-face
+// cell coordinates, slower one first: (z,y) on x faces, (z,x) on y faces, (y,x) on z faces.
+void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+                                double dt, double dh, const srhd_ref_params* par,
+                                srhd_ref_stats* stats, int nthreads);
 void srhd_ref_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
                          const srhd_ref_params* par, srhd_ref_stats* stats, int nthreads) {
+  srhd_ref_fluid_step_fluxes(cons_in, cons_out, nullptr, npg, dt, dh, par, stats, nthreads);
+}
+void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+                                double dt, double dh, const srhd_ref_params* par,
+                                srhd_ref_stats* stats, int nthreads) {
   const int nxt = 16 + 2 * par->ghost;
   const size_t in_pg = (size_t)5 * nxt * nxt * nxt, out_pg = (size_t)8 * 5 * 512;
   unsigned long long f1 = 0, f2 = 0, f3 = 0, f4 = 0;
@@ -551,7 +566,29 @@ void srhd_ref_fluid_step(const double* cons_in, double* cons_out, int npg, doubl
     srhd_ref_stats st;
     std::memset(&st, 0, sizeof(st));
     std::vector<double> box((size_t)5 * 4096);
-    step_box(cons_in + pg * in_pg, box.data(), 16, 16, 16, dt, dh, *par, st);
+    std::vector<double> fl(flux_out ? (size_t)3 * in_pg : 0);
+    step_box(cons_in + pg * in_pg, box.data(), 16, 16, 16, dt, dh, *par, st, flux_out ? fl.data() : nullptr);
+    if (flux_out) {
+      const int g = par->ghost;
+      const size_t np = (size_t)nxt * nxt * nxt;
+      auto at = [&](int i, int j, int k) { return ((size_t)(k + g) * nxt + (j + g)) * nxt + (i + g); };
+      double* fo = flux_out + (size_t)pg * 8 * 6 * 5 * 64;
+      for (int p = 0; p < 8; ++p) {
+        const int i0 = 8 * (p & 1), j0 = 8 * ((p >> 1) & 1), k0 = 8 * (p >> 2);
+        for (int f = 0; f < 6; ++f) {
+          const int d = f >> 1, hi = f & 1;
+          for (int q = 0; q < 5; ++q)
+            for (int a = 0; a < 8; ++a)
+              for (int bb = 0; bb < 8; ++bb) {
+                int i, j, k;
+                if (d == 0) { i = i0 + (hi ? 7 : -1); j = j0 + bb; k = k0 + a; }
+                else if (d == 1) { i = i0 + bb; j = j0 + (hi ? 7 : -1); k = k0 + a; }
+                else { i = i0 + bb; j = j0 + a; k = k0 + (hi ? 7 : -1); }
+                fo[(((size_t)p * 6 + f) * 5 + q) * 64 + a * 8 + bb] = fl[((size_t)d * 5 + q) * np + at(i, j, k)];
+              }
+        }
+      }
+    }
     double* out = cons_out + pg * out_pg;
     for (int q = 0; q < 5; ++q)
       for (int k = 0; k < 16; ++k)

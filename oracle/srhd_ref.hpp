@@ -76,6 +76,14 @@ int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, i
 void srhd_ref_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
                          const srhd_ref_params* par, srhd_ref_stats* stats, int nthreads);
 
+// The same step that also returns the fluxes through the six boundary faces of every 8^3 patch, as
+// the AMR flux-correction step needs them (section 3.3(4)): flux_out [npg][8][6][5][8][8]
+// (patch, face x-lo x-hi y-lo y-hi z-lo z-hi, component, in-face coordinates slower one first:
+// (z,y) / (z,x) / (y,x)); fluxes of the accepted pass, positive along +axis.  May be null.
+void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+                                double dt, double dh, const srhd_ref_params* par,
+                                srhd_ref_stats* stats, int nthreads);
+
 // single Riemann flux along direction dir (0,1,2), for tests: WL/UL/WR/UR are 5-vectors
 void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL,
                            const double* WR, const double* UR, double* F);

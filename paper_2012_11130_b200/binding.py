@@ -38,7 +38,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
            "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -67,6 +67,8 @@ def load_library(exact=False):
     L.srhd_max_signal_speed.argtypes = [_VP, C.c_size_t, C.c_size_t, C.POINTER(Params), _VP, _VP]
     L.srhd_fluid_step.restype = C.c_int
     L.srhd_fluid_step.argtypes = [_VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
+    L.srhd_fluid_step_fluxes.restype = C.c_int
+    L.srhd_fluid_step_fluxes.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_workspace_bytes.restype = C.c_size_t
     L.srhd_workspace_bytes.argtypes = [C.c_int, C.POINTER(Params)]
     L.srhd_grid_gather.restype = C.c_int
@@ -177,6 +179,22 @@ def fluid_step(cons_in, dt, dh, par, cons_out=None, stats=None, exact=False):
     _check(L.srhd_fluid_step(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(), npg, float(dt),
                              float(dh), C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, stats
+
+
+def fluid_step_fluxes(cons_in, dt, dh, par, cons_out=None, flux_out=None, stats=None, exact=False):
+    """srhd_fluid_step_fluxes: as fluid_step, plus the patch-boundary fluxes (npg,8,6,5,8,8)."""
+    L = load_library(exact)
+    cons_in = _dev(cons_in, "cons_in")
+    npg = cons_in.shape[0]
+    if cons_out is None:
+        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=torch.float64, device=cons_in.device)
+    if flux_out is None:
+        flux_out = torch.empty((npg, 8, 6, 5, 8, 8), dtype=torch.float64, device=cons_in.device)
+    stats = new_stats(cons_in.device) if stats is None else stats
+    _check(L.srhd_fluid_step_fluxes(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(),
+                                    _dev(flux_out, "flux_out").data_ptr(), npg, float(dt), float(dh),
+                                    C.byref(par), stats.data_ptr(), _stream()), L)
+    return cons_out, flux_out, stats
 
 
 def _bc(bc):

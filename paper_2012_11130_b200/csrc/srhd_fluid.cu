@@ -128,8 +128,9 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
 
 template <int G, int RS>
 __global__ void __launch_bounds__(kFluidThreads, 1)
-fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out, double dt, double dh,
-                  double beta0, int max_retry, double rtol, int max_iter, srhd_stats* __restrict__ stats) {
+fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out,
+                  double* __restrict__ flux_out, double dt, double dh, double beta0, int max_retry, double rtol,
+                  int max_iter, srhd_stats* __restrict__ stats) {
   using P = Plan<G>;
   constexpr int NT = kFluidThreads, NW = NT / 32;
   constexpr int NXT = P::NXT, PL = P::PL, T3 = P::T3, R = P::R;
@@ -154,6 +155,12 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const double* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
   double* __restrict__ out = cons_out + (size_t)blockIdx.x * 8 * 5 * 512;
+  double* __restrict__ fout = flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr;
+  // flux through a patch-boundary face -> flux_out[patch][face][comp][a][b] (include/srhd.h)
+  auto put_flux = [&](int p, int f, int a, int b, const double F[5]) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) fout[(((size_t)p * 6 + f) * 5 + q) * 64 + a * 8 + b] = F[q];
+  };
 
   if (tid == 0) {
     mbar_init(&ctl->mbar, 1);
@@ -367,6 +374,29 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           riemann_flux<RS>(d, W[0], U[0], aux[0], W[1], U[1], aux[1], F);
           my_iters += (unsigned)(it[0] + it[1]);
           my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
+          if (fout) {                               // faces on the boundary of an 8^3 patch
+            if (idx < 256) {
+              if ((kh & 7) == 0) {
+                const int i = idx & 15, j = idx >> 4, pxy = (i >> 3) + 2 * (j >> 3);
+                if (kh < 16) put_flux(pxy + 4 * (kh >> 3), 4, j & 7, i & 7, F);
+                if (kh > 0) put_flux(pxy + 4 * ((kh - 1) >> 3), 5, j & 7, i & 7, F);
+              }
+            } else if (idx < 256 + P::NFXY) {
+              const int f = idx - 256, jj = f / 17, fi = f - jj * 17;
+              if ((fi & 7) == 0) {
+                const int pyz = 2 * (jj >> 3) + 4 * (kh >> 3);
+                if (fi < 16) put_flux((fi >> 3) + pyz, 0, kh & 7, jj & 7, F);
+                if (fi > 0) put_flux(((fi - 1) >> 3) + pyz, 1, kh & 7, jj & 7, F);
+              }
+            } else {
+              const int f = idx - 256 - P::NFXY, jf = f >> 4, i = f & 15;
+              if ((jf & 7) == 0) {
+                const int pxz = (i >> 3) + 4 * (kh >> 3);
+                if (jf < 16) put_flux(pxz + 2 * (jf >> 3), 2, kh & 7, i & 7, F);
+                if (jf > 0) put_flux(pxz + 2 * ((jf - 1) >> 3), 3, kh & 7, i & 7, F);
+              }
+            }
+          }
           if (idx < 256) {
             if (kh >= 1) {                          // update cell (i, j, kh-1): Eq. 4a, 4b, 7; S12
               const int ku = kh - 1, i = idx & 15, j = idx >> 4;
@@ -434,13 +464,13 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
 }
 
 template <int G, int RS>
-int launch_fluid(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
                  const srhd_params* p, srhd_stats* stats, cudaStream_t st) {
   auto kern = fluid_step_kernel<G, RS>;
   const size_t smem = Plan<G>::bytes;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
-  kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, dt, dh, p->minmod_coeff, p->max_retry,
+  kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, flux_out, dt, dh, p->minmod_coeff, p->max_retry,
                                          newton_stop_rtol(p->newton_rtol), p->newton_max_iter, stats);
   return (int)cudaGetLastError();
 }
@@ -451,8 +481,9 @@ using namespace srhd;
 
 extern "C" size_t srhd_workspace_bytes(int, const srhd_params*) { return 0; }
 
-extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
-                               const srhd_params* params, srhd_stats* stats, void* stream) {
+extern "C" int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+                                      double dt, double dh, const srhd_params* params, srhd_stats* stats,
+                                      void* stream) {
   if (npg > 0 && (!cons_in || !cons_out)) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
@@ -473,10 +504,15 @@ extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg,
   if (npg == 0) return SRHD_OK;
   if (params->recon == SRHD_RECON_PLM) {
     return params->riemann == SRHD_RIEMANN_HLLE
-               ? launch_fluid<2, 0>(cons_in, cons_out, npg, dt, dh, params, stats, st)
-               : launch_fluid<2, 1>(cons_in, cons_out, npg, dt, dh, params, stats, st);
+               ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st)
+               : launch_fluid<2, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st);
   }
   return params->riemann == SRHD_RIEMANN_HLLE
-             ? launch_fluid<3, 0>(cons_in, cons_out, npg, dt, dh, params, stats, st)
-             : launch_fluid<3, 1>(cons_in, cons_out, npg, dt, dh, params, stats, st);
+             ? launch_fluid<3, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st)
+             : launch_fluid<3, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st);
+}
+
+extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+                               const srhd_params* params, srhd_stats* stats, void* stream) {
+  return srhd_fluid_step_fluxes(cons_in, cons_out, nullptr, npg, dt, dh, params, stats, stream);
 }

@@ -124,3 +124,31 @@ def test_grid_gather_scatter_bit_exact(ref, ghost):
     want = ref.grid_scatter(out, (32, 16, 48))
     got = B.grid_scatter(dev(out), (32, 16, 48)).cpu().numpy()
     assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("recon,riemann", [("plm", "hlle"), ("ppm", "hllc")])
+def test_patch_boundary_fluxes_parity(ref, recon, riemann):
+    """srhd_fluid_step_fluxes: the fluxes through the faces of every 8^3 patch; a retry pass
+    must leave the ACCEPTED pass's fluxes behind.  Exact build bit for bit, production to 1e-11 of the
+    largest flux of the face."""
+    po = ref.params(recon, riemann, max_retry=3)
+    npg, dh = 4, 1.0 / 64
+    for rough_dt in (False, True):
+        kw = dict(umax=30.0, rough=3.0, log_theta=(-8.0, 2.0)) if rough_dt else {}
+        tiles = make_tiles(ref, npg, po.ghost, seed=5 if rough_dt else 11 + po.ghost, **kw)
+        dt = (4.0 if rough_dt else 1.0) * cfl_dt(ref, tiles, dh)
+        want, wflux, st = ref.fluid_step_fluxes(tiles, dt, dh, po)
+        assert st.n_retry_pg > 0 or not rough_dt          # the rough case must go through the ladder
+        got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, dh, B.params(recon, riemann, max_retry=3, exact=True),
+                                               exact=True)
+        assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+        assert np.array_equal(gflux.cpu().numpy(), wflux, equal_nan=True)
+        assert B.stats_to_host(sbuf).as_dict() == st.as_dict()
+        if not rough_dt:
+            got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, dh, B.params(recon, riemann, max_retry=3))
+            assert B.stats_to_host(sbuf).n_retry_pg == st.n_retry_pg      # same rungs of the ladder
+            gf = gflux.cpu().numpy()
+            scale = np.abs(wflux).max(axis=(4, 5), keepdims=True)
+            assert (np.abs(gf - wflux) / scale).max() <= 1e-11
+            plain, _ = B.fluid_step(dev(tiles), dt, dh, B.params(recon, riemann, max_retry=3))
+            assert np.array_equal(plain.cpu().numpy(), got.cpu().numpy())

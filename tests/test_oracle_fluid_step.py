@@ -180,3 +180,38 @@ def test_shock_tube_config0_against_exact_riemann_solution(ref):
     plateau = (x > tail + 4 * dh) & (x < 0.5 + float(ex.v_star) * t_end - 4 * dh)
     if plateau.sum() >= 3:
         assert np.abs(W[4, plateau] / float(ex.p_star) - 1).max() < 0.1
+
+
+def test_patch_boundary_fluxes_obey_the_divergence_theorem(ref):
+    """P:285 (flux correction needs the patch-face fluxes): the change of a patch's content equals
+    -dt/dh times the net flux through its six faces (interior faces cancel in the update), and the
+    face shared by two patches carries one flux.  Pins the flux output against the update itself."""
+    for recon, riemann in (("plm", "hlle"), ("ppm", "hllc")):
+        par = ref.params(recon, riemann)
+        prim = wl.random_patch_groups(2, par.ghost, seed=21, rough=0.2)
+        nxt = 16 + 2 * par.ghost
+        cons = ref.prim2cons(prim.transpose(1, 0, 2, 3, 4).reshape(5, -1)).reshape(5, 2, nxt, nxt, nxt)
+        tiles = np.ascontiguousarray(cons.transpose(1, 0, 2, 3, 4))
+        dh = 1.0 / 64
+        dt = 0.4 * dh / ref.max_signal_speed(cons.reshape(5, -1))
+        out, flux, st = ref.fluid_step_fluxes(tiles, dt, dh, par)
+        out2, st2 = ref.fluid_step(tiles, dt, dh, par)
+        assert np.array_equal(out, out2)
+        g = par.ghost
+        for pg in range(2):
+            for p in range(8):
+                i0, j0, k0 = 8 * (p & 1), 8 * ((p >> 1) & 1), 8 * (p >> 2)
+                old = tiles[pg][:, g + k0:g + k0 + 8, g + j0:g + j0 + 8, g + i0:g + i0 + 8]
+                dU = (out[pg, p] - old).reshape(5, -1).sum(1)
+                net = sum(flux[pg, p, 2 * d + 1].reshape(5, -1).sum(1) - flux[pg, p, 2 * d].reshape(5, -1).sum(1)
+                          for d in range(3))
+                scale = np.abs(flux[pg, p]).transpose(1, 0, 2, 3).reshape(5, -1).sum(1) * dt / dh + 1e-300
+                assert np.all(np.abs(dU + dt / dh * net) <= 1e-12 * scale), (dU, -dt / dh * net)
+            # shared faces: x-hi of patch (0,py,pz) is x-lo of patch (1,py,pz), same for y and z
+            for p in range(8):
+                if not p & 1:
+                    assert np.array_equal(flux[pg, p, 1], flux[pg, p + 1, 0])
+                if not p & 2:
+                    assert np.array_equal(flux[pg, p, 3], flux[pg, p + 2, 2])
+                if not p & 4:
+                    assert np.array_equal(flux[pg, p, 5], flux[pg, p + 4, 4])
