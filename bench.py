@@ -188,7 +188,7 @@ def aggregate_value(ncell_per_rank, steps, ms_local, world, device):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE fluid_step_kernel launch, from the ncu --set full
 # capture named beside each entry (profiles/); None until a capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"blast256": 2.4638e9}   # profiles/r1a_fluid_step_ppm_hllc.md (1.758 GB read + 0.705 GB written)
+NCU_TRAFFIC_BYTES = {"blast256": 2.3960e9}   # profiles/r1d_fluid_step_ppm_hllc.md (1.747 GB read + 0.649 GB written)
 
 
 def run_conv(args):
