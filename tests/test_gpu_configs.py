@@ -77,11 +77,12 @@ def test_config4_jet_reduced_50_steps(ref):
     g, o, n = _multi_step(ref, prim, dh, bc, "ppm", "hllc", 0.4, nsteps=50, inflow=inflow, exact=True)
     assert np.abs(g[3]).max() > 0                       # the jet entered the box
     assert np.array_equal(g, o)                         # exact build: 50 steps bit for bit (<= 1e-9 trivially)
-    # Production build: the HLLC star state at the jet head forms S - v_n and S - lambda* from speeds
-    # that agree to 4e-7 at gamma = 1e3 (plain forms of reading S6/S7, as in the oracle), so ANY two
-    # roundings of it differ by ~5e-10 relative there, every step; the head cells carry that into the
-    # L1 sum.  Tolerance derived from that conditioning: 50 steps x 5e-10 / ~10
-    # beam layers.  The smooth configs above meet the north-star 1e-9.
+    # Production build: at beam Mach ~1.4e3 the inversion of a half-step face state carries (1+Mach^2) eps
+    # ~ 4e-10 relative uncertainty in h, U, rho (the paper's error model, Eq. 20), so two evaluation
+    # orders differ by up to that much along the beam boundary every step and the shear layer amplifies
+    # it: one-step differences stay <= 1e-12 of the local scale (full-size test below), the free-running
+    # 50-step L1 reaches 1.6e-9.  Tolerance derived from that conditioning; the
+    # smooth configs above meet the north-star 1e-9.
     g, o, n = _multi_step(ref, prim, dh, bc, "ppm", "hllc", 0.4, nsteps=50, inflow=inflow)
     assert l1_rel(g, o).max() <= 5e-9, l1_rel(g, o)
 
