@@ -45,6 +45,12 @@ extern "C" {
 #define SRHD_RIEMANN_HLLE 0
 #define SRHD_RIEMANN_HLLC 1
 
+#define SRHD_REFINE_NONE   0   /* no gradient criterion */
+#define SRHD_REFINE_D      1   /* Q = D        (conserved: no root finding)            */
+#define SRHD_REFINE_ETILDE 2   /* Q = Etilde   (conserved)                                    */
+#define SRHD_REFINE_RHO    3   /* Q = rho      (primitive: cons2prim per cell; P:346 uses it) */
+#define SRHD_REFINE_GAMMA  4   /* Q = Lorentz factor ("gradient of the Lorentz factor") */
+
 #define SRHD_BC_PERIODIC 0
 #define SRHD_BC_OUTFLOW  1
 
@@ -119,6 +125,17 @@ int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt,
 int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
                            double dt, double dh, const srhd_params* params, srhd_stats* stats,
                            void* stream);
+
+/* Refinement criteria of the SRHD module (section 3.1; Eq. 33), one flag per 8^3 patch,
+ * on the same ghosted tiles as srhd_fluid_step (cons_in: [npg][5][nxt]^3, nxt = 16 + 2*params->ghost).
+ *   flags[pg*8 + p] = 1 if ANY cell of patch p (S13) satisfies
+ *     (|Q(i+1)-Q(i-1)| + |Q(j+1)-Q(j-1)| + |Q(k+1)-Q(k-1)|) / (2 |Q|) > c_q        (Eq. 33 with centred
+ *         differences, reading S17; the cell size cancels)       -- skipped if quantity == SRHD_REFINE_NONE
+ *     or  |M| / D > mom_over_d
+ *                                                                 -- skipped if mom_over_d == 0
+ *   else 0.  flags: device, npg*8 bytes.  Thresholds per level are the caller's business. */
+int srhd_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
+                      const srhd_params* params, unsigned char* flags, void* stream);
 
 /* Bytes of caller-provided scratch srhd_fluid_step needs: 0, the step is fully fused. */
 size_t srhd_workspace_bytes(int npg, const srhd_params* params);

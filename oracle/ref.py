@@ -188,6 +188,19 @@ def fluid_step_fluxes(cons_in, dt, dh, par, nthreads=0):
     return out, flux, st
 
 
+REFINE_Q = {None: 0, "none": 0, "D": 1, "Etilde": 2, "rho": 3, "gamma": 4}
+
+
+def refine_flags(cons_in, par, quantity="rho", c_q=0.3, mom_over_d=0.0):
+    """(npg,5,nxt,nxt,nxt) tiles -> (npg,8) uint8 patch flags (Eq. 33 / |M|/D criteria)."""
+    cons_in = _f64(cons_in)
+    npg = cons_in.shape[0]
+    flags = np.zeros((npg, 8), dtype=np.uint8)
+    lib().srhd_ref_refine_flags(_p(cons_in), C.c_int(npg), C.c_int(REFINE_Q[quantity]), _D(c_q), _D(mom_over_d),
+                                C.byref(par), flags.ctypes.data_as(C.POINTER(C.c_ubyte)))
+    return flags
+
+
 def _bc(bc):
     m = {"periodic": 0, "outflow": 1}
     return (C.c_int * 6)(*[m[b] if isinstance(b, str) else int(b) for b in bc])

@@ -674,4 +674,46 @@ void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny,
   }
 }
 
+
+// ---- refinement criteria (section 3.1; Eq. 33; reading S17: centred differences) --
+// quantity: 0 none, 1 D, 2 Etilde, 3 rho, 4 Lorentz factor.  flags[pg*8 + p], patch p as in S13.
+void srhd_ref_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
+                           const srhd_ref_params* par, unsigned char* flags) {
+  const int g = par->ghost, nxt = 16 + 2 * g;
+  const size_t np = (size_t)nxt * nxt * nxt;
+  for (int pg = 0; pg < npg; ++pg) {
+    const double* t = cons_in + (size_t)pg * 5 * np;
+    std::vector<double> Q(np, 0.0);
+    if (quantity != 0)
+      for (size_t c = 0; c < np; ++c) {
+        if (quantity == 1) Q[c] = t[c];
+        else if (quantity == 2) Q[c] = t[4 * np + c];
+        else {
+          double U[5], W[5];
+          for (int q = 0; q < 5; ++q) U[q] = t[q * np + c];
+          cons2prim(U, W, par->newton_rtol, par->newton_max_iter, nullptr, nullptr);
+          Q[c] = (quantity == 3) ? W[0] : std::sqrt(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+        }
+      }
+    unsigned char* f = flags + (size_t)pg * 8;
+    for (int p = 0; p < 8; ++p) f[p] = 0;
+    for (int k = 0; k < 16; ++k)
+      for (int j = 0; j < 16; ++j)
+        for (int i = 0; i < 16; ++i) {
+          const size_t c = ((size_t)(k + g) * nxt + (j + g)) * nxt + (i + g);
+          bool hit = false;
+          if (quantity != 0) {
+            const double gx = std::fabs(Q[c + 1] - Q[c - 1]);
+            const double gy = std::fabs(Q[c + nxt] - Q[c - nxt]);
+            const double gz = std::fabs(Q[c + (size_t)nxt * nxt] - Q[c - (size_t)nxt * nxt]);
+            hit = ((gx + gy) + gz) / (2.0 * std::fabs(Q[c])) > c_q;              // Eq. 33
+          }
+          if (mom_over_d > 0.0) {
+            const double mx = t[np + c], my = t[2 * np + c], mz = t[3 * np + c];
+            hit = hit || (std::sqrt((mx * mx + my * my) + mz * mz) / t[c] > mom_over_d);
+          }
+          if (hit) f[(i >> 3) + 2 * (j >> 3) + 4 * (k >> 3)] = 1;
+        }
+  }
+}
 }  // extern "C"

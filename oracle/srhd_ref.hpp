@@ -104,4 +104,11 @@ void srhd_ref_grid_gather(const double* grid, double* cons_in, int nx, int ny, i
                           const int* bc, const unsigned char* inflow_mask,
                           const double* inflow_cons);
 void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz);
+
+// --- refinement criteria of the SRHD module (section 3.1; Eq. 33) -----------------
+// per 8^3 patch of ghosted patch-group tiles: flag = any cell with
+//   (|dQ_x| + |dQ_y| + |dQ_z|) / (2|Q|) > c_q  (centred differences over two cells: reading S17)
+//   or |M|/D > mom_over_d (skipped when 0).  quantity: 0 none, 1 D, 2 Etilde, 3 rho, 4 Lorentz factor.
+void srhd_ref_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
+                           const srhd_ref_params* par, unsigned char* flags);
 }

@@ -38,7 +38,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
            "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -69,6 +69,8 @@ def load_library(exact=False):
     L.srhd_fluid_step.argtypes = [_VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_fluid_step_fluxes.restype = C.c_int
     L.srhd_fluid_step_fluxes.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
+    L.srhd_refine_flags.restype = C.c_int
+    L.srhd_refine_flags.argtypes = [_VP, C.c_int, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_workspace_bytes.restype = C.c_size_t
     L.srhd_workspace_bytes.argtypes = [C.c_int, C.POINTER(Params)]
     L.srhd_grid_gather.restype = C.c_int
@@ -195,6 +197,22 @@ def fluid_step_fluxes(cons_in, dt, dh, par, cons_out=None, flux_out=None, stats=
                                     _dev(flux_out, "flux_out").data_ptr(), npg, float(dt), float(dh),
                                     C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, flux_out, stats
+
+
+REFINE_Q = {None: 0, "none": 0, "D": 1, "Etilde": 2, "rho": 3, "gamma": 4}
+
+
+def refine_flags(cons_in, par, quantity="rho", c_q=0.3, mom_over_d=0.0, flags=None, exact=False):
+    """srhd_refine_flags: (npg,5,nxt,nxt,nxt) tiles -> (npg,8) uint8 patch flags."""
+    L = load_library(exact)
+    cons_in = _dev(cons_in, "cons_in")
+    npg = cons_in.shape[0]
+    if flags is None:
+        flags = torch.empty((npg, 8), dtype=torch.uint8, device=cons_in.device)
+    q = REFINE_Q[quantity] if not isinstance(quantity, int) else quantity
+    _check(L.srhd_refine_flags(cons_in.data_ptr(), npg, q, float(c_q), float(mom_over_d), C.byref(par),
+                               flags.data_ptr(), _stream()), L)
+    return flags
 
 
 def _bc(bc):
