@@ -37,8 +37,9 @@ def _multi_step(ref, prim, dh, bc, recon, riemann, cfl, nsteps=None, t_end=None,
     """Advance GPU and oracle side by side with the GPU's dt; returns (gpu grid, oracle grid, steps)."""
     st = _stepper(prim, dh, bc, recon, riemann, cfl, inflow, exact)
     par = ref.params(recon, riemann)
-    o = st.grid.cpu().numpy().copy()            # identical starting point (GPU prim2cons is within 1e-13)
-    o_inflow = None if st.inflow is None else (st.inflow[0].cpu().numpy(), np.array(st.inflow[1]))
+    # the oracle starts from ITS OWN prim2cons of the seeded primitives (nothing from the CUDA path)
+    o = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    o_inflow = None if inflow is None else (inflow[0], ref.prim2cons(np.asarray(inflow[1]).reshape(5, 1))[:, 0])
     n = 0
     while (nsteps is None or n < nsteps) and (t_end is None or st.t < t_end):
         dt = st.step(t_end)
