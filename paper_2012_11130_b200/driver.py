@@ -20,12 +20,15 @@ class GridStepper:
     """Owns the device buffers of one uniform grid (5, nz, ny, nx) of conserved variables."""
 
     def __init__(self, shape, dh, bc, recon="plm", riemann="hllc", cfl=0.4, inflow=None, exact=False,
-                 device="cuda", **par_overrides):
+                 device="cuda", dt_speed="signal", **par_overrides):
         nz, ny, nx = shape
         if nx % 16 or ny % 16 or nz % 16:
             raise B.SrhdError("grid extents must be multiples of 16 (whole patch groups)")
         self.shape, self.dh, self.bc, self.cfl, self.exact = (nz, ny, nx), float(dh), list(bc), float(cfl), exact
         self.par = B.params(recon, riemann, exact=exact, **par_overrides)
+        if dt_speed not in ("signal", "light"):
+            raise B.SrhdError("dt_speed must be 'signal' (Eq. 26-28) or 'light' (S_max replaced by c, P:229)")
+        self.dt_speed = dt_speed
         self.npg = (nx // 16) * (ny // 16) * (nz // 16)
         self.ncell = nx * ny * nz
         nxt = 16 + 2 * self.par.ghost
@@ -48,7 +51,7 @@ class GridStepper:
             self.smax_inflow = float(B.max_signal_speed(c, self.par, exact=exact).cpu())
         self.t = 0.0
         self.nstep = 0
-        self.launches_per_step = 5   # c2p-max, smax finish, gather, fluid step, scatter
+        self.launches_per_step = 5 if dt_speed == "signal" else 3   # c2p-max, smax finish, gather, fluid step, scatter
 
     # ---- state in / out -------------------------------------------------------------------------
     def set_prim(self, prim):
@@ -70,6 +73,8 @@ class GridStepper:
 
     # ---- one step -------------------------------------------------------------------------------
     def signal_speed(self):
+        if self.dt_speed == "light":           # the conservative CFL condition, no reduction kernel
+            return 1.0
         B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
         return max(float(self.smax.cpu()), self.smax_inflow)   # the one device->host double per step
 

@@ -152,3 +152,19 @@ def test_patch_boundary_fluxes_parity(ref, recon, riemann):
             assert (np.abs(gf - wflux) / scale).max() <= 1e-11
             plain, _ = B.fluid_step(dev(tiles), dt, dh, B.params(recon, riemann, max_retry=3))
             assert np.array_equal(plain.cpu().numpy(), got.cpu().numpy())
+
+
+def test_speed_of_light_time_step_option(ref):
+    """the second CFL condition replaces S_max by c: dt = C dh exactly, no reduction kernel."""
+    from paper_2012_11130_b200 import workloads as wl
+    from paper_2012_11130_b200.driver import GridStepper
+    prim, dh, bc = wl.shock_tube(n_long=32, n_trans=16)
+    a = GridStepper(prim.shape[1:], dh, bc, "plm", "hllc", cfl=0.5, dt_speed="light").set_prim(prim)
+    b = GridStepper(prim.shape[1:], dh, bc, "plm", "hllc", cfl=0.5).set_prim(prim)
+    assert a.step() == 0.5 * dh
+    assert b.step() > 0.5 * dh                        # S_max < c: the signal-speed condition allows more
+    po = ref.params("plm", "hllc")
+    o = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    want, _ = ref.grid_step_tiled(o, 0.5 * dh, dh, po, bc)
+    from tests.gpu_util import l1_rel
+    assert l1_rel(a.grid.cpu().numpy(), want).max() <= 1e-11
