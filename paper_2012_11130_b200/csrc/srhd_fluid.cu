@@ -176,6 +176,32 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   const int hd = (lane < 30) ? lane % 3 : 2;
   const int hc = (lane < 30) ? lane / 3 : 9;
   const int hbase = 3 * hc;
+  // Each thread meets the same two (cell, direction) items in every plane (chunks warp and warp + NW
+  // of the 32): decode them once.  info = in-plane tile index | store offset << 9 | has-edge-array
+  // << 18 | interior-column << 19
+  static_assert(NW * 2 * 10 >= 320, "two Hancock rounds must cover the 320 cells");
+  double* const hpm = (hd == 0) ? XSm : ((hd == 1) ? YSm : ZSm);
+  double* const hpp = (hd == 0) ? XSp : ((hd == 1) ? YSp : ZSp);
+  const int hqs = (hd == 0) ? P::XS : ((hd == 1) ? P::YS : P::ZS);
+  int hinfo[2];
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    int cell = (warp + NW * r) * 10 + hc;
+    if (cell > 319) cell = 319;
+    int i, j;
+    if (cell < 256) {
+      i = cell & 15;
+      j = cell >> 4;
+    } else {
+      const int e = cell - 256, side = e >> 4, t = e & 15;
+      i = (side == 0) ? -1 : ((side == 1) ? 16 : t);
+      j = (side == 2) ? -1 : ((side == 3) ? 16 : t);
+    }
+    const int cidx = (j + G) * NXT + (i + G);
+    const int soff = (hd == 0) ? j * 18 + (i + 1) : ((hd == 1) ? (j + 1) * 16 + i : cell);
+    const bool hs = (hd == 0) ? (j >= 0 && j <= 15) : ((hd == 1) ? (i >= 0 && i <= 15) : (cell < 256));
+    hinfo[r] = cidx | ((hs ? soff : 0) << 9) | ((hs ? 1 : 0) << 18) | ((cell < 256 ? 1 : 0) << 19);
+  }
 
   const double hdt = dt / (2.0 * dh);
   const double dtdh = dt / dh;
@@ -257,24 +283,14 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
       // ---- interval Y: edge states + Hancock half step of plane kh (S3-S5)
       if (kh >= -1 && kh <= 16) {
         const bool inplane = (kh >= 0) && (kh <= 15);
-        const int nh = inplane ? 320 : 256;       // interior columns + the ring of cells around them
-        const int nchunk = (nh + 9) / 10;
+        const int nchunk = inplane ? 32 : 26;     // 320 cells (interior columns + the ring around them) or 256
         const int tk = kh + G;
         const int zb = (kh + 2) & 1;
-        for (int chunk = warp; chunk < nchunk; chunk += NW) {
-          int cell = chunk * 10 + hc;
-          const bool valid = (lane < 30) && (cell < nh);
-          if (cell >= nh) cell = nh - 1;
-          int i, j;
-          if (cell < 256) {
-            i = cell & 15;
-            j = cell >> 4;
-          } else {
-            const int e = cell - 256, side = e >> 4, t = e & 15;
-            i = (side == 0) ? -1 : ((side == 1) ? 16 : t);
-            j = (side == 2) ? -1 : ((side == 3) ? 16 : t);
-          }
-          const int cidx = (j + G) * NXT + (i + G);
+        for (int r = 0; r < 2; ++r) {
+          if (warp + NW * r >= nchunk) break;       // warp uniform
+          const int info = hinfo[r];
+          const int cidx = info & 511, soff = (info >> 9) & 511;
+          const bool valid = (lane < 30) && (inplane || ((info >> 19) & 1));
           int o[2 * G - 1];
 #pragma unroll
           for (int m = -(G - 1); m <= G - 1; ++m)
@@ -282,26 +298,10 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
                                      : ((tk % R) * 5 * PL + cidx + m * ((hd == 0) ? 1 : NXT));
           double um[5], up[5], dF[5];
           hancock_lane<G>(Wr, hd, o, beta, beta0, um, up, dF);
-          double* pm;
-          double* pp;
-          int qs;
-          bool has;
-          if (hd == 0) {
-            pm = XSm + j * 18 + (i + 1);
-            pp = XSp + j * 18 + (i + 1);
-            qs = P::XS;
-            has = inplane && (j >= 0) && (j <= 15);
-          } else if (hd == 1) {
-            pm = YSm + (j + 1) * 16 + i;
-            pp = YSp + (j + 1) * 16 + i;
-            qs = P::YS;
-            has = inplane && (i >= 0) && (i <= 15);
-          } else {
-            pm = ZSm + cell;
-            pp = ZSp + zb * 5 * P::ZS + cell;
-            qs = P::ZS;
-            has = cell < 256;
-          }
+          double* pm = hpm + soff;
+          double* pp = hpp + soff + ((hd == 2) ? zb * 5 * P::ZS : 0);
+          const int qs = hqs;
+          bool has = ((info >> 18) & 1) && (hd == 2 || inplane);
           has = has && valid;
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
