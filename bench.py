@@ -281,6 +281,12 @@ def run_conv(args):
     print(json.dumps(out))
 
 
+# Warp-instruction counts of ONE fluid_step_kernel launch from the ncu capture named beside them
+# (smsp__inst_executed.sum and its fp64 part): feed the issue-cycle accounting of DESIGN.md section 6
+# (an fp64 warp instruction holds a sub-partition's issue port for 2 cycles, any other for 1).
+NCU_WARP_INST = {"blast256": {"fp64": 1.623e9, "other": 1.837e9, "source": "profiles/r1d_fluid_step_ppm_hllc.md"}}
+
+
 def run_ours(args):
     if args.workload == "conv":
         return run_conv(args)
@@ -400,6 +406,13 @@ def run_ours(args):
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
     hbm_ach = ncell * fm.FLUID_STEP_BYTES_PER_CELL / (k_ms * 1e-3) / 1e9
+    issue = None
+    if args.workload in NCU_WARP_INST and args.scale == 1:
+        wi = NCU_WARP_INST[args.workload]
+        cycles = k_ms * 1e-3 * (clocks["sm_mhz"] or clocks["sm_max_mhz"] or 1965.0) * 1e6 * fm.NUM_SMS * 4
+        issue = {"frac": (2 * wi["fp64"] + wi["other"]) / cycles, "fp64_pipe_frac": 2 * wi["fp64"] / cycles,
+                 "fp64_warp_inst": wi["fp64"], "other_warp_inst": wi["other"], "counts_from": wi["source"],
+                 "rule": "fp64 instruction = 2 issue cycles per sub-partition, any other = 1 (measured, DESIGN.md section 6)"}
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -417,7 +430,7 @@ def run_ours(args):
                      "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
                      "peak_measured_source": "srhd_fp64_peak_probe (register-only DFMA loop) in this run",
                      "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (ms / args.steps),
-                     "flops_per_cell": flops / ncell,
+                     "flops_per_cell": flops / ncell, "issue_cycles": issue,
                      "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
                              "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"}},
         "gpu_launches": st.launches_per_step * args.steps,
