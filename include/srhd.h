@@ -151,6 +151,12 @@ int srhd_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz
                      void* stream);
 int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz, void* stream);
 
+/* srhd_grid_scatter fused with srhd_max_signal_speed of the state it writes: *d_max_speed (device)
+ * receives S_max (Eq. 26-27) of the scattered grid, ready for the next step's dt (Eq. 28).  The copy is
+ * memory bound and the conversion ALU bound, so the fused kernel costs about as much as the slower one. */
+int srhd_grid_scatter_speed(const double* cons_out, double* grid, int nx, int ny, int nz,
+                            const srhd_params* params, double* d_max_speed, void* stream);
+
 /* Measurement helper (not part of the solver): launches a register-only DFMA loop that fills every
  * fp64 lane of the GPU (148 x 8 CTAs x 256 threads, 32*iters dependent-chain DFMA per thread in 8
  * independent chains) on `stream`; *flops (HOST pointer, may be NULL) receives the flop count of the

@@ -38,7 +38,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed",
            "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -78,6 +78,8 @@ def load_library(exact=False):
                                    C.POINTER(C.c_double), _VP]
     L.srhd_grid_scatter.restype = C.c_int
     L.srhd_grid_scatter.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, _VP]
+    L.srhd_grid_scatter_speed.restype = C.c_int
+    L.srhd_grid_scatter_speed.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, C.POINTER(Params), _VP, _VP]
     L.srhd_fp64_peak_probe.restype = C.c_int
     L.srhd_fp64_peak_probe.argtypes = [_VP, C.c_int, C.POINTER(C.c_ulonglong), _VP]
     L.srhd_error_string.restype = C.c_char_p
@@ -250,6 +252,19 @@ def grid_scatter(cons_out, shape, grid=None, exact=False):
         grid = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=cons_out.device)
     _check(L.srhd_grid_scatter(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, _stream()), L)
     return grid
+
+
+def grid_scatter_speed(cons_out, shape, par, grid=None, out=None, exact=False):
+    """srhd_grid_scatter_speed: scatter + S_max of the scattered state (1-element device tensor)."""
+    L = load_library(exact)
+    cons_out = _dev(cons_out, "cons_out")
+    nz, ny, nx = shape
+    if grid is None:
+        grid = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=cons_out.device)
+    out = torch.empty(1, dtype=torch.float64, device=cons_out.device) if out is None else out
+    _check(L.srhd_grid_scatter_speed(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, C.byref(par),
+                                     out.data_ptr(), _stream()), L)
+    return grid, out
 
 
 def fp64_peak_probe(iters=4096, reps=5):

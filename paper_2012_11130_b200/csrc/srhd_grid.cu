@@ -72,6 +72,41 @@ __global__ void __launch_bounds__(256) grid_scatter_kernel(const double* __restr
   }
 }
 
+// The scatter fused with the CFL reduction of the state it writes (Eq. 26): one CTA per patch group,
+// each thread moves all five components of its cells, converts them (cons2prim) and keeps the
+// running max of U_max; the copy is memory bound and the conversion ALU bound, so they overlap.
+__global__ void __launch_bounds__(256) grid_scatter_speed_kernel(const double* __restrict__ cons_out,
+                                                                 double* __restrict__ grid, int nx, int ny, int nz,
+                                                                 double rtol, int max_iter,
+                                                                 double* __restrict__ umax_out) {
+  const int px = nx / 16, py = ny / 16;
+  const int pg = blockIdx.x;
+  const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+  const size_t n = (size_t)nx * ny * nz;
+  const double* __restrict__ src = cons_out + (size_t)pg * 8 * 5 * 512;
+  double umax = 0.0;
+  for (int c = threadIdx.x; c < 4096; c += 256) {          // 4096 = 16 x 256: every lane of every warp works
+    const int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
+    const int p = (i >> 3) + 2 * (j >> 3) + 4 * (k >> 3);
+    const size_t so = (size_t)p * 5 * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7);
+    const size_t go = ((size_t)(gz * 16 + k) * ny + (gy * 16 + j)) * nx + (gx * 16 + i);
+    double U[1][5], W[1][5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      U[0][q] = __ldg(src + so + (size_t)q * 512);
+      grid[(size_t)q * n + go] = U[0][q];
+    }
+    bool phys[1];
+    int it[1];
+    Aux aux[1];
+    cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
+    umax = fmax(umax, umax_of_prim(W[0], aux[0]));
+  }
+  umax = warp_max(umax);
+  if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax_out, umax);
+}
+__global__ void smax_finish_kernel2(double* v) { *v = smax_of_umax(*v); }   // Eq. 27 once, after the max
+
 }  // namespace srhd
 
 using namespace srhd;
@@ -112,6 +147,23 @@ extern "C" int srhd_grid_scatter(const double* cons_out, double* grid, int nx, i
   if (ce) return ce;
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   grid_scatter_kernel<<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(cons_out, grid, nx, ny, nz);
+  return (int)cudaGetLastError();
+}
+
+extern "C" int srhd_grid_scatter_speed(const double* cons_out, double* grid, int nx, int ny, int nz,
+                                       const srhd_params* params, double* d_max_speed, void* stream) {
+  if (!cons_out || !grid || !d_max_speed) return SRHD_ERR_NULL_POINTER;
+  const int pc = check_params(params);
+  if (pc) return pc;
+  const int ce = check_extents(nx, ny, nz);
+  if (ce) return ce;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(double), st);
+  if (e != cudaSuccess) return (int)e;
+  const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  grid_scatter_speed_kernel<<<npg, 256, 0, st>>>(cons_out, grid, nx, ny, nz, newton_stop_rtol(params->newton_rtol),
+                                                 params->newton_max_iter, d_max_speed);
+  smax_finish_kernel2<<<1, 1, 0, st>>>(d_max_speed);
   return (int)cudaGetLastError();
 }
 

@@ -51,7 +51,8 @@ class GridStepper:
             self.smax_inflow = float(B.max_signal_speed(c, self.par, exact=exact).cpu())
         self.t = 0.0
         self.nstep = 0
-        self.launches_per_step = 5 if dt_speed == "signal" else 3   # c2p-max, smax finish, gather, fluid step, scatter
+        self._smax_fresh = False   # True when self.smax holds S_max of self.grid (written by the fused scatter)
+        self.launches_per_step = 4 if dt_speed == "signal" else 3   # gather, fluid step, scatter(+speed), smax finish
 
     # ---- state in / out -------------------------------------------------------------------------
     def set_prim(self, prim):
@@ -59,11 +60,13 @@ class GridStepper:
         p = prim if isinstance(prim, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(prim))
         p = p.to(self.grid.device).reshape(5, -1).contiguous()
         B.prim2cons(p, cons=self.grid.view(5, -1), exact=self.exact)
+        self._smax_fresh = False
         return self
 
     def set_cons(self, cons):
         c = cons if isinstance(cons, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(cons))
-        self.grid.copy_(c.reshape(self.grid.shape))
+        self.grid.copy_(c.reshape(self.grid.shape), non_blocking=True)
+        self._smax_fresh = False
         return self
 
     def prim(self):
@@ -75,6 +78,8 @@ class GridStepper:
     def signal_speed(self):
         if self.dt_speed == "light":           # the conservative CFL condition, no reduction kernel
             return 1.0
+        if self._smax_fresh:                   # the previous step's scatter already reduced this state
+            return max(float(self.smax.cpu()), self.smax_inflow)
         B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
         return max(float(self.smax.cpu()), self.smax_inflow)   # the one device->host double per step
 
@@ -90,7 +95,11 @@ class GridStepper:
         if kernel_events is not None:
             e1.record()
             kernel_events.append((e0, e1))
-        B.grid_scatter(self.patches, self.shape, grid=self.grid, exact=self.exact)
+        if self.dt_speed == "signal":          # scatter fused with the CFL reduction of the new state
+            B.grid_scatter_speed(self.patches, self.shape, self.par, grid=self.grid, out=self.smax, exact=self.exact)
+            self._smax_fresh = True
+        else:
+            B.grid_scatter(self.patches, self.shape, grid=self.grid, exact=self.exact)
         self.t += dt
         self.nstep += 1
 

@@ -168,3 +168,24 @@ def test_speed_of_light_time_step_option(ref):
     want, _ = ref.grid_step_tiled(o, 0.5 * dh, dh, po, bc)
     from tests.gpu_util import l1_rel
     assert l1_rel(a.grid.cpu().numpy(), want).max() <= 1e-11
+
+
+def test_fused_scatter_speed_equals_scatter_then_max_signal_speed(ref):
+    rng = np.random.default_rng(4)
+    prim = wl.random_patch_groups(6, 0, seed=8, rough=0.1)             # (6,5,16,16,16) primitives
+    cons = ref.prim2cons(prim.transpose(1, 0, 2, 3, 4).reshape(5, -1)).reshape(5, 6, 16, 16, 16)
+    # patch layout (npg,8,5,8,8,8) of a 32x16x48 grid
+    blocks = cons.transpose(1, 0, 2, 3, 4)
+    patches = np.ascontiguousarray(
+        blocks.reshape(6, 5, 2, 8, 2, 8, 2, 8).transpose(0, 2, 4, 6, 1, 3, 5, 7).reshape(6, 8, 5, 8, 8, 8))
+    for exact in (True, False):
+        par = B.params("plm", "hllc", exact=exact)
+        grid, smax = B.grid_scatter_speed(dev(patches), (32, 16, 48), par, exact=exact)
+        plain = B.grid_scatter(dev(patches), (32, 16, 48), exact=exact)
+        assert torch.equal(grid, plain)
+        assert np.array_equal(grid.cpu().numpy(), ref.grid_scatter(patches, (32, 16, 48)))
+        sep = B.max_signal_speed(plain.reshape(5, -1).contiguous(), par, exact=exact)
+        assert float(smax.cpu()) == float(sep.cpu())
+        want = ref.max_signal_speed(ref.grid_scatter(patches, (32, 16, 48)).reshape(5, -1))
+        assert abs(float(smax.cpu()) - want) <= (0.0 if exact else 1e-13) * want
+    assert rng is not None
