@@ -19,8 +19,9 @@ SRHD_DEV int map_index(int i, int n, int bc_lo, int bc_hi) {
   return i;
 }
 
-// one CTA per (patch group, component); a warp copies whole tile rows (lane = x index, so the x
-// mapping is computed once per thread), four rows in flight per warp
+// one CTA per (patch group, component): the tile is written as one contiguous run (fully coalesced
+// stores, all lanes busy); the tile extent is a compile-time constant so the index split is cheap;
+// four elements in flight per thread
 template <int G>
 __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restrict__ grid,
                                                           double* __restrict__ cons_in, int nx, int ny,
@@ -33,24 +34,27 @@ __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restri
   const size_t n = (size_t)nx * ny * nz;
   const double* __restrict__ src = grid + (size_t)q * n;
   double* __restrict__ dst = cons_in + ((size_t)pg * 5 + q) * t3;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (lane >= nxt) return;
-  const int si = map_index(gx * 16 + lane - G, nx, b.bc[0], b.bc[1]);
   const double inflow_q = b.inflow[q];
-  for (int r0 = warp * 4; r0 < nrow; r0 += 32) {
+  for (int c0 = threadIdx.x; c0 < t3; c0 += 4 * 256) {
     double v[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      const int r = r0 + u;                       // nrow is a multiple of 4
-      const int k = r / nxt, j = r - k * nxt;
-      const int kk = gz * 16 + k - G;
-      const int sj = map_index(gy * 16 + j - G, ny, b.bc[2], b.bc[3]);
-      const int sk = map_index(kk, nz, b.bc[4], b.bc[5]);
-      const bool inflow = b.has_inflow && kk < 0 && mask[(size_t)sj * nx + si];
-      v[u] = inflow ? inflow_q : __ldg(src + ((size_t)sk * ny + sj) * nx + si);
+      const int c = c0 + u * 256;
+      if (c < t3) {
+        const int k = c / nrow, r = c - k * nrow, j = r / nxt, i = r - j * nxt;
+        const int kk = gz * 16 + k - G;
+        const int si = map_index(gx * 16 + i - G, nx, b.bc[0], b.bc[1]);
+        const int sj = map_index(gy * 16 + j - G, ny, b.bc[2], b.bc[3]);
+        const int sk = map_index(kk, nz, b.bc[4], b.bc[5]);
+        const bool inflow = b.has_inflow && kk < 0 && mask[(size_t)sj * nx + si];
+        v[u] = inflow ? inflow_q : __ldg(src + ((size_t)sk * ny + sj) * nx + si);
+      }
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u) dst[(r0 + u) * nxt + lane] = v[u];
+    for (int u = 0; u < 4; ++u) {
+      const int c = c0 + u * 256;
+      if (c < t3) dst[c] = v[u];
+    }
   }
 }
 
