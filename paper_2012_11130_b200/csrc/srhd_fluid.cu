@@ -325,8 +325,9 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
         const int np1 = (s + 1 < NXT) ? NP1 : 0;
         const int zbl = (kh + 1) & 1;             // buffer of plane kh-1
         bool zfirst = (kh >= 0) && (kh <= 16) && (warp < 8);
-        for (;;) {
-          int idx;                                // face index, or -1 - chunk for a cons2prim chunk
+        int cq = -1;                              // queue ticket that turned out to be a cons2prim chunk
+        for (;;) {                                // ---- face chunks
+          int idx;
           if (zfirst) {
             zfirst = false;
             idx = tid;
@@ -334,12 +335,11 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
             int c = 0;
             if (lane == 0) c = atomicAdd(&ctl->queue, 1);
             c = __shfl_sync(0xffffffffu, c, 0);
-            if (c >= nxy + np1) break;
-            idx = (c < nxy) ? 256 + c * 32 + lane : -1 - (c - nxy);
-          }
-          if (idx < 0) {
-            convert_chunk(s + 1, -1 - idx);
-            continue;
+            if (c >= nxy) {
+              cq = c;
+              break;
+            }
+            idx = 256 + c * 32 + lane;
           }
           int d, qs;
           const double *pL, *pR;
@@ -421,6 +421,12 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
 #pragma unroll
             for (int q = 0; q < 5; ++q) FY[q * P::NFXY + (idx - 256 - P::NFXY)] = F[q];
           }
+        }
+        while (cq < nxy + np1) {                  // ---- cons2prim chunks of the next tile plane
+          convert_chunk(s + 1, cq - nxy);
+          int c = 0;
+          if (lane == 0) c = atomicAdd(&ctl->queue, 1);
+          cq = __shfl_sync(0xffffffffu, c, 0);
         }
       }
       __syncthreads();
