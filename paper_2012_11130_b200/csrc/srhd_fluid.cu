@@ -113,8 +113,19 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
     double a[2 * G - 1];
 #pragma unroll
     for (int m = 0; m < 2 * G - 1; ++m) a[m] = Wr[o[m] + q * P::PL];
-    if (G == 2) recon_plm(a, beta, wm[q], wp[q]);
-    else recon_ppm(a, beta, beta0, wm[q], wp[q]);
+    // A constant stencil (ambient gas ahead of a blast wave or a jet) has zero slopes and edge values
+    // equal to the cell value BIT FOR BIT in both schemes, so it skips the limiter arithmetic.
+    bool flat = true;
+#pragma unroll
+    for (int m = 0; m < 2 * G - 1; ++m) flat = flat && (a[m] == a[G - 1]);
+    if (flat) {
+      wm[q] = a[G - 1];
+      wp[q] = a[G - 1];
+    } else if (G == 2) {
+      recon_plm(a, beta, wm[q], wp[q]);
+    } else {
+      recon_ppm(a, beta, beta0, wm[q], wp[q]);
+    }
   }
   double Fm[5], Fp[5];
   Aux am, ap;
