@@ -108,6 +108,7 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
                            double beta0, double um[5], double up[5], double dF[5]) {
   using P = Plan<G>;
   double wm[5], wp[5];
+  bool allflat = true;
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
     double a[2 * G - 1];
@@ -118,6 +119,7 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
     bool flat = true;
 #pragma unroll
     for (int m = 0; m < 2 * G - 1; ++m) flat = flat && (a[m] == a[G - 1]);
+    allflat = allflat && flat;
     if (flat) {
       wm[q] = a[G - 1];
       wp[q] = a[G - 1];
@@ -129,7 +131,17 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
   }
   double Fm[5], Fp[5];
   Aux am, ap;
-  prim2cons_aux(wm, um, am);
+  if (__all_sync(0xffffffffu, allflat)) {
+    // every lane's two edge states are the same state: one conversion, and F(W+) - F(W-) = +0 exactly
+    prim2cons_aux(wm, um, am);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      up[q] = um[q];
+      dF[q] = 0.0;
+    }
+    return;
+  }
+  prim2cons_aux(wm, um, am);      // two independent chains: the compiler interleaves them
   prim2cons_aux(wp, up, ap);
   phys_flux_rt(d, wm, um, am, Fm);
   phys_flux_rt(d, wp, up, ap, Fp);
