@@ -393,8 +393,24 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           bool phys[2];
           int it[2];
           Aux aux[2];
-          cons2prim_multi<2>(U, W, aux, rtol, max_iter, phys, it);
-          riemann_flux<RS>(d, W[0], U[0], aux[0], W[1], U[1], aux[1], F);
+          // Faces inside a uniform region carry the same state on both sides: when that holds for
+          // the whole warp one conversion serves both (cons2prim is a function of its input, so the
+          // bits are those of converting twice; the iteration counter still counts both).
+          bool same = true;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) same = same && (U[0][q] == U[1][q]);
+          same = __all_sync(0xffffffffu, same);
+          if (same) {
+            cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) W[1][q] = W[0][q];
+            aux[1] = aux[0];
+            phys[1] = phys[0];
+            it[1] = it[0];
+          } else {
+            cons2prim_multi<2>(U, W, aux, rtol, max_iter, phys, it);
+          }
+          riemann_flux<RS>(d, W[0], U[0], aux[0], W[1], U[1], aux[1], F, same);
           my_iters += (unsigned)(it[0] + it[1]);
           my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
           if (fout) {                               // faces on the boundary of an 8^3 patch
