@@ -126,6 +126,16 @@ int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux
                            double dt, double dh, const srhd_params* params, srhd_stats* stats,
                            void* stream);
 
+/* The same step with the time step formed ON THE DEVICE from a signal speed that is already there
+ * (srhd_max_signal_speed / srhd_grid_scatter_speed wrote it): dt = cfl * dh / max(*d_max_speed, min_speed)
+ * (Eq. 28).  No host round trip for dt, so a sequence of steps can be enqueued without a
+ * synchronisation.  d_max_speed: device, one double, read by every CTA at kernel start; min_speed >= 0
+ * bounds the speed from below (e.g. the signal speed of a fixed-inflow state that is not in the
+ * grid yet); the caller guarantees max(*d_max_speed, min_speed) > 0.  flux_out may be NULL. */
+int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_out, int npg, double cfl,
+                        double dh, const double* d_max_speed, double min_speed,
+                        const srhd_params* params, srhd_stats* stats, void* stream);
+
 /* Refinement criteria of the SRHD module (section 3.1; Eq. 33), one flag per 8^3 patch,
  * on the same ghosted tiles as srhd_fluid_step (cons_in: [npg][5][nxt]^3, nxt = 16 + 2*params->ghost).
  *   flags[pg*8 + p] = 1 if ANY cell of patch p (S13) satisfies

@@ -38,7 +38,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed",
            "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -69,6 +69,8 @@ def load_library(exact=False):
     L.srhd_fluid_step.argtypes = [_VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_fluid_step_fluxes.restype = C.c_int
     L.srhd_fluid_step_fluxes.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
+    L.srhd_fluid_step_cfl.restype = C.c_int
+    L.srhd_fluid_step_cfl.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, _VP, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_refine_flags.restype = C.c_int
     L.srhd_refine_flags.argtypes = [_VP, C.c_int, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_workspace_bytes.restype = C.c_size_t
@@ -199,6 +201,22 @@ def fluid_step_fluxes(cons_in, dt, dh, par, cons_out=None, flux_out=None, stats=
                                     _dev(flux_out, "flux_out").data_ptr(), npg, float(dt), float(dh),
                                     C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, flux_out, stats
+
+
+def fluid_step_cfl(cons_in, cfl, dh, max_speed, par, min_speed=0.0, cons_out=None, flux_out=None, stats=None,
+                   exact=False):
+    """srhd_fluid_step_cfl: dt = cfl*dh/max(*max_speed, min_speed) formed on the device (no host sync)."""
+    L = load_library(exact)
+    cons_in = _dev(cons_in, "cons_in")
+    npg = cons_in.shape[0]
+    if cons_out is None:
+        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=torch.float64, device=cons_in.device)
+    stats = new_stats(cons_in.device) if stats is None else stats
+    _check(L.srhd_fluid_step_cfl(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(),
+                                 0 if flux_out is None else _dev(flux_out, "flux_out").data_ptr(), npg,
+                                 float(cfl), float(dh), _dev(max_speed, "max_speed").data_ptr(), float(min_speed),
+                                 C.byref(par), stats.data_ptr(), _stream()), L)
+    return cons_out, stats
 
 
 REFINE_Q = {None: 0, "none": 0, "D": 1, "Etilde": 2, "rho": 3, "gamma": 4}

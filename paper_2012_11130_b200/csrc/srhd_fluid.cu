@@ -153,7 +153,8 @@ template <int G, int RS>
 __global__ void __launch_bounds__(kFluidThreads, 1)
 fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out,
                   double* __restrict__ flux_out, double dt, double dh, double beta0, int max_retry, double rtol,
-                  int max_iter, srhd_stats* __restrict__ stats) {
+                  int max_iter, srhd_stats* __restrict__ stats, const double* __restrict__ d_smax, double cfl,
+                  double min_speed) {
   using P = Plan<G>;
   constexpr int NT = kFluidThreads, NW = NT / 32;
   constexpr int NXT = P::NXT, PL = P::PL, T3 = P::T3, R = P::R;
@@ -226,6 +227,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     hinfo[r] = cidx | ((hs ? soff : 0) << 9) | ((hs ? 1 : 0) << 18) | ((cell < 256 ? 1 : 0) << 19);
   }
 
+  if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);   // Eq. 28 formed on the device (srhd_fluid_step_cfl)
   const double hdt = dt / (2.0 * dh);
   const double dtdh = dt / dh;
   unsigned long long my_iters = 0;
@@ -510,13 +512,15 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
 
 template <int G, int RS>
 int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-                 const srhd_params* p, srhd_stats* stats, cudaStream_t st) {
+                 const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
+                 double min_speed) {
   auto kern = fluid_step_kernel<G, RS>;
   const size_t smem = Plan<G>::bytes;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
   kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, flux_out, dt, dh, p->minmod_coeff, p->max_retry,
-                                         newton_stop_rtol(p->newton_rtol), p->newton_max_iter, stats);
+                                         newton_stop_rtol(p->newton_rtol), p->newton_max_iter, stats, d_smax, cfl,
+                                         min_speed);
   return (int)cudaGetLastError();
 }
 
@@ -526,9 +530,9 @@ using namespace srhd;
 
 extern "C" size_t srhd_workspace_bytes(int, const srhd_params*) { return 0; }
 
-extern "C" int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
-                                      double dt, double dh, const srhd_params* params, srhd_stats* stats,
-                                      void* stream) {
+static int fluid_step_impl(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt,
+                           double dh, const srhd_params* params, srhd_stats* stats, void* stream,
+                           const double* d_smax, double cfl, double min_speed) {
   if (npg > 0 && (!cons_in || !cons_out)) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
@@ -549,15 +553,31 @@ extern "C" int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, d
   if (npg == 0) return SRHD_OK;
   if (params->recon == SRHD_RECON_PLM) {
     return params->riemann == SRHD_RIEMANN_HLLE
-               ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st)
-               : launch_fluid<2, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st);
+               ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed)
+               : launch_fluid<2, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed);
   }
   return params->riemann == SRHD_RIEMANN_HLLE
-             ? launch_fluid<3, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st)
-             : launch_fluid<3, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st);
+             ? launch_fluid<3, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed)
+             : launch_fluid<3, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed);
+}
+
+extern "C" int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+                                      double dt, double dh, const srhd_params* params, srhd_stats* stats,
+                                      void* stream) {
+  return fluid_step_impl(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, stream, nullptr, 0.0, 0.0);
 }
 
 extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
                                const srhd_params* params, srhd_stats* stats, void* stream) {
-  return srhd_fluid_step_fluxes(cons_in, cons_out, nullptr, npg, dt, dh, params, stats, stream);
+  return fluid_step_impl(cons_in, cons_out, nullptr, npg, dt, dh, params, stats, stream, nullptr, 0.0, 0.0);
+}
+
+extern "C" int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_out, int npg, double cfl,
+                                   double dh, const double* d_max_speed, double min_speed,
+                                   const srhd_params* params, srhd_stats* stats, void* stream) {
+  if (!d_max_speed) return SRHD_ERR_NULL_POINTER;
+  if (!(cfl > 0.0) || !std::isfinite(cfl) || !(min_speed >= 0.0)) return SRHD_ERR_BAD_STEP;
+  // dt is formed on the device; the host-side check of dt is replaced by the one of cfl (dt = 1 passes it)
+  return fluid_step_impl(cons_in, cons_out, flux_out, npg, 1.0, dh, params, stats, stream, d_max_speed, cfl,
+                         min_speed);
 }

@@ -111,6 +111,28 @@ class GridStepper:
         self.advance(dt, kernel_events)
         return dt
 
+    def step_async(self, kernel_events=None):
+        """One full step with NO host synchronisation: dt = C dh / S_max is formed on the device by
+        srhd_fluid_step_cfl from the speed the previous scatter (or a CFL kernel) left there.  The
+        host does not learn dt, so self.t is not advanced: use step() when the time matters."""
+        if self.dt_speed == "light":
+            return self.advance(self.cfl * self.dh, kernel_events)
+        if not self._smax_fresh:
+            B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
+        B.grid_gather(self.grid, self.par.ghost, self.bc, self.inflow, cons_in=self.tiles, exact=self.exact)
+        if kernel_events is not None:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+        B.fluid_step_cfl(self.tiles, self.cfl, self.dh, self.smax, self.par, min_speed=self.smax_inflow,
+                         cons_out=self.patches, stats=self.stats, exact=self.exact)
+        if kernel_events is not None:
+            e1.record()
+            kernel_events.append((e0, e1))
+        # the fluid step has read self.smax (stream order), the fused scatter may now overwrite it
+        B.grid_scatter_speed(self.patches, self.shape, self.par, grid=self.grid, out=self.smax, exact=self.exact)
+        self._smax_fresh = True
+        self.nstep += 1
+
     def run(self, nsteps=None, t_end=None):
         n = 0
         while (nsteps is None or n < nsteps) and (t_end is None or self.t < t_end):

@@ -189,3 +189,21 @@ def test_fused_scatter_speed_equals_scatter_then_max_signal_speed(ref):
         want = ref.max_signal_speed(ref.grid_scatter(patches, (32, 16, 48)).reshape(5, -1))
         assert abs(float(smax.cpu()) - want) <= (0.0 if exact else 1e-13) * want
     assert rng is not None
+
+
+def test_device_side_time_step_equals_host_side(ref):
+    """srhd_fluid_step_cfl forms dt = C dh / max(S_max, floor) on the device (Eq. 28): a run enqueued
+    without any host synchronisation must equal, bit for bit, the run whose dt went through the host."""
+    from paper_2012_11130_b200.driver import GridStepper
+    prim, dh, bc, inflow = wl.jet(nx=32, ny=32, nz=64, radius=0.16)
+    mask, prim_jet = inflow
+    cj = B.prim2cons(dev(prim_jet.reshape(5, 1))).cpu().numpy().ravel()
+    a = GridStepper(prim.shape[1:], dh, bc, "ppm", "hllc", cfl=0.4, inflow=(mask, cj)).set_prim(prim)
+    b = GridStepper(prim.shape[1:], dh, bc, "ppm", "hllc", cfl=0.4, inflow=(mask, cj)).set_prim(prim)
+    for _ in range(4):
+        a.step()
+        b.step_async()
+    torch.cuda.synchronize()
+    assert torch.equal(a.grid, b.grid)
+    assert float(a.smax.cpu()) == float(b.smax.cpu())
+    assert a.last_stats().as_dict() == b.last_stats().as_dict()
