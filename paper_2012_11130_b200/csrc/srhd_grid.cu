@@ -20,18 +20,30 @@ SRHD_DEV int map_index(int i, int n, int bc_lo, int bc_hi) {
 }
 
 // one CTA per (patch group, component): the tile is written as one contiguous run (fully coalesced
-// stores, all lanes busy); the tile extent is a compile-time constant so the index split is cheap;
-// four elements in flight per thread
+// stores, all lanes busy).  The boundary mapping of the 3 x nxt tile coordinates is done once per CTA
+// into shared-memory tables, so an element costs one index split (compile-time extents), three table
+// reads, one load and one store; four elements in flight per thread.
 template <int G>
 __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restrict__ grid,
                                                           double* __restrict__ cons_in, int nx, int ny,
                                                           int nz, GridBC b,
                                                           const unsigned char* __restrict__ mask) {
   constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
+  __shared__ int xs[nxt], ys[nxt];            // source x index; source y index * nx
+  __shared__ long long zs[nxt];               // source z index * ny * nx; -1 - that for a plane below z = 0
   const int px = nx / 16, py = ny / 16;
   const int pg = blockIdx.x, q = blockIdx.y;
   const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
   const size_t n = (size_t)nx * ny * nz;
+  if (threadIdx.x < nxt) {
+    const int t = threadIdx.x;
+    xs[t] = map_index(gx * 16 + t - G, nx, b.bc[0], b.bc[1]);
+    ys[t] = map_index(gy * 16 + t - G, ny, b.bc[2], b.bc[3]) * nx;
+    const int kk = gz * 16 + t - G;
+    const long long off = (long long)map_index(kk, nz, b.bc[4], b.bc[5]) * ny * nx;
+    zs[t] = (b.has_inflow && kk < 0) ? -1 - off : off;
+  }
+  __syncthreads();
   const double* __restrict__ src = grid + (size_t)q * n;
   double* __restrict__ dst = cons_in + ((size_t)pg * 5 + q) * t3;
   const double inflow_q = b.inflow[q];
@@ -42,12 +54,14 @@ __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restri
       const int c = c0 + u * 256;
       if (c < t3) {
         const int k = c / nrow, r = c - k * nrow, j = r / nxt, i = r - j * nxt;
-        const int kk = gz * 16 + k - G;
-        const int si = map_index(gx * 16 + i - G, nx, b.bc[0], b.bc[1]);
-        const int sj = map_index(gy * 16 + j - G, ny, b.bc[2], b.bc[3]);
-        const int sk = map_index(kk, nz, b.bc[4], b.bc[5]);
-        const bool inflow = b.has_inflow && kk < 0 && mask[(size_t)sj * nx + si];
-        v[u] = inflow ? inflow_q : __ldg(src + ((size_t)sk * ny + sj) * nx + si);
+        const int xy = ys[j] + xs[i];
+        long long z = zs[k];
+        bool inflow = false;
+        if (z < 0) {                              // ghost plane below z = 0 of a fixed-inflow boundary
+          z = -1 - z;
+          inflow = mask[xy] != 0;
+        }
+        v[u] = inflow ? inflow_q : __ldg(src + z + xy);
       }
     }
 #pragma unroll
@@ -138,10 +152,10 @@ extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   if (ghost == 2)
     grid_gather_kernel<2><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
-                                                                                        b, inflow_mask);
+                                                                                            b, inflow_mask);
   else
     grid_gather_kernel<3><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
-                                                                                        b, inflow_mask);
+                                                                                            b, inflow_mask);
   return (int)cudaGetLastError();
 }
 
