@@ -104,7 +104,7 @@ struct Ctl {                       // lives in shared memory
 // (stencil offsets o[] into the primitive ring, component stride PL), prim2cons and physical flux
 // of both edge states; returns the un-evolved conserved edge states and dF = F(W+) - F(W-).
 template <int G>
-SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 * G - 1], double beta,
+SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 * G - 1], double beta,
                            double beta0, double um[5], double up[5], double dF[5]) {
   using P = Plan<G>;
   double wm[5], wp[5];
@@ -139,7 +139,7 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
       up[q] = um[q];
       dF[q] = 0.0;
     }
-    return;
+    return true;
   }
   prim2cons_aux(wm, um, am);      // two independent chains: the compiler interleaves them
   prim2cons_aux(wp, up, ap);
@@ -147,6 +147,7 @@ SRHD_DEV void hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
   phys_flux_rt(d, wp, up, ap, Fp);
 #pragma unroll
   for (int q = 0; q < 5; ++q) dF[q] = Fp[q] - Fm[q];
+  return false;
 }
 
 template <int G, int RS>
@@ -322,12 +323,24 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
             o[m + G - 1] = (hd == 2) ? (((tk + m) % R) * 5 * PL + cidx)
                                      : ((tk % R) * 5 * PL + cidx + m * ((hd == 0) ? 1 : NXT));
           double um[5], up[5], dF[5];
-          hancock_lane<G>(Wr, hd, o, beta, beta0, um, up, dF);
+          const bool warp_flat = hancock_lane<G>(Wr, hd, o, beta, beta0, um, up, dF);
           double* pm = hpm + soff;
           double* pp = hpp + soff + ((hd == 2) ? zb * 5 * P::ZS : 0);
           const int qs = hqs;
           bool has = ((info >> 18) & 1) && (hd == 2 || inplane);
           has = has && valid;
+          if (warp_flat) {
+            // every flux difference of the warp is +0: the common increment is -hdt*0 = -0 and
+            // x + (-0) = x bit for bit, so the evolved edge states are the un-evolved ones
+            if (has) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) {
+                pm[q * qs] = um[q];
+                pp[q * qs] = up[q];
+              }
+            }
+            continue;
+          }
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
             const double fx = __shfl_sync(0xffffffffu, dF[q], hbase);
