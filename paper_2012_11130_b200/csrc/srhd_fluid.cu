@@ -22,10 +22,8 @@
 
 namespace srhd {
 
-#ifndef SRHD_FLUID_THREADS
-#define SRHD_FLUID_THREADS 512
-#endif
-constexpr int kFluidThreads = SRHD_FLUID_THREADS;   // 16 warps, <= 128 registers per thread, one CTA per SM
+constexpr int kFluidThreads = 512;   // 16 warps, <= 128 registers per thread, one CTA per SM (384 ... 768
+                                     // threads were measured in round 1: 512 is best)
 
 // ---- TMA bulk copy + mbarrier (PTX; SASS: UBLKCP / SYNCS) -------------------------------------
 SRHD_DEV uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -204,7 +202,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   // Each thread meets the same two (cell, direction) items in every plane (chunks warp and warp + NW
   // of the 32): decode them once.  info = in-plane tile index | store offset << 9 | has-edge-array
   // << 18 | interior-column << 19
-  static_assert(NW * 2 * 10 >= 320, "two Hancock rounds must cover the 320 cells");
+  static_assert(NW == 16, "the Hancock stage maps 32 chunks of 10 cells onto exactly two rounds of 16 warps");
   double* const hpm = (hd == 0) ? XSm : ((hd == 1) ? YSm : ZSm);
   double* const hpp = (hd == 0) ? XSp : ((hd == 1) ? YSp : ZSp);
   const int hqs = (hd == 0) ? P::XS : ((hd == 1) ? P::YS : P::ZS);
