@@ -73,6 +73,16 @@ def test_argument_errors_without_gpu():
     assert L.srhd_fluid_step(16, 1 << 30, -1, 0.1, 1.0, C.byref(p), None, None) == -3
     assert L.srhd_fluid_step(24, 1 << 30, 1, 0.1, 1.0, C.byref(p), None, None) == -6
     assert L.srhd_fluid_step(1 << 20, (1 << 20) + 64, 1, 0.1, 1.0, C.byref(p), None, None) == -5
+    # device-side dt variant: needs the speed pointer and a positive Courant number
+    assert L.srhd_fluid_step_cfl(16, 1 << 30, None, 1, 0.4, 1.0, None, 0.0, C.byref(p), None, None) == -1
+    assert L.srhd_fluid_step_cfl(16, 1 << 30, None, 1, 0.0, 1.0, 64, 0.0, C.byref(p), None, None) == -4
+    assert L.srhd_fluid_step_cfl(16, 1 << 30, None, 1, 0.4, -1.0, 64, 0.0, C.byref(p), None, None) == -4
+    # refinement flags: quantity and thresholds are checked
+    assert L.srhd_refine_flags(16, 1, 9, 0.3, 0.0, C.byref(p), 64, None) == -2
+    assert L.srhd_refine_flags(16, 1, 3, -1.0, 0.0, C.byref(p), 64, None) == -2
+    assert L.srhd_refine_flags(None, 1, 3, 0.3, 0.0, C.byref(p), 64, None) == -1
+    assert L.srhd_grid_scatter_speed(16, 32, 16, 16, 16, C.byref(p), None, None) == -1
+    assert L.srhd_fp64_peak_probe(None, 4, None, None) == -1
     bc = (C.c_int * 6)(0, 0, 0, 0, 0, 0)
     assert L.srhd_grid_gather(16, 32, 16, 24, 16, 2, bc, None, None, None) == -3
     assert L.srhd_grid_scatter(16, 32, 16, 16, 0, None) == -3
