@@ -18,3 +18,11 @@ def ref():
     from oracle import ref as _ref
     _ref.lib()
     return _ref
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_libraries():
+    """Make sure the in-tree C-ABI libraries exist and are current (nvcc cross-compiles without a GPU;
+    a no-op when they are fresh).  The tests never fall back to anything else if this fails."""
+    from paper_2012_11130_b200 import build
+    build.build()
