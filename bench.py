@@ -4,8 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload blast256|random512|jet|tube|conv]
                     [--impl ours|reference] [--no-e2e] [--no-cpu-baseline]
 
-A "step" is one pass of the whole hot path over the grid (driver.GridStepper.step): the CFL
-reduction (srhd_max_signal_speed), ghost-zone gather, srhd_fluid_step, scatter.  Default workload:
+A "step" is one pass of the whole hot path over the grid (driver.GridStepper.step_async): ghost-zone
+fill from the patches of the previous step fused with the CFL reduction (srhd_patch_gather_speed), then
+srhd_fluid_step_cfl (dt formed on the device).  Default workload:
 BASELINE.json configs[2] (256^3 spherical blast, PPM+HLLC, CFL 0.4) -- the 3-D fluid step the
 metric "fp64 SRHD cell updates/s" is quoted on.  N > 1 runs N independent
 replicas (the path does not shard on this tier: DESIGN.md section 8); value = all ranks' cell

@@ -167,6 +167,16 @@ int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int 
 int srhd_grid_scatter_speed(const double* cons_out, double* grid, int nx, int ny, int nz,
                             const srhd_params* params, double* d_max_speed, void* stream);
 
+/* Ghost-zone fill straight from the PATCH layout srhd_fluid_step wrote (cons_out of the previous
+ * step of the same uniform grid: patch group pg = gx + (nx/16)*(gy + (ny/16)*gz)), fused with
+ * srhd_max_signal_speed of that state: patches -> cons_in tiles (as srhd_grid_gather would build them
+ * from the scattered grid, bit for bit) and *d_max_speed = S_max.  With it a uniform-grid step is two
+ * kernels (this one and srhd_fluid_step_cfl) and the grid is only materialised on demand.  The ghost
+ * width is params->ghost.  Boundary arguments as srhd_grid_gather. */
+int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int ny, int nz, const int* bc,
+                            const unsigned char* inflow_mask, const double* inflow_cons,
+                            const srhd_params* params, double* d_max_speed, void* stream);
+
 /* Measurement helper (not part of the solver): launches a register-only DFMA loop that fills every
  * fp64 lane of the GPU (148 x 8 CTAs x 256 threads, 32*iters dependent-chain DFMA per thread in 8
  * independent chains) on `stream`; *flops (HOST pointer, may be NULL) receives the flop count of the

@@ -38,7 +38,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed",
            "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -82,6 +82,9 @@ def load_library(exact=False):
     L.srhd_grid_scatter.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, _VP]
     L.srhd_grid_scatter_speed.restype = C.c_int
     L.srhd_grid_scatter_speed.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, C.POINTER(Params), _VP, _VP]
+    L.srhd_patch_gather_speed.restype = C.c_int
+    L.srhd_patch_gather_speed.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), _VP,
+                                          C.POINTER(C.c_double), C.POINTER(Params), _VP, _VP]
     L.srhd_fp64_peak_probe.restype = C.c_int
     L.srhd_fp64_peak_probe.argtypes = [_VP, C.c_int, C.POINTER(C.c_ulonglong), _VP]
     L.srhd_error_string.restype = C.c_char_p
@@ -283,6 +286,25 @@ def grid_scatter_speed(cons_out, shape, par, grid=None, out=None, exact=False):
     _check(L.srhd_grid_scatter_speed(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, C.byref(par),
                                      out.data_ptr(), _stream()), L)
     return grid, out
+
+
+def patch_gather_speed(patches, shape, par, bc, inflow=None, cons_in=None, out=None, exact=False):
+    """srhd_patch_gather_speed: patches (npg,8,5,8,8,8) -> tiles (npg,5,nxt,nxt,nxt) and S_max (1 element)."""
+    L = load_library(exact)
+    patches = _dev(patches, "patches")
+    nz, ny, nx = shape
+    nxt = 16 + 2 * par.ghost
+    if cons_in is None:
+        cons_in = torch.empty((patches.shape[0], 5, nxt, nxt, nxt), dtype=torch.float64, device=patches.device)
+    out = torch.empty(1, dtype=torch.float64, device=patches.device) if out is None else out
+    mask_ptr, icons = None, None
+    if inflow is not None:
+        mask, vals = inflow
+        mask_ptr = mask.data_ptr()
+        icons = (C.c_double * 5)(*[float(v) for v in vals])
+    _check(L.srhd_patch_gather_speed(patches.data_ptr(), cons_in.data_ptr(), nx, ny, nz, _bc(bc), mask_ptr, icons,
+                                     C.byref(par), out.data_ptr(), _stream()), L)
+    return cons_in, out
 
 
 def fp64_peak_probe(iters=4096, reps=5):

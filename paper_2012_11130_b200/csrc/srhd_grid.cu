@@ -123,6 +123,84 @@ __global__ void __launch_bounds__(256) grid_scatter_speed_kernel(const double* _
   umax = warp_max(umax);
   if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax_out, umax);
 }
+// Ghost-zone fill straight from the patch layout the fluid step wrote (no uniform grid in between) fused
+// with the CFL reduction of that state: one CTA per destination patch group.  Loop A copies the
+// (16+2g)^3 tile cells of all five components from the source patches (boundary mapping of the three
+// tile axes in shared-memory tables, as in grid_gather_kernel); loop B converts the group's own 16^3
+// cells (cons2prim) and keeps the running max of U_max (Eq. 26).
+template <int G>
+__global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* __restrict__ patches,
+                                                                 double* __restrict__ cons_in, int nx, int ny,
+                                                                 int nz, GridBC b,
+                                                                 const unsigned char* __restrict__ mask,
+                                                                 double rtol, int max_iter,
+                                                                 double* __restrict__ umax_out) {
+  constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
+  __shared__ int ax[nxt], ay[nxt], mx[nxt], my[nxt];
+  __shared__ long long az[nxt];               // -1 - offset for a plane below z = 0 of an inflow boundary
+  const int px = nx / 16, py = ny / 16;
+  const int pg = blockIdx.x;
+  const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+  if (threadIdx.x < nxt) {
+    const int t = threadIdx.x;
+    const int X = map_index(gx * 16 + t - G, nx, b.bc[0], b.bc[1]);
+    const int Y = map_index(gy * 16 + t - G, ny, b.bc[2], b.bc[3]);
+    const int kk = gz * 16 + t - G;
+    const int Z = map_index(kk, nz, b.bc[4], b.bc[5]);
+    ax[t] = (X >> 4) * 20480 + ((X >> 3) & 1) * 2560 + (X & 7);
+    ay[t] = (Y >> 4) * px * 20480 + ((Y >> 3) & 1) * 2 * 2560 + (Y & 7) * 8;
+    mx[t] = X;
+    my[t] = Y * nx;
+    const long long off = (long long)(Z >> 4) * px * py * 20480 + ((Z >> 3) & 1) * 4 * 2560 + (Z & 7) * 64;
+    az[t] = (b.has_inflow && kk < 0) ? -1 - off : off;
+  }
+  __syncthreads();
+  double* __restrict__ dst = cons_in + (size_t)pg * 5 * t3;
+  for (int c0 = threadIdx.x; c0 < t3; c0 += 2 * 256) {     // loop A: two cells (ten loads) in flight
+    double v[2][5];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int c = c0 + u * 256;
+      if (c < t3) {
+        const int k = c / nrow, r = c - k * nrow, j = r / nxt, i = r - j * nxt;
+        long long z = az[k];
+        bool inflow = false;
+        if (z < 0) {
+          z = -1 - z;
+          inflow = mask[my[j] + mx[i]] != 0;
+        }
+        const double* __restrict__ sp = patches + z + ay[j] + ax[i];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) v[u][q] = inflow ? b.inflow[q] : __ldg(sp + q * 512);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int c = c0 + u * 256;
+      if (c < t3) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) dst[(size_t)q * t3 + c] = v[u][q];
+      }
+    }
+  }
+  // loop B: S_max of the group's own cells (every lane of every warp works: 4096 = 16 x 256)
+  const double* __restrict__ own = patches + (size_t)pg * 8 * 5 * 512;
+  double umax = 0.0;
+  for (int c = threadIdx.x; c < 4096; c += 256) {
+    const size_t so = (size_t)(c >> 9) * 5 * 512 + (c & 511);
+    double U[1][5], W[1][5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) U[0][q] = __ldg(own + so + (size_t)q * 512);
+    bool phys[1];
+    int it[1];
+    Aux aux[1];
+    cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
+    umax = fmax(umax, umax_of_prim(W[0], aux[0]));
+  }
+  umax = warp_max(umax);
+  if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax_out, umax);
+}
+
 __global__ void smax_finish_kernel2(double* v) { *v = smax_of_umax(*v); }   // Eq. 27 once, after the max
 
 }  // namespace srhd
@@ -181,6 +259,37 @@ extern "C" int srhd_grid_scatter_speed(const double* cons_out, double* grid, int
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   grid_scatter_speed_kernel<<<npg, 256, 0, st>>>(cons_out, grid, nx, ny, nz, newton_stop_rtol(params->newton_rtol),
                                                  params->newton_max_iter, d_max_speed);
+  smax_finish_kernel2<<<1, 1, 0, st>>>(d_max_speed);
+  return (int)cudaGetLastError();
+}
+
+extern "C" int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int ny, int nz,
+                                       const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
+                                       const srhd_params* params, double* d_max_speed, void* stream) {
+  if (!patches || !cons_in || !bc || !d_max_speed) return SRHD_ERR_NULL_POINTER;
+  const int pc = check_params(params);
+  if (pc) return pc;
+  const int ce = check_extents(nx, ny, nz);
+  if (ce) return ce;
+  GridBC b;
+  for (int i = 0; i < 6; ++i) {
+    if (bc[i] != SRHD_BC_PERIODIC && bc[i] != SRHD_BC_OUTFLOW) return SRHD_ERR_BAD_PARAMS;
+    b.bc[i] = bc[i];
+  }
+  b.has_inflow = (inflow_mask != nullptr);
+  if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
+  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(double), st);
+  if (e != cudaSuccess) return (int)e;
+  const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  const double rtol = newton_stop_rtol(params->newton_rtol);
+  if (params->ghost == 2)
+    patch_gather_speed_kernel<2><<<npg, 256, 0, st>>>(patches, cons_in, nx, ny, nz, b, inflow_mask, rtol,
+                                                      params->newton_max_iter, d_max_speed);
+  else
+    patch_gather_speed_kernel<3><<<npg, 256, 0, st>>>(patches, cons_in, nx, ny, nz, b, inflow_mask, rtol,
+                                                      params->newton_max_iter, d_max_speed);
   smax_finish_kernel2<<<1, 1, 0, st>>>(d_max_speed);
   return (int)cudaGetLastError();
 }

@@ -1,14 +1,17 @@
 """Uniform-grid stepper on top of the C-ABI calls: the "whole hot path" that bench.py times.
 
-One step (collapsed onto the GPU):
-    srhd_max_signal_speed(grid)          K2 of the paper: the CFL reduction (Eq. 26-28)
-    dt = C_CFL * dh / S_max              one double crosses to the host (Eq. 28, formed by the caller)
-    srhd_grid_gather(grid) -> tiles      ghost-zone fill of every 16^3 patch group (stands in for P:219)
-    srhd_fluid_step(tiles) -> patches    K1 of the paper: the fused MUSCL-Hancock update
-    srhd_grid_scatter(patches) -> grid
-
-Nothing here computes on the host except the scalar division for dt; all buffers are torch CUDA
-tensors allocated once.  There is no CPU fallback.
+The state lives in the PATCH layout the solver writes (cons_out of srhd_fluid_step: 8^3 patches, as in
+the paper's AMR code); a uniform grid (5, nz, ny, nx) is only materialised when it is asked for.
+One step (collapsed onto the GPU), 3 launches:
+    srhd_patch_gather_speed(patches) -> tiles, S_max   ghost-zone fill of every 16^3 patch group from the
+                                                       neighbouring patches (stands in for P:219) fused
+                                                       with the CFL reduction of that state (Eq. 26-27)
+    srhd_fluid_step_cfl(tiles) -> patches              the fused MUSCL-Hancock update with
+                                                       dt = C dh / S_max formed on the device (Eq. 28)
+The first step after set_prim / set_cons starts from the grid instead: srhd_max_signal_speed +
+srhd_grid_gather.  step() reads S_max back (one double) because the host wants t; step_async() does not
+synchronise.  Nothing here computes on the host except that scalar arithmetic; all buffers are torch
+CUDA tensors allocated once.  There is no CPU fallback.
 """
 import numpy as np
 import torch
@@ -17,7 +20,7 @@ from . import binding as B
 
 
 class GridStepper:
-    """Owns the device buffers of one uniform grid (5, nz, ny, nx) of conserved variables."""
+    """Owns the device buffers of one uniform grid of conserved variables."""
 
     def __init__(self, shape, dh, bc, recon="plm", riemann="hllc", cfl=0.4, inflow=None, exact=False,
                  device="cuda", dt_speed="signal", **par_overrides):
@@ -33,7 +36,7 @@ class GridStepper:
         self.ncell = nx * ny * nz
         nxt = 16 + 2 * self.par.ghost
         f64 = dict(dtype=torch.float64, device=device)
-        self.grid = torch.empty((5, nz, ny, nx), **f64)
+        self._grid = torch.empty((5, nz, ny, nx), **f64)
         self.tiles = torch.empty((self.npg, 5, nxt, nxt, nxt), **f64)
         self.patches = torch.empty((self.npg, 8, 5, 8, 8, 8), **f64)
         self.smax = torch.zeros(1, **f64)
@@ -51,87 +54,108 @@ class GridStepper:
             self.smax_inflow = float(B.max_signal_speed(c, self.par, exact=exact).cpu())
         self.t = 0.0
         self.nstep = 0
-        self._smax_fresh = False   # True when self.smax holds S_max of self.grid (written by the fused scatter)
-        self.launches_per_step = 4 if dt_speed == "signal" else 3   # gather, fluid step, scatter(+speed), smax finish
+        self._in_patches = False   # True: self.patches holds the current state (self._grid may be stale)
+        self._grid_stale = False
+        self.launches_per_step = 3   # ghost-zone fill (+ speed), smax finish (signal) or plain gather, fluid step
 
     # ---- state in / out -------------------------------------------------------------------------
+    @property
+    def grid(self):
+        """The current state as a uniform grid (5,nz,ny,nx); scattered from the patches on demand."""
+        if self._grid_stale:
+            B.grid_scatter(self.patches, self.shape, grid=self._grid, exact=self.exact)
+            self._grid_stale = False
+        return self._grid
+
     def set_prim(self, prim):
         """Upload a primitive field (5,nz,ny,nx) (numpy or CUDA tensor) and convert with srhd_prim2cons."""
         p = prim if isinstance(prim, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(prim))
-        p = p.to(self.grid.device).reshape(5, -1).contiguous()
-        B.prim2cons(p, cons=self.grid.view(5, -1), exact=self.exact)
-        self._smax_fresh = False
+        p = p.to(self._grid.device).reshape(5, -1).contiguous()
+        B.prim2cons(p, cons=self._grid.view(5, -1), exact=self.exact)
+        self._in_patches = self._grid_stale = False
         return self
 
     def set_cons(self, cons):
         c = cons if isinstance(cons, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(cons))
-        self.grid.copy_(c.reshape(self.grid.shape), non_blocking=True)
-        self._smax_fresh = False
+        self._grid.copy_(c.reshape(self._grid.shape), non_blocking=True)
+        self._in_patches = self._grid_stale = False
         return self
 
     def prim(self):
         """Primitive field of the current state via srhd_cons2prim (device tensor (5,nz,ny,nx))."""
         w, _ = B.cons2prim(self.grid.view(5, -1), self.par, exact=self.exact)
-        return w.view(self.grid.shape)
+        return w.view(self._grid.shape)
 
     # ---- one step -------------------------------------------------------------------------------
-    def signal_speed(self):
-        if self.dt_speed == "light":           # P:229: the conservative CFL condition, no reduction kernel
-            return 1.0
-        if self._smax_fresh:                   # the previous step's scatter already reduced this state
-            return max(float(self.smax.cpu()), self.smax_inflow)
-        B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
-        return max(float(self.smax.cpu()), self.smax_inflow)   # the one device->host double per step
-
-    def advance(self, dt, kernel_events=None):
-        """gather -> fluid_step -> scatter with a given dt (asynchronous on the current stream).
-        kernel_events: a list that receives a (start, end) CUDA event pair around srhd_fluid_step."""
-        B.grid_gather(self.grid, self.par.ghost, self.bc, self.inflow, cons_in=self.tiles, exact=self.exact)
-        if kernel_events is not None:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-        B.fluid_step(self.tiles, dt, self.dh, self.par, cons_out=self.patches, stats=self.stats,
-                     exact=self.exact)
-        if kernel_events is not None:
-            e1.record()
-            kernel_events.append((e0, e1))
-        if self.dt_speed == "signal":          # scatter fused with the CFL reduction of the new state
-            B.grid_scatter_speed(self.patches, self.shape, self.par, grid=self.grid, out=self.smax, exact=self.exact)
-            self._smax_fresh = True
+    def _fill_tiles(self, need_speed):
+        """Ghost-zone fill of the current state into self.tiles; S_max of it into self.smax if asked."""
+        if self._in_patches:
+            # fused: tiles from the neighbouring patches + CFL reduction (the speed costs nothing extra to skip)
+            B.patch_gather_speed(self.patches, self.shape, self.par, self.bc, self.inflow, cons_in=self.tiles,
+                                 out=self.smax, exact=self.exact)
         else:
-            B.grid_scatter(self.patches, self.shape, grid=self.grid, exact=self.exact)
-        self.t += dt
+            if need_speed:
+                B.max_signal_speed(self._grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
+            B.grid_gather(self._grid, self.par.ghost, self.bc, self.inflow, cons_in=self.tiles, exact=self.exact)
+
+    def _timed(self, kernel_events, launch):
+        if kernel_events is None:
+            return launch()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        launch()
+        e1.record()
+        kernel_events.append((e0, e1))
+
+    def _done(self):
+        self._in_patches = self._grid_stale = True
         self.nstep += 1
 
+    def advance(self, dt, kernel_events=None):
+        """Ghost-zone fill -> srhd_fluid_step with a given dt (asynchronous on the current stream)."""
+        self._fill_tiles(need_speed=False)
+        self._timed(kernel_events, lambda: B.fluid_step(self.tiles, dt, self.dh, self.par, cons_out=self.patches,
+                                                        stats=self.stats, exact=self.exact))
+        self.t += dt
+        self._done()
+
     def step(self, t_end=None, kernel_events=None):
-        """One full step: CFL reduction, dt (clipped to hit t_end exactly), update.  Returns dt."""
-        dt = self.cfl * self.dh / self.signal_speed()
+        """One full step with dt on the host: CFL reduction, dt (clipped to hit t_end exactly), update."""
+        if self.dt_speed == "light":           # P:229: the conservative CFL condition, no reduction
+            smax = 1.0
+        else:
+            self._fill_tiles(need_speed=True)
+            smax = max(float(self.smax.cpu()), self.smax_inflow)   # the one device->host double per step
+        dt = self.cfl * self.dh / smax
         if t_end is not None and self.t + dt > t_end:
             dt = t_end - self.t
-        self.advance(dt, kernel_events)
+        if self.dt_speed == "light":
+            self.advance(dt, kernel_events)
+            return dt
+        self._timed(kernel_events, lambda: B.fluid_step(self.tiles, dt, self.dh, self.par, cons_out=self.patches,
+                                                        stats=self.stats, exact=self.exact))
+        self.t += dt
+        self._done()
         return dt
 
     def step_async(self, kernel_events=None):
         """One full step with NO host synchronisation: dt = C dh / S_max is formed on the device by
-        srhd_fluid_step_cfl from the speed the previous scatter (or a CFL kernel) left there.  The
-        host does not learn dt, so self.t is not advanced: use step() when the time matters."""
+        srhd_fluid_step_cfl.  The host does not learn dt, so self.t is not advanced: use step() when
+        the time matters."""
         if self.dt_speed == "light":
             return self.advance(self.cfl * self.dh, kernel_events)
-        if not self._smax_fresh:
-            B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
-        B.grid_gather(self.grid, self.par.ghost, self.bc, self.inflow, cons_in=self.tiles, exact=self.exact)
-        if kernel_events is not None:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-        B.fluid_step_cfl(self.tiles, self.cfl, self.dh, self.smax, self.par, min_speed=self.smax_inflow,
-                         cons_out=self.patches, stats=self.stats, exact=self.exact)
-        if kernel_events is not None:
-            e1.record()
-            kernel_events.append((e0, e1))
-        # the fluid step has read self.smax (stream order), the fused scatter may now overwrite it
-        B.grid_scatter_speed(self.patches, self.shape, self.par, grid=self.grid, out=self.smax, exact=self.exact)
-        self._smax_fresh = True
-        self.nstep += 1
+        self._fill_tiles(need_speed=True)
+        self._timed(kernel_events, lambda: B.fluid_step_cfl(self.tiles, self.cfl, self.dh, self.smax, self.par,
+                                                            min_speed=self.smax_inflow, cons_out=self.patches,
+                                                            stats=self.stats, exact=self.exact))
+        self._done()
+
+    def signal_speed(self):
+        """S_max of the current state (Eq. 26-27, bounded below by the inflow state's) on the host."""
+        if self.dt_speed == "light":
+            return 1.0
+        B.max_signal_speed(self.grid.view(5, -1), self.par, out=self.smax, exact=self.exact)
+        return max(float(self.smax.cpu()), self.smax_inflow)
 
     def run(self, nsteps=None, t_end=None):
         n = 0

@@ -207,3 +207,37 @@ def test_device_side_time_step_equals_host_side(ref):
     assert torch.equal(a.grid, b.grid)
     assert float(a.smax.cpu()) == float(b.smax.cpu())
     assert a.last_stats().as_dict() == b.last_stats().as_dict()
+
+
+@pytest.mark.parametrize("ghost", [2, 3])
+def test_patch_gather_speed_equals_scatter_then_gather(ref, ghost):
+    """srhd_patch_gather_speed: ghost-zone fill straight from the patch layout (+ S_max) must equal
+    srhd_grid_scatter -> srhd_grid_gather (+ srhd_max_signal_speed) bit for bit, for every boundary type."""
+    rng = np.random.default_rng(ghost)
+    shape = (32, 16, 48)
+    prim = np.empty((5,) + shape)
+    prim[0] = 10.0 ** rng.uniform(-1, 1, shape)
+    prim[1:4] = rng.standard_normal((3,) + shape)
+    prim[4] = prim[0] * 10.0 ** rng.uniform(-3, 1, shape)
+    grid = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    npg = 6
+    # grid -> patch layout (the inverse of the oracle's scatter)
+    patches = np.empty((npg, 8, 5, 8, 8, 8))
+    for pg in range(npg):
+        gx, gy, gz = pg % 3, (pg // 3) % 1, pg // 3
+        blk = grid[:, gz * 16:gz * 16 + 16, gy * 16:gy * 16 + 16, gx * 16:gx * 16 + 16]
+        patches[pg] = blk.reshape(5, 2, 8, 2, 8, 2, 8).transpose(1, 3, 5, 0, 2, 4, 6).reshape(8, 5, 8, 8, 8)
+    assert np.array_equal(ref.grid_scatter(patches, shape), grid)
+    mask = (rng.random((16, 48)) < 0.2).astype(np.uint8)
+    vals = ref.prim2cons(np.array([[1e-2], [0.0], [0.0], [5.0], [1e-1]]))[:, 0]
+    recon = "plm" if ghost == 2 else "ppm"
+    for bc in (["periodic"] * 6, ["outflow"] * 6, ["outflow", "periodic", "periodic", "outflow", "outflow", "outflow"]):
+        for inflow in (None, (mask, vals)):
+            want = ref.grid_gather(grid, ghost, bc, inflow)
+            for exact in (True, False):
+                par = B.params(recon, "hllc", exact=exact)
+                di = None if inflow is None else (dev(mask), vals)
+                tiles, smax = B.patch_gather_speed(dev(patches), shape, par, bc, di, exact=exact)
+                assert np.array_equal(tiles.cpu().numpy(), want)
+                sep = B.max_signal_speed(dev(grid).reshape(5, -1).contiguous(), par, exact=exact)
+                assert float(smax.cpu()) == float(sep.cpu())
