@@ -189,7 +189,7 @@ def aggregate_value(ncell_per_rank, steps, ms_local, world, device):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE fluid_step_kernel launch, from the ncu --set full
 # capture named beside each entry (profiles/); None until a capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"blast256": 2.40e9}   # profiles/r1h_fluid_step_ppm_hllc.md (dram read + write of one launch)
+NCU_TRAFFIC_BYTES = {"blast256": 2.40e9}   # profiles/r1i_fluid_step_ppm_hllc.md (dram read + write of one launch)
 
 
 def run_conv(args):
@@ -285,7 +285,7 @@ def run_conv(args):
 # Warp-instruction counts of ONE fluid_step_kernel launch from the ncu capture named beside them
 # (smsp__inst_executed.sum and its fp64 part): feed the issue-cycle accounting of DESIGN.md section 6
 # (an fp64 warp instruction holds a sub-partition's issue port for 2 cycles, any other for 1).
-NCU_WARP_INST = {"blast256": {"fp64": 0.690e9, "other": 1.197e9, "source": "profiles/r1h_fluid_step_ppm_hllc.md"}}
+NCU_WARP_INST = {"blast256": {"fp64": 0.687e9, "other": 1.190e9, "source": "profiles/r1i_fluid_step_ppm_hllc.md"}}
 
 
 def run_ours(args):
