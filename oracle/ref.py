@@ -141,6 +141,14 @@ def phys_flux(d, W, U):
     return F
 
 
+def wave_speeds(d, W):
+    """(lambda_-, lambda_+) of one primitive state along direction d (reading S6)."""
+    W = _f64(W)
+    out = np.empty(2)
+    lib().srhd_ref_wave_speeds(C.c_int(d), _p(W), _p(out))
+    return out[0], out[1]
+
+
 def riemann_flux(riemann, d, WL, UL, WR, UR):
     WL, UL, WR, UR = map(_f64, (WL, UL, WR, UR))
     s = {"hlle": 0, "hllc": 1}[riemann] if isinstance(riemann, str) else int(riemann)

@@ -466,6 +466,15 @@ void srhd_ref_recon_1d(int recon, const double* a, double beta, double beta0, do
   recon_1d(recon, a, beta, beta0, *am, *ap);
 }
 void srhd_ref_phys_flux(int dir, const double* W, const double* U, double* F) { phys_flux(dir, W, U, F); }
+// test hook: the acoustic wave speeds of one state along dir (reading S6); out = {lambda_minus, lambda_plus}
+void srhd_ref_wave_speeds(int dir, const double* W, double* out) {
+  double U[5];
+  prim2cons(W, U);
+  Side s;
+  side_setup(dir, W, U, s);
+  out[0] = s.lam_m;
+  out[1] = s.lam_p;
+}
 void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL, const double* WR,
                            const double* UR, double* F) {
   riemann_flux(riemann, dir, WL, UL, WR, UR, F);

@@ -14,6 +14,11 @@ from mpmath import mp, mpf, sqrt
 mp.dps = 40
 
 
+def _mp(w):
+    """fp64 inputs enter exactly; values that are already 40-digit numbers stay as they are."""
+    return w if isinstance(w, mpf) else mpf(float(w))
+
+
 def h_of_T(T):
     T = mpf(T)
     return mpf(5) / 2 * T + sqrt(mpf(9) / 4 * T * T + 1)
@@ -26,7 +31,7 @@ def cs2_of_T(T):
 
 
 def prim2cons(W):
-    rho, ux, uy, uz, p = [mpf(float(w)) for w in W]
+    rho, ux, uy, uz, p = [_mp(w) for w in W]
     T = p / rho
     h = h_of_T(T)
     g = sqrt(1 + ux * ux + uy * uy + uz * uz)
@@ -37,7 +42,7 @@ def prim2cons(W):
 
 def phys_flux(d, W):
     """Eq. 4a, 4b, and the reduced-energy flux in its DEFINING form (M_n - D v_n), line 81."""
-    rho, ux, uy, uz, p = [mpf(float(w)) for w in W]
+    rho, ux, uy, uz, p = [_mp(w) for w in W]
     U = prim2cons(W)
     g = sqrt(1 + ux * ux + uy * uy + uz * uz)
     v = [ux, uy, uz][d] / g
@@ -58,7 +63,7 @@ def f_eq15(ht, musq):
 
 def lambda_pm_3vel(W, d):
     """Textbook acoustic eigenvalues in 3-velocity form (Mignone & Bodo 2005 Eq. 23 form)."""
-    rho, ux, uy, uz, p = [mpf(float(w)) for w in W]
+    rho, ux, uy, uz, p = [_mp(w) for w in W]
     g = sqrt(1 + ux * ux + uy * uy + uz * uz)
     v = [ux / g, uy / g, uz / g]
     v2 = sum(x * x for x in v)
@@ -66,3 +71,166 @@ def lambda_pm_3vel(W, d):
     vn = v[d]
     disc = sqrt(cs2 * (1 - v2) * (1 - v2 * cs2 - vn * vn * (1 - cs2)))
     return (vn * (1 - cs2) - disc) / (1 - v2 * cs2), (vn * (1 - cs2) + disc) / (1 - v2 * cs2)
+
+
+# ---------------------------------------------------------------------------------------------
+# Riemann solvers written out from their plain definitions (Mignone & Bodo 2005/2006 as the paper
+# adapts them: TM sound speed, E = Etilde + D) in 40-digit arithmetic, with the
+# TEXTBOOK 3-velocity eigenvalues above.  Plain subtractions everywhere: at 40 digits they are exact
+# for our purposes, which is what makes these a pin for any fp64 evaluation order.
+def _rot(d):
+    return [0, 1 + d, 1 + (d + 1) % 3, 1 + (d + 2) % 3, 4]
+
+
+def _side(W, d):
+    rho, ux, uy, uz, p = [_mp(w) for w in W]
+    U = prim2cons(W)
+    F = phys_flux(d, W)
+    g = sqrt(1 + ux * ux + uy * uy + uz * uz)
+    lm, lp = lambda_pm_3vel(W, d)
+    return dict(U=U, F=F, p=p, vn=[ux, uy, uz][d] / g, lm=lm, lp=lp)
+
+
+def hll_speeds(WL, WR, d):
+    L, R = _side(WL, d), _side(WR, d)
+    return min(L["lm"], R["lm"]), max(L["lp"], R["lp"])
+
+
+def hlle_flux(WL, WR, d):
+    """F = (S_R F_L - S_L F_R + S_L S_R (U_R - U_L)) / (S_R - S_L), upwinded outside [S_L, S_R]."""
+    L, R = _side(WL, d), _side(WR, d)
+    SL, SR = min(L["lm"], R["lm"]), max(L["lp"], R["lp"])
+    if SL >= 0:
+        return L["F"]
+    if SR <= 0:
+        return R["F"]
+    return [(SR * L["F"][c] - SL * R["F"][c] + SL * SR * (R["U"][c] - L["U"][c])) / (SR - SL) for c in range(5)]
+
+
+def hllc_flux(WL, WR, d):
+    """HLLC with the contact speed from the HLL averages of (D, M_n, E = Etilde + D) and the star state
+    of the side the contact leaves behind (reading S7), all in plain 40-digit arithmetic on the TOTAL
+    energy E (the textbook form); the reduced-energy flux is F_E - F_D at the end."""
+    L, R = _side(WL, d), _side(WR, d)
+    SL, SR = min(L["lm"], R["lm"]), max(L["lp"], R["lp"])
+    if SL >= 0:
+        return L["F"]
+    if SR <= 0:
+        return R["F"]
+    n = 1 + d
+    # total energy and its flux: E = Etilde + D, F_E = F_Etilde + F_D = M_n
+    EL, ER = L["U"][4] + L["U"][0], R["U"][4] + R["U"][0]
+    FEL, FER = L["U"][n], R["U"][n]
+
+    def hll(uL, uR, fL, fR):
+        return (SR * uR - SL * uL + fL - fR) / (SR - SL), (SR * fL - SL * fR + SL * SR * (uR - uL)) / (SR - SL)
+
+    Eh, FEh = hll(EL, ER, FEL, FER)
+    mh, Fmh = hll(L["U"][n], R["U"][n], L["F"][n], R["F"][n])
+    a, b, c = FEh, -(Eh + Fmh), mh
+    lam = (-b - sqrt(b * b - 4 * a * c)) / (2 * a) if a != 0 else -c / b     # the root in (-1, 1)
+    ps = Fmh - lam * FEh
+    K, S, EK = (L, SL, EL) if lam >= 0 else (R, SR, ER)
+    A, den = S - K["vn"], S - lam
+    Us = [K["U"][c_] * A / den for c_ in range(5)]
+    Us[n] = (K["U"][n] * A + ps - K["p"]) / den
+    Es = (EK * A + ps * lam - K["p"] * K["vn"]) / den
+    Us[4] = Es - Us[0]                                                       # Etilde* = E* - D*
+    return [K["F"][c_] + S * (Us[c_] - K["U"][c_]) for c_ in range(5)]
+
+
+# ---------------------------------------------------------------------------------------------
+# cons -> prim from the DEFINITIONS (Eq. 5a-5c, 8, 10): find h with D h gamma - p = Etilde + D where
+# gamma^2 = 1 + |M|^2/(D h)^2, rho = D/gamma, p = rho T(h), T(h) = (5h - sqrt(9h^2+16))/8 (Eq. 10
+# solved for T; the subtraction is harmless at 40 digits).  No Eq. 15/16, no App. A guess.
+def T_of_h(h):
+    return (5 * h - sqrt(9 * h * h + 16)) / 8
+
+
+def cons2prim(U):
+    from mpmath import findroot
+    D, mx, my, mz, Et = [_mp(u) for u in U]
+    m2 = mx * mx + my * my + mz * mz
+
+    def resid(h):
+        g = sqrt(1 + m2 / (D * h) ** 2)
+        return D * h * g - (D / g) * T_of_h(h) - (Et + D)
+
+    hi = 2 + 2 * (Et + D) / D
+    h = findroot(resid, (mpf(1), hi), solver="anderson", tol=mpf(10) ** -70, maxsteps=200)
+    g = sqrt(1 + m2 / (D * h) ** 2)
+    rho = D / g
+    return [rho, mx / (D * h), my / (D * h), mz / (D * h), rho * T_of_h(h)]
+
+
+def limited_slope(sL, sR, beta):
+    """reading S3: van Leer harmonic mean capped by the generalised minmod."""
+    if sL * sR <= 0:
+        return mpf(0)
+    mag = min(2 * abs(sL * sR) / abs(sL + sR), mpf(beta) * min(abs(sL), abs(sR)))
+    return mag if sL > 0 else -mag
+
+
+def plm_edges(am1, a0, ap1, beta):
+    d = limited_slope(a0 - am1, ap1 - a0, beta)
+    return a0 - d / 2, a0 + d / 2
+
+
+def step_cells(cons, cells, dt, dh, riemann="hllc", beta=1.5):
+    """One PLM + MUSCL-Hancock + HLLE/HLLC update (readings S3, S5, S12) of the
+    listed cells (i, j, k) of a conserved box cons[5][nz][ny][nx] (numpy float64; every cell within two
+    of a listed cell must be inside the box), in 40-digit arithmetic from the definitions above.
+    Returns {cell: [5 mpf]}.  Python loops with memoisation: a handful of cells only."""
+    dt, dh = mpf(dt), mpf(dh)
+    flux_fn = hllc_flux if riemann == "hllc" else hlle_flux
+    Wc, edges, fluxes = {}, {}, {}
+
+    def prim(c):
+        if c not in Wc:
+            i, j, k = c
+            Wc[c] = cons2prim([float(cons[q, k, j, i]) for q in range(5)])
+        return Wc[c]
+
+    def shift(c, d, s):
+        c = list(c)
+        c[d] += s
+        return tuple(c)
+
+    def half_step(c):
+        """Evolved PRIMITIVE edge states of cell c: {(d, side): W}, side 0 = minus edge, 1 = plus edge."""
+        if c in edges:
+            return edges[c]
+        W0 = prim(c)
+        Wm, Wp = {}, {}
+        for d in range(3):
+            a, b = prim(shift(c, d, -1)), prim(shift(c, d, +1))
+            em, ep = zip(*[plm_edges(a[q], W0[q], b[q], beta) for q in range(5)])
+            Wm[d], Wp[d] = list(em), list(ep)
+        # one COMMON increment from all three directions (unsplit, reading S5)
+        dU = [mpf(0)] * 5
+        for d in range(3):
+            Fm, Fp = phys_flux(d, Wm[d]), phys_flux(d, Wp[d])
+            dU = [dU[q] - dt / (2 * dh) * (Fp[q] - Fm[q]) for q in range(5)]
+        out = {}
+        for d in range(3):
+            for side, W in ((0, Wm[d]), (1, Wp[d])):
+                U = prim2cons(W)
+                out[(d, side)] = cons2prim([U[q] + dU[q] for q in range(5)])
+        edges[c] = out
+        return out
+
+    def face_flux(c, d):
+        """Flux through the face between c and c + e_d."""
+        if (c, d) not in fluxes:
+            fluxes[(c, d)] = flux_fn(half_step(c)[(d, 1)], half_step(shift(c, d, +1))[(d, 0)], d)
+        return fluxes[(c, d)]
+
+    res = {}
+    for c in cells:
+        i, j, k = c
+        tot = [mpf(0)] * 5
+        for d in range(3):
+            Fp, Fm = face_flux(c, d), face_flux(shift(c, d, -1), d)
+            tot = [tot[q] + (Fp[q] - Fm[q]) for q in range(5)]
+        res[c] = [mpf(float(cons[q, k, j, i])) - dt / dh * tot[q] for q in range(5)]
+    return res

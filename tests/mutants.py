@@ -1,0 +1,92 @@
+"""Mutation check of the oracle's pins ("Next round" #1).
+
+Each entry makes ONE plausible one-line mistake in a scratch copy of oracle/srhd_ref.cpp, rebuilds the
+oracle there and runs the pin tests named beside it against the mutant: at least one must FAIL.  A pin
+that still passes means that part of the oracle is unpinned.  Nothing here touches the real oracle/.
+
+    python tests/mutants.py            # run all, print a table, exit 1 if any mutant survives
+(tests/test_oracle_mutants.py runs the same from pytest.)
+"""
+import os
+import shutil
+import subprocess
+import sys
+import tempfile
+from concurrent.futures import ThreadPoolExecutor
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+PINS = "tests/test_oracle_pins_r2.py"
+
+# (name, cited passage, old text, new text, pytest node ids / -k expression that must fail)
+MUTANTS = [
+    ("umax: gamma_s dropped", "P:241 Eq. 26",
+     "return gs * (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + 3.0 * gamma * Us;",
+     "return (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + 3.0 * gamma * Us;",
+     "test_umax"),
+    ("umax: gamma dropped from 3 gamma U_s", "P:241 Eq. 26",
+     "+ 3.0 * gamma * Us;", "+ 3.0 * Us;", "test_umax"),
+    ("wave speeds: U_s^2 dropped from the denominator", "reading S6",
+     "s.lam_p = (gamma * Un + Us * Q) / (g2 + Us2);\n  s.lam_m = (gamma * Un - Us * Q) / (g2 + Us2);",
+     "s.lam_p = (gamma * Un + Us * Q) / (g2);\n  s.lam_m = (gamma * Un - Us * Q) / (g2);",
+     "test_wave_speed_values or test_riemann_flux_values or test_hlle_satisfies"),
+    ("HLLE: dissipative term halved", "P:225 (Mignone & Bodo 2005)",
+     "    F[c] = (SR * L.F[c] - SL * R.F[c] + SL * SR * (R.U[c] - L.U[c])) / (SR - SL);",
+     "    F[c] = (SR * L.F[c] - SL * R.F[c] + 0.5 * SL * SR * (R.U[c] - L.U[c])) / (SR - SL);",
+     "test_hlle_satisfies or test_riemann_flux_values"),
+    ("HLLC: p* term dropped from Etilde*", "reading S7",
+     "Us[4] = (K.U[4] * A + ps * lam - K.p * K.vn) / den;", "Us[4] = (K.U[4] * A - K.p * K.vn) / den;",
+     "test_riemann_flux_values"),
+    ("Hancock predictor: per-direction (split) increment", "P:225, reading S5",
+     "Um[(d * 5 + q) * np + c] = Ucm[d][q] + dU[q];\n              Up[(d * 5 + q) * np + c] = Ucp[d][q] + dU[q];",
+     "Um[(d * 5 + q) * np + c] = Ucm[d][q] - hdt * dF[d][q];\n              Up[(d * 5 + q) * np + c] = Ucp[d][q] - hdt * dF[d][q];",
+     "test_second_order_convergence_on_the_3d_diagonal_wave"),
+    ("Hancock predictor: split increment (bitwise / 40-digit pins)", "P:225, reading S5",
+     "Um[(d * 5 + q) * np + c] = Ucm[d][q] + dU[q];\n              Up[(d * 5 + q) * np + c] = Ucp[d][q] + dU[q];",
+     "Um[(d * 5 + q) * np + c] = Ucm[d][q] - hdt * dF[d][q];\n              Up[(d * 5 + q) * np + c] = Ucp[d][q] - hdt * dF[d][q];",
+     "test_one_step_matches_40_digit or test_retry_ladder_equals"),
+    ("retry ladder: factor 0.75 -> 0.5", "P:273",
+     "beta = (pass <= K) ? beta * 0.75 : 0.0;", "beta = (pass <= K) ? beta * 0.5 : 0.0;",
+     "test_retry_ladder_equals"),
+    ("retry ladder: failing face states ignored", "reading S15",
+     "if ((face_fail == 0 && cell_fail == 0) || beta == 0.0) break;",
+     "if ((cell_fail == 0) || beta == 0.0) break;",
+     "test_retry_ladder_equals"),
+    ("update: flux difference with the wrong sign in z", "Eq. 4a, reading S12",
+     "Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);",
+     "Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) - dfz);",
+     "test_one_step_matches_40_digit"),
+]
+
+
+def run_mutant(m):
+    name, cite, old, new, kexpr = m
+    src = open(os.path.join(ROOT, "oracle", "srhd_ref.cpp")).read()
+    if src.count(old) < 1:
+        return name, cite, "STALE", f"pattern not found in oracle/srhd_ref.cpp: {old[:60]!r}"
+    tmp = tempfile.mkdtemp(prefix="srhd_mutant_")
+    try:
+        shutil.copytree(os.path.join(ROOT, "oracle"), os.path.join(tmp, "oracle"),
+                        ignore=shutil.ignore_patterns("*.so", "__pycache__"))
+        with open(os.path.join(tmp, "oracle", "srhd_ref.cpp"), "w") as f:
+            f.write(src.replace(old, new))
+        env = dict(os.environ, SRHD_TEST_ORACLE_ROOT=tmp, SRHD_TEST_SKIP_CUDA_BUILD="1", OMP_NUM_THREADS="2")
+        r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider", PINS, "-k", kexpr],
+                           cwd=ROOT, env=env, capture_output=True, text=True, timeout=600)
+        tail = (r.stdout.strip().splitlines() or [""])[-1]
+        if r.returncode == 1:
+            return name, cite, "KILLED", tail
+        return name, cite, "SURVIVED" if r.returncode == 0 else "ERROR", tail + r.stderr[-300:]
+    finally:
+        shutil.rmtree(tmp, ignore_errors=True)
+
+
+def run_all(workers=4):
+    with ThreadPoolExecutor(workers) as ex:
+        return list(ex.map(run_mutant, MUTANTS))
+
+
+if __name__ == "__main__":
+    res = run_all()
+    for name, cite, verdict, tail in res:
+        print(f"{verdict:9s} {name}  [{cite}]  -- {tail}")
+    sys.exit(0 if all(v == "KILLED" for _, _, v, _ in res) else 1)
