@@ -143,10 +143,15 @@ def phys_flux(d, W, U):
 
 def wave_speeds(d, W):
     """(lambda_-, lambda_+) of one primitive state along direction d (reading S6)."""
+    return tuple(wave_speed_differences(d, W)[:2])
+
+
+def wave_speed_differences(d, W):
+    """[lambda_-, lambda_+, lambda_+ - v_n, v_n - lambda_-, 1 - lambda_+, 1 + lambda_-] (reading S6)."""
     W = _f64(W)
-    out = np.empty(2)
+    out = np.empty(6)
     lib().srhd_ref_wave_speeds(C.c_int(d), _p(W), _p(out))
-    return out[0], out[1]
+    return out
 
 
 def riemann_flux(riemann, d, WL, UL, WR, UR):

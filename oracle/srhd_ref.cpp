@@ -175,11 +175,22 @@ void phys_flux(int d, const double W[5], const double U[5], double F[5]) {
 // One side of a Riemann problem in the rotated frame (n = normal, t1, t2 = tangential).
 struct Side {
   double U[5];   // D, M_n, M_t1, M_t2, Etilde
-  double F[5];   // physical flux along n
+  double F[5];   // physical flux along n = U v_n + pt
+  double pt[5];  // its pressure terms (0, p, 0, 0, p v_n)
   double p, vn, lam_m, lam_p;
+  double dp, dm; // lam_p - v_n and v_n - lam_m (both >= 0), formed without cancellation (reading S6)
+  double cp, cm; // 1 - lam_p and 1 + lam_m, formed without cancellation (reading S6)
 };
 // Acoustic eigenvalues in 4-velocity form (reading S6):
 //   lambda_pm = (gamma U_n +- U_s Q) / (gamma^2 + U_s^2),  Q = sqrt(1 + U_t^2 + U_s^2)
+// and, for Lorentz factors where lambda, v_n and 1 agree to many digits, their DIFFERENCES as products
+// and sums of positive numbers (SURVEY.md 8c S6, section 7 "S - v, 1 - S ... without subtracting
+// near-equal numbers"; with a = 1 + U_t^2, u = |U_n| and (gamma Q - u U_s)(gamma Q + u U_s) =
+// a (gamma^2 + U_s^2)):
+//   wave running WITH the flow:    |lambda - v_n| = U_s a / (gamma (gamma Q + u U_s)),
+//                                  1 - |lambda|   = a^2 / ((gamma + u)(Q + U_s)(gamma Q + u U_s));
+//   wave running AGAINST the flow: |lambda - v_n| = U_s (gamma Q + u U_s) / (gamma (gamma^2 + U_s^2)),
+//                                  1 - |lambda| needs no care there (|lambda| stays well below 1).
 void side_setup(int d, const double W[5], const double U[5], Side& s) {
   const int n = 1 + d, t1 = 1 + (d + 1) % 3, t2 = 1 + (d + 2) % 3;
   const double rho = W[0], Un = W[n], Ut1 = W[t1], Ut2 = W[t2], p = W[4];
@@ -194,12 +205,33 @@ void side_setup(int d, const double W[5], const double U[5], Side& s) {
   s.lam_p = (gamma * Un + Us * Q) / (g2 + Us2);
   s.lam_m = (gamma * Un - Us * Q) / (g2 + Us2);
   s.vn = Un / gamma;
+  const double a = 1.0 + Utsq, u = std::fabs(Un);
+  const double w = gamma * Q + u * Us;
+  const double d_with = Us * a / (gamma * w);
+  const double d_against = Us * w / (gamma * (g2 + Us2));
+  const double c_with = a * a / ((gamma + u) * (Q + Us) * w);
+  if (Un >= 0.0) {
+    s.dp = d_with;
+    s.dm = d_against;
+    s.cp = c_with;
+    s.cm = 1.0 + s.lam_m;
+  } else {
+    s.dp = d_against;
+    s.dm = d_with;
+    s.cp = 1.0 - s.lam_p;
+    s.cm = c_with;
+  }
   s.p = p;
   s.U[0] = U[0];
   s.U[1] = U[n];
   s.U[2] = U[t1];
   s.U[3] = U[t2];
   s.U[4] = U[4];
+  s.pt[0] = 0.0;
+  s.pt[1] = p;
+  s.pt[2] = 0.0;
+  s.pt[3] = 0.0;
+  s.pt[4] = p * s.vn;
   s.F[0] = s.U[0] * s.vn;
   s.F[1] = s.U[1] * s.vn + p;
   s.F[2] = s.U[2] * s.vn;
@@ -207,23 +239,49 @@ void side_setup(int d, const double W[5], const double U[5], Side& s) {
   s.F[4] = (s.U[4] + p) * s.vn;
 }
 
+// The two-wave (HLL) averages of Mignone & Bodo 2005 with the S6 speeds,
+//   U^hll = (S_R U_R - S_L U_L + F_L - F_R)/(S_R - S_L),  F^hll = (S_R F_L - S_L F_R + S_L S_R (U_R - U_L))/(S_R - S_L),
+// written with F = U v_n + pt through A_R = S_R - v_R > 0 and B_L = v_L - S_L > 0 (S6: differences of wave
+// and flow speeds are never formed by subtracting the speeds themselves):
+//   U^hll = (A_R U_R + B_L U_L + pt_L - pt_R)/(S_R - S_L)
+//   F^hll = (S_R B_L U_L + S_L A_R U_R + S_R pt_L - S_L pt_R)/(S_R - S_L)
+// S_R may belong to either side, v_R to the right one: A_R = (lam_p - v_n)_R + (S_R - (lam_p)_R).
+struct Hll {
+  double SL, SR, AR, BL;
+};
+Hll hll_speeds(const Side& L, const Side& R) {
+  Hll h;
+  h.SL = std::min(L.lam_m, R.lam_m);
+  h.SR = std::max(L.lam_p, R.lam_p);
+  // S_R - lam_p of the RIGHT state (zero unless the left state sets S_R): near the light cone as a
+  // difference of the complements 1 - lambda (tiny numbers known to full relative accuracy), elsewhere of
+  // the speeds themselves -- whichever pair of operands is the smaller one
+  const double cpS = std::min(L.cp, R.cp), cmS = std::min(L.cm, R.cm);   // 1 - S_R, 1 + S_L
+  h.AR = R.dp + ((h.SR > 0.5) ? (R.cp - cpS) : (h.SR - R.lam_p));
+  h.BL = L.dm + ((h.SL < -0.5) ? (L.cm - cmS) : (L.lam_m - h.SL));
+  return h;
+}
 // HLLE (Mignone & Bodo 2005 form with the S6 speeds); rotated frame
 void hlle_rot(const Side& L, const Side& R, double F[5]) {
-  const double SL = std::min(L.lam_m, R.lam_m), SR = std::max(L.lam_p, R.lam_p);
+  const Hll h = hll_speeds(L, R);
+  const double SL = h.SL, SR = h.SR, AR = h.AR, BL = h.BL;
   if (SL >= 0.0) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
   if (SR <= 0.0) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
+  const double den = SR - SL;
   for (int c = 0; c < 5; ++c)
-    F[c] = (SR * L.F[c] - SL * R.F[c] + SL * SR * (R.U[c] - L.U[c])) / (SR - SL);
+    F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;
 }
 // HLLC adapted to Etilde ("replacing E with Etilde + D c^2"; reading S7); rotated frame
 void hllc_rot(const Side& L, const Side& R, double F[5]) {
-  const double SL = std::min(L.lam_m, R.lam_m), SR = std::max(L.lam_p, R.lam_p);
+  const Hll h = hll_speeds(L, R);
+  const double SL = h.SL, SR = h.SR, AR = h.AR, BL = h.BL;
   if (SL >= 0.0) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
   if (SR <= 0.0) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
+  const double den = SR - SL;
   double Uh[5], Fh[5];                                        // HLL state and flux
   for (int c = 0; c < 5; ++c) {
-    Uh[c] = (SR * R.U[c] - SL * L.U[c] + L.F[c] - R.F[c]) / (SR - SL);
-    Fh[c] = (SR * L.F[c] - SL * R.F[c] + SL * SR * (R.U[c] - L.U[c])) / (SR - SL);
+    Uh[c] = (AR * R.U[c] + BL * L.U[c] + (L.pt[c] - R.pt[c])) / den;
+    Fh[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;
   }
   const double Eh = Uh[4] + Uh[0];                            // E = Etilde + D   (sums only)
   const double FEh = Fh[4] + Fh[0];
@@ -231,17 +289,24 @@ void hllc_rot(const Side& L, const Side& R, double F[5]) {
   // contact speed: root of a lam^2 - b lam + m = 0 in (-1,1), rationalised (safe for a -> 0)
   const double lam = 2.0 * m / (b + std::sqrt(b * b - 4.0 * a * m));
   const double ps = Fh[1] - lam * FEh;                        // p*
-  const Side& K = (lam >= 0.0) ? L : R;
-  const double S = (lam >= 0.0) ? SL : SR;
-  const double A = S - K.vn;
-  const double den = S - lam;
+  const bool left = lam >= 0.0;
+  const Side& K = left ? L : R;
+  const double S = left ? SL : SR;
+  const double A = left ? -BL : AR;                           // S - v_n of side K
+  const double dK = S - lam;                                  // S and lam have opposite signs: a sum
   double Us[5];
-  Us[0] = K.U[0] * A / den;
-  Us[1] = (K.U[1] * A + ps - K.p) / den;
-  Us[2] = K.U[2] * A / den;
-  Us[3] = K.U[3] * A / den;
-  Us[4] = (K.U[4] * A + ps * lam - K.p * K.vn) / den;         // linear in E: no D is subtracted
-  for (int c = 0; c < 5; ++c) F[c] = K.F[c] + S * (Us[c] - K.U[c]);
+  Us[0] = K.U[0] * A / dK;
+  Us[1] = (K.U[1] * A + ps - K.p) / dK;
+  Us[2] = K.U[2] * A / dK;
+  Us[3] = K.U[3] * A / dK;
+  Us[4] = (K.U[4] * A + ps * lam - K.p * K.vn) / dK;          // linear in E: no D is subtracted
+  // F* = F_K + S (U* - U_K) across the wave S; with the star state above this is identically the flux
+  // of a state moving with the contact, (D* lam, M* lam + p* e_n, (Etilde* + p*) lam): products only
+  F[0] = Us[0] * lam;
+  F[1] = Us[1] * lam + ps;
+  F[2] = Us[2] * lam;
+  F[3] = Us[3] * lam;
+  F[4] = (Us[4] + ps) * lam;
 }
 void riemann_flux(int riemann, int d, const double WL[5], const double UL[5], const double WR[5],
                   const double UR[5], double F[5]) {
@@ -466,7 +531,8 @@ void srhd_ref_recon_1d(int recon, const double* a, double beta, double beta0, do
   recon_1d(recon, a, beta, beta0, *am, *ap);
 }
 void srhd_ref_phys_flux(int dir, const double* W, const double* U, double* F) { phys_flux(dir, W, U, F); }
-// test hook: the acoustic wave speeds of one state along dir (reading S6); out = {lambda_minus, lambda_plus}
+// test hook: the acoustic wave speeds of one state along dir (reading S6);
+// out = {lambda_-, lambda_+, lambda_+ - v_n, v_n - lambda_-, 1 - lambda_+, 1 + lambda_-}
 void srhd_ref_wave_speeds(int dir, const double* W, double* out) {
   double U[5];
   prim2cons(W, U);
@@ -474,6 +540,10 @@ void srhd_ref_wave_speeds(int dir, const double* W, double* out) {
   side_setup(dir, W, U, s);
   out[0] = s.lam_m;
   out[1] = s.lam_p;
+  out[2] = s.dp;
+  out[3] = s.dm;
+  out[4] = s.cp;
+  out[5] = s.cm;
 }
 void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL, const double* WR,
                            const double* UR, double* F) {

@@ -87,7 +87,8 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
 // single Riemann flux along direction dir (0,1,2), for tests: WL/UL/WR/UR are 5-vectors
 void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL,
                            const double* WR, const double* UR, double* F);
-// acoustic wave speeds (reading S6) of one primitive state along dir, for tests: out = {lambda_-, lambda_+}
+// acoustic wave speeds (reading S6) of one primitive state along dir, for tests:
+// out[6] = {lambda_-, lambda_+, lambda_+ - v_n, v_n - lambda_-, 1 - lambda_+, 1 + lambda_-}
 void srhd_ref_wave_speeds(int dir, const double* W, double* out);
 // physical flux along dir (Eq. 4a, 4b; Eq. 7)
 void srhd_ref_phys_flux(int dir, const double* W, const double* U, double* F);

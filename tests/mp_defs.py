@@ -96,27 +96,47 @@ def hll_speeds(WL, WR, d):
     return min(L["lm"], R["lm"]), max(L["lp"], R["lp"])
 
 
-def hlle_flux(WL, WR, d):
-    """F = (S_R F_L - S_L F_R + S_L S_R (U_R - U_L)) / (S_R - S_L), upwinded outside [S_L, S_R]."""
+def _pt(K, d):
+    """pressure terms of the physical flux: F = U v_n + pt."""
+    out = [mpf(0)] * 5
+    out[1 + d] = K["p"]
+    out[4] = K["p"] * K["vn"]
+    return out
+
+
+def _upwind_pieces(K, d):
+    return [abs(K["U"][c] * K["vn"]) + abs(_pt(K, d)[c]) for c in range(5)]
+
+
+def hlle_flux(WL, WR, d, pieces=False):
+    """F = (S_R F_L - S_L F_R + S_L S_R (U_R - U_L)) / (S_R - S_L), upwinded outside [S_L, S_R].
+    pieces=True also returns, per component, the summed magnitude of the terms that do not cancel by
+    arithmetic alone: S_R (v_L - S_L) U_L, S_L (S_R - v_R) U_R and the two pressure terms (a tolerance scale)."""
     L, R = _side(WL, d), _side(WR, d)
     SL, SR = min(L["lm"], R["lm"]), max(L["lp"], R["lp"])
     if SL >= 0:
-        return L["F"]
+        return (L["F"], _upwind_pieces(L, d)) if pieces else L["F"]
     if SR <= 0:
-        return R["F"]
-    return [(SR * L["F"][c] - SL * R["F"][c] + SL * SR * (R["U"][c] - L["U"][c])) / (SR - SL) for c in range(5)]
+        return (R["F"], _upwind_pieces(R, d)) if pieces else R["F"]
+    F = [(SR * L["F"][c] - SL * R["F"][c] + SL * SR * (R["U"][c] - L["U"][c])) / (SR - SL) for c in range(5)]
+    if not pieces:
+        return F
+    ptL, ptR = _pt(L, d), _pt(R, d)
+    pc = [(abs(SR * (L["vn"] - SL) * L["U"][c]) + abs(SL * (SR - R["vn"]) * R["U"][c]) + abs(SR * ptL[c]) + abs(SL * ptR[c]))
+          / (SR - SL) for c in range(5)]
+    return F, pc
 
 
-def hllc_flux(WL, WR, d):
+def hllc_flux(WL, WR, d, pieces=False):
     """HLLC with the contact speed from the HLL averages of (D, M_n, E = Etilde + D) and the star state
     of the side the contact leaves behind (reading S7), all in plain 40-digit arithmetic on the TOTAL
     energy E (the textbook form); the reduced-energy flux is F_E - F_D at the end."""
     L, R = _side(WL, d), _side(WR, d)
     SL, SR = min(L["lm"], R["lm"]), max(L["lp"], R["lp"])
     if SL >= 0:
-        return L["F"]
+        return (L["F"], _upwind_pieces(L, d)) if pieces else L["F"]
     if SR <= 0:
-        return R["F"]
+        return (R["F"], _upwind_pieces(R, d)) if pieces else R["F"]
     n = 1 + d
     # total energy and its flux: E = Etilde + D, F_E = F_Etilde + F_D = M_n
     EL, ER = L["U"][4] + L["U"][0], R["U"][4] + R["U"][0]
@@ -136,7 +156,24 @@ def hllc_flux(WL, WR, d):
     Us[n] = (K["U"][n] * A + ps - K["p"]) / den
     Es = (EK * A + ps * lam - K["p"] * K["vn"]) / den
     Us[4] = Es - Us[0]                                                       # Etilde* = E* - D*
-    return [K["F"][c_] + S * (Us[c_] - K["U"][c_]) for c_ in range(5)]
+    F = [K["F"][c_] + S * (Us[c_] - K["U"][c_]) for c_ in range(5)]
+    if not pieces:
+        return F
+    ptK = _pt(K, d)
+    # the star state itself is a sum of pieces, (U_K A + pressure terms)/(S - lam): take their magnitudes
+    star = [abs(K["U"][c_] * A / den) for c_ in range(5)]
+    # (p* = F_M^hll - lam* F_E^hll is a subtraction in the DEFINITION of the solver, reading S7: its two
+    # operands count as pieces, not their difference)
+    psz = abs(Fmh) + abs(lam * FEh)
+    star[n] += (psz + abs(K["p"])) / abs(den)
+    star[4] += (psz * abs(lam) + abs(K["p"] * K["vn"])) / abs(den)
+    # conditioning of the contact speed: the two roots of a lam^2 - b lam + m = 0 approach each other (and the
+    # light cone) when an ultra-relativistic stream hits slow gas; lam* then carries sqrt(kappa) ulp
+    kappa = b * b / (b * b - 4 * a * c)
+    pc = [abs(S) * star[c_] + abs(A * K["U"][c_]) + abs(ptK[c_]) for c_ in range(5)]
+    pc[n] += psz                                       # F*_n = M_n* lam* + p*,  F*_E = (Etilde* + p*) lam*
+    pc[4] += psz * abs(lam)
+    return F, pc, kappa
 
 
 # ---------------------------------------------------------------------------------------------

@@ -29,12 +29,28 @@ MUTANTS = [
      "s.lam_p = (gamma * Un + Us * Q) / (g2 + Us2);\n  s.lam_m = (gamma * Un - Us * Q) / (g2 + Us2);",
      "s.lam_p = (gamma * Un + Us * Q) / (g2);\n  s.lam_m = (gamma * Un - Us * Q) / (g2);",
      "test_wave_speed_values or test_riemann_flux_values or test_hlle_satisfies"),
-    ("HLLE: dissipative term halved", "P:225 (Mignone & Bodo 2005)",
-     "    F[c] = (SR * L.F[c] - SL * R.F[c] + SL * SR * (R.U[c] - L.U[c])) / (SR - SL);",
-     "    F[c] = (SR * L.F[c] - SL * R.F[c] + 0.5 * SL * SR * (R.U[c] - L.U[c])) / (SR - SL);",
+    ("wave-speed differences: U_t^2 dropped from lambda - v_n", "reading S6",
+     "const double d_with = Us * a / (gamma * w);", "const double d_with = Us / (gamma * w);",
+     "test_wave_speed_differences or test_riemann_flux"),
+    ("wave-speed differences: 1 - lambda with a single factor a", "reading S6",
+     "const double c_with = a * a / ((gamma + u) * (Q + Us) * w);", "const double c_with = a / ((gamma + u) * (Q + Us) * w);",
+     "test_wave_speed_differences or test_riemann_flux_at_lorentz"),
+    ("HLL: S_R - v_R without the other side's wave", "reading S6",
+     "h.AR = R.dp + ((h.SR > 0.5) ? (R.cp - cpS) : (h.SR - R.lam_p));", "h.AR = R.dp;",
+     "test_riemann_flux_values or test_hlle_satisfies"),
+    ("HLLE: the right state's term halved", "P:225 (Mignone & Bodo 2005)",
+     "    F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
+     "    F[c] = (SR * BL * L.U[c] + 0.5 * SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
+     "test_hlle_satisfies or test_riemann_flux_values"),
+    ("HLLE: wave speeds swapped on the pressure terms", "P:225 (Mignone & Bodo 2005)",
+     "    F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
+     "    F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SL * L.pt[c] - SR * R.pt[c]) / den;",
      "test_hlle_satisfies or test_riemann_flux_values"),
     ("HLLC: p* term dropped from Etilde*", "reading S7",
-     "Us[4] = (K.U[4] * A + ps * lam - K.p * K.vn) / den;", "Us[4] = (K.U[4] * A - K.p * K.vn) / den;",
+     "Us[4] = (K.U[4] * A + ps * lam - K.p * K.vn) / dK;", "Us[4] = (K.U[4] * A - K.p * K.vn) / dK;",
+     "test_riemann_flux_values"),
+    ("HLLC: star momentum flux without p*", "reading S7",
+     "F[1] = Us[1] * lam + ps;", "F[1] = Us[1] * lam;",
      "test_riemann_flux_values"),
     ("Hancock predictor: per-direction (split) increment", "P:225, reading S5",
      "Um[(d * 5 + q) * np + c] = Ucm[d][q] + dU[q];\n              Up[(d * 5 + q) * np + c] = Ucp[d][q] + dU[q];",
