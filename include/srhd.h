@@ -74,8 +74,17 @@ typedef struct {
                                          accepted beta = 0 pass (S15)                                 */
   unsigned long long n_retry_pg;      /* patch groups that needed >= 1 retry pass         */
   unsigned long long n_unphys_final;  /* updated cells still violating Eq. 30 after beta = 0 (S10)    */
-  unsigned long long newton_iters;    /* total Newton-Raphson iterations (for the flop model)         */
+  unsigned long long newton_iters;    /* Newton-Raphson iterations of the ALGORITHM's conversions: every
+                                         tile cell once + both states of every face in the accepted pass
+                                         (for the flop model; retries that were thrown away not counted) */
   double             max_speed;       /* max S_max (Eq. 27) over the INPUT interior cells       */
+  unsigned long long n_passes;        /* passes over patch groups, retry passes included (>= npg)     */
+  /* work the kernel actually EXECUTED (srhd_fluid_step only; for the executed-flop roofline figure):
+   * retry passes are abandoned at the first plane that shows a failure, uniform regions take shortcuts */
+  unsigned long long exec_c2p;        /* conversions executed (cons2prim calls)                       */
+  unsigned long long exec_newton;     /* Newton-Raphson iterations executed                           */
+  unsigned long long exec_riemann;    /* HLLE / HLLC solves executed                                  */
+  unsigned long long exec_hancock;    /* (cell, direction) edge-state pairs reconstructed + converted */
 } srhd_stats;
 
 /* Fill *p with the defaults above for the given recon / riemann choice (host pointer). */

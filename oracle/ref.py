@@ -25,7 +25,7 @@ class Params(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_c2p_fail", C.c_ulonglong), ("n_retry_pg", C.c_ulonglong),
                 ("n_unphys_final", C.c_ulonglong), ("newton_iters", C.c_ulonglong),
-                ("max_speed", C.c_double)]
+                ("max_speed", C.c_double), ("n_passes", C.c_ulonglong)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

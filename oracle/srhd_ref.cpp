@@ -411,12 +411,13 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
   std::vector<double> Flux(3 * 5 * np);                       // [dir][comp][cell c] = F at c+1/2 n
   const int K = par.max_retry;
   double beta = par.minmod_coeff;
-  unsigned long long face_fail = 0, cell_fail = 0;
+  unsigned long long face_fail = 0, cell_fail = 0, face_iters = 0;
   int pass = 0;
   for (;; ++pass) {
     if (pass > 0) beta = (pass <= K) ? beta * 0.75 : 0.0;     // P:273, reading S9
     face_fail = 0;
     cell_fail = 0;
+    face_iters = 0;
     // O5b + O6
     for (int k = -1; k <= nz; ++k)
       for (int j = -1; j <= ny; ++j)
@@ -469,9 +470,9 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
             }
             int it = 0;
             if (!cons2prim(UL, WL, par.newton_rtol, par.newton_max_iter, &it, nullptr)) ++face_fail;  // S15
-            st.newton_iters += (unsigned long long)it;
+            face_iters += (unsigned long long)it;
             if (!cons2prim(UR, WR, par.newton_rtol, par.newton_max_iter, &it, nullptr)) ++face_fail;
-            st.newton_iters += (unsigned long long)it;
+            face_iters += (unsigned long long)it;
             riemann_flux(par.riemann, d, WL, UL, WR, UR, F);
             for (int q = 0; q < 5; ++q) Flux[(d * 5 + q) * np + c] = F[q];
           }
@@ -498,6 +499,8 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
   }
   if (flux_keep) std::copy(Flux.begin(), Flux.end(), flux_keep);
   if (pass > 0) ++st.n_retry_pg;
+  st.n_passes += (unsigned long long)(pass + 1);
+  st.newton_iters += face_iters;     // informational: every tile cell once + the face states of the ACCEPTED pass
   st.n_c2p_fail += face_fail;        // only non-zero in an accepted beta = 0 pass (S15)
   st.n_unphys_final += cell_fail;
   return pass + 1;
@@ -633,14 +636,14 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
                                 srhd_ref_stats* stats, int nthreads) {
   const int nxt = 16 + 2 * par->ghost;
   const size_t in_pg = (size_t)5 * nxt * nxt * nxt, out_pg = (size_t)8 * 5 * 512;
-  unsigned long long f1 = 0, f2 = 0, f3 = 0, f4 = 0;
+  unsigned long long f1 = 0, f2 = 0, f3 = 0, f4 = 0, f5 = 0;
   double ms = 0.0;
 #ifdef _OPENMP
   if (nthreads <= 0) nthreads = omp_get_max_threads();
 #else
   nthreads = 1;
 #endif
-#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : f1, f2, f3, f4) reduction(max : ms)
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : f1, f2, f3, f4, f5) reduction(max : ms)
   for (int pg = 0; pg < npg; ++pg) {
     srhd_ref_stats st;
     std::memset(&st, 0, sizeof(st));
@@ -681,6 +684,7 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
     f2 += st.n_retry_pg;
     f3 += st.n_unphys_final;
     f4 += st.newton_iters;
+    f5 += st.n_passes;
     ms = std::max(ms, st.max_speed);
   }
   if (stats) {
@@ -689,6 +693,7 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
     stats->n_unphys_final = f3;
     stats->newton_iters = f4;
     stats->max_speed = ms;
+    stats->n_passes = f5;
   }
 }
 

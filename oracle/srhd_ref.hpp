@@ -36,8 +36,10 @@ struct srhd_ref_stats {
   unsigned long long n_c2p_fail;      // Eq. 30 violations on input to a conversion
   unsigned long long n_retry_pg;      // patch groups that needed >= 1 retry
   unsigned long long n_unphys_final;  // output cells still violating Eq. 30 in the accepted pass
-  unsigned long long newton_iters;    // total Newton iterations (informational)
+  unsigned long long newton_iters;    // Newton iterations of the algorithm's conversions (informational): every
+                                      // tile cell once + both states of every face in the ACCEPTED pass
   double             max_speed;       // max S_max (Eq. 27) over the input interior cells
+  unsigned long long n_passes;        // passes over patch groups, retries included (>= number of groups)
 };
 
 // --- O1 EoS (Eq. 10, Eq. 22, Eq. 16, Eq. 14) --------------------------

@@ -85,8 +85,8 @@ struct Plan {
   static constexpr int oFX = oZSp + 2 * 5 * ZS;
   static constexpr int oFY = oFX + 5 * NFXY;
   static constexpr int oFZ = oFY + 5 * NFXY;          // z flux through the lower face of each column's cell
-  static constexpr int oCtl = oFZ + 5 * ZS;           // control block: 8 x 8 bytes
-  static constexpr int nDoubles = oCtl + 8;
+  static constexpr int oCtl = oFZ + 5 * ZS;           // control block (struct Ctl)
+  static constexpr int nDoubles = oCtl + 10;
   static constexpr size_t bytes = (size_t)nDoubles * sizeof(double);
 };
 
@@ -96,6 +96,9 @@ struct Ctl {                       // lives in shared memory
   unsigned long long umax_bits;
   unsigned int face_fail, cell_fail, in_fail;
   int queue;                       // next chunk of interval X
+  unsigned int abort;              // a failure was seen in this (non-final) pass: abandon it at the plane's end
+  unsigned int exec_c2p, exec_riemann, exec_hancock;
+  unsigned long long exec_newton;
 };
 
 // Hancock stage of one (cell, direction) lane: PLM/PPM edge values of the five primitives along d
@@ -191,6 +194,9 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     ctl->umax_bits = 0ull;
     ctl->face_fail = ctl->cell_fail = ctl->in_fail = 0u;
     ctl->queue = 0;
+    ctl->abort = 0u;
+    ctl->exec_c2p = ctl->exec_riemann = ctl->exec_hancock = 0u;
+    ctl->exec_newton = 0ull;
     fence_proxy_async();
   }
   __syncthreads();
@@ -229,7 +235,11 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);   // Eq. 28 formed on the device (srhd_fluid_step_cfl)
   const double hdt = dt / (2.0 * dh);
   const double dtdh = dt / dh;
-  unsigned long long my_iters = 0;
+  unsigned long long my_iters = 0;     // iterations of the algorithm's conversions (centre cells + accepted pass)
+  unsigned long long ex_newton = 0;    // executed work (every pass, shortcuts taken into account)
+  unsigned ex_c2p = 0, ex_riemann = 0, ex_hancock = 0;
+  int phase_base = 0;                  // TMA phases completed before the current pass (mbarrier parity)
+  int planes_counted = 0;              // tile planes whose cells already fed newton_iters / S_max / Eq. 30 counters
   unsigned my_in_fail = 0;
   double my_umax = 0.0;
   double beta = beta0;
@@ -247,7 +257,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   // cons2prim of 32 cells of the staged plane pl into its ring slot (Eq. 15-18); pass 0 also feeds
   // the CFL reduction (Eq. 26) and the Eq. 30 counter from the input-interior cells
   auto convert_chunk = [&](int pl, int chunk) {
-    mbar_wait(&ctl->mbar, (uint32_t)(pl & 1));     // NXT is even: plane parity is the same in every pass
+    mbar_wait(&ctl->mbar, (uint32_t)((phase_base + pl) & 1));   // one phase per staged plane, in order
     double* Ws = Wr + (pl % R) * 5 * PL;
     const int item = chunk * 32 + lane;
     const bool valid = item < PL;
@@ -262,7 +272,9 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     if (valid) {
 #pragma unroll
       for (int q = 0; q < 5; ++q) Ws[q * PL + c] = W[0][q];
-      if (pass == 0) {
+      ++ex_c2p;
+      ex_newton += (unsigned)it[0];
+      if (pl >= planes_counted) {          // each tile plane feeds the input-state counters exactly once
         my_iters += (unsigned)it[0];
         const int ti = c % NXT, tj = c / NXT;
         const bool interior = (ti >= G) && (ti < G + 16) && (tj >= G) && (tj < G + 16) && (pl >= G) &&
@@ -280,9 +292,13 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     if (tid == 0) {
       ctl->face_fail = 0u;
       ctl->cell_fail = 0u;
+      ctl->abort = 0u;
       issue_plane(0);
     }
     unsigned my_face_fail = 0, my_cell_fail = 0;
+    unsigned long long pass_iters = 0;            // Newton iterations of this pass's face conversions
+    bool flagged = false, aborted = false;
+    int planes_staged = NXT;
     double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // (Fx+ - Fx-) + (Fy+ - Fy-) of this thread's column cell
 
     // ---- prologue: tile plane 0 -> primitives; stage plane 1
@@ -322,6 +338,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
                                      : ((tk % R) * 5 * PL + cidx + m * ((hd == 0) ? 1 : NXT));
           double um[5], up[5], dF[5];
           const bool warp_flat = hancock_lane<G>(Wr, hd, o, beta, beta0, um, up, dF);
+          ex_hancock += (valid && !warp_flat) ? 1u : 0u;
           double* pm = hpm + soff;
           double* pp = hpp + soff + ((hd == 2) ? zb * 5 * P::ZS : 0);
           const int qs = hqs;
@@ -424,7 +441,10 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
             cons2prim_multi<2>(U, W, aux, rtol, max_iter, phys, it);
           }
           riemann_flux<RS>(d, W[0], U[0], aux[0], W[1], U[1], aux[1], F, same);
-          my_iters += (unsigned)(it[0] + it[1]);
+          pass_iters += (unsigned)(it[0] + it[1]);
+          ex_c2p += same ? 1u : 2u;
+          ex_newton += (unsigned)(same ? it[0] : it[0] + it[1]);
+          ex_riemann += (SRHD_EXACT || !same) ? 1u : 0u;
           my_face_fail += (phys[0] ? 0u : 1u) + (phys[1] ? 0u : 1u);      // S15
           if (fout) {                               // faces on the boundary of an 8^3 patch
             if (idx < 256) {
@@ -480,10 +500,28 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           if (lane == 0) c = atomicAdd(&ctl->queue, 1);
           cq = __shfl_sync(0xffffffffu, c, 0);
         }
+        // A failure anywhere fails the whole pass (S9, S15), so a pass that is not the last rung of the
+        // ladder can be abandoned as soon as one is seen: same verdict, same accepted pass, less work.
+        if (!flagged && beta != 0.0 && (my_face_fail | my_cell_fail) != 0u) {
+          *reinterpret_cast<volatile unsigned int*>(&ctl->abort) = 1u;
+          flagged = true;
+        }
       }
       __syncthreads();
+      if (beta != 0.0 && s + 1 < NXT && *reinterpret_cast<volatile unsigned int*>(&ctl->abort) != 0u) {
+        aborted = true;                           // block uniform; planes 0 .. s+1 were staged and consumed
+        planes_staged = s + 2;
+        break;
+      }
       // the staging buffer is free again: stage conserved plane s+2
       if (tid == 0 && s + 2 < NXT) issue_plane(s + 2);
+    }
+
+    phase_base += planes_staged;
+    planes_counted = max(planes_counted, planes_staged);
+    if (aborted) {
+      __syncthreads();                            // everyone has read ctl->abort before thread 0 clears it
+      continue;                                   // (the loop header moves on to the next rung)
     }
 
     // ---- verdict of this pass for the whole patch group (S9, S10, S15)
@@ -497,14 +535,25 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     n_face_fail = ctl->face_fail;
     n_cell_fail = ctl->cell_fail;
     __syncthreads();
-    if ((n_face_fail == 0 && n_cell_fail == 0) || beta == 0.0) break;
+    if ((n_face_fail == 0 && n_cell_fail == 0) || beta == 0.0) {
+      my_iters += pass_iters;                     // the accepted pass's face conversions count, no other pass's
+      break;
+    }
   }
 
   // ---- per-call counters
   my_iters = warp_sum(my_iters);
   my_in_fail = (unsigned)warp_sum(my_in_fail);
   my_umax = warp_max(my_umax);
+  ex_newton = warp_sum(ex_newton);
+  ex_c2p = (unsigned)warp_sum(ex_c2p);
+  ex_riemann = (unsigned)warp_sum(ex_riemann);
+  ex_hancock = (unsigned)warp_sum(ex_hancock);
   if (lane == 0) {
+    atomicAdd(&ctl->exec_newton, ex_newton);
+    atomicAdd(&ctl->exec_c2p, ex_c2p);
+    atomicAdd(&ctl->exec_riemann, ex_riemann);
+    atomicAdd(&ctl->exec_hancock, ex_hancock);
     atomicAdd(&ctl->newton, my_iters);
     if (my_in_fail) atomicAdd(&ctl->in_fail, my_in_fail);
     atomicMax(&ctl->umax_bits, (unsigned long long)__double_as_longlong(my_umax));
@@ -516,6 +565,11 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     if (nf) atomicAdd(&stats->n_c2p_fail, nf);
     if (n_cell_fail) atomicAdd(&stats->n_unphys_final, (unsigned long long)n_cell_fail);
     if (pass > 0) atomicAdd(&stats->n_retry_pg, 1ull);
+    atomicAdd(&stats->n_passes, (unsigned long long)(pass + 1));
+    atomicAdd(&stats->exec_newton, ctl->exec_newton);
+    atomicAdd(&stats->exec_c2p, (unsigned long long)ctl->exec_c2p);
+    atomicAdd(&stats->exec_riemann, (unsigned long long)ctl->exec_riemann);
+    atomicAdd(&stats->exec_hancock, (unsigned long long)ctl->exec_hancock);
     const double umax = __longlong_as_double((long long)ctl->umax_bits);
     atomic_max_nonneg(&stats->max_speed, smax_of_umax(umax));      // Eq. 27 per group, then max
   }

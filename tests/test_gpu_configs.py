@@ -158,7 +158,7 @@ def _sampled_full_size(ref, st, recon, riemann, nsteps, nsample, seed, always=()
         # exact build on the same ghosted input: every cell and counter, bit for bit
         ex, sbuf = B.fluid_step(d_tiles, dt, st.dh, B.params(recon, riemann, exact=True), exact=True)
         assert np.array_equal(ex.cpu().numpy(), want)
-        assert B.stats_to_host(sbuf).as_dict() == ost.as_dict()
+        assert B.stats_to_host(sbuf).algorithm_dict() == ost.as_dict()
         err = step_err_local(got, want, tiles, st.par.ghost)
         worst = max(worst, float(err.max()))
         frac_bad.append(float((err > TOL_STEP).mean()))

@@ -52,7 +52,7 @@ def test_two_patch_groups_all_instantiations(ref, recon, riemann, forced_retry):
         if exact:
             assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
             assert np.array_equal(gflux.cpu().numpy(), wflux, equal_nan=True)
-            assert s.as_dict() == st.as_dict()
+            assert s.algorithm_dict() == st.as_dict()
         elif st.n_retry_pg == 0:
             assert step_err(got.cpu().numpy(), want, 2).max() <= 1e-11
 
