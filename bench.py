@@ -1,16 +1,20 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the whole SRHD hot path on B200 (one JSON line on stdout).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload blast256|random512|jet|tube|conv]
-                    [--impl ours|reference] [--no-e2e] [--no-cpu-baseline]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload jet|random512|blast256|tube|conv]
+                    [--impl ours|reference] [--no-e2e] [--no-cpu-baseline] [--no-per-workload]
 
 A "step" is one pass of the whole hot path over the grid (driver.GridStepper.step_async): ghost-zone
 fill from the patches of the previous step fused with the CFL reduction (srhd_patch_gather_speed), then
-srhd_fluid_step_cfl (dt formed on the device).  Default workload:
-BASELINE.json configs[2] (256^3 spherical blast, PPM+HLLC, CFL 0.4) -- the 3-D fluid step the
-metric "fp64 SRHD cell updates/s" is quoted on.  N > 1 runs N independent
-replicas (the path does not shard on this tier: DESIGN.md section 8); value = all ranks' cell
-updates / max-over-ranks device time.
+srhd_fluid_step_cfl (dt formed on the device).  The headline `value` is K steps after W warm-up steps of
+the default workload, BASELINE.json configs[4] (512x512x1024 jet, PPM+HLLC, CFL 0.4: the largest
+configuration, it fits one GPU).  `config.per_workload` carries the three 3-D configs (blast256,
+random512, jet) each timed over ITS OWN step count (100 / 50 / 50) from its initial condition, and
+`roofline` is quoted on random512 -- the general path: no uniform region, so no shortcut applies --
+with the headline workload's figures beside it.  Two fractions: `frac` from the flops of the work the
+method defines per cell update, `frac_executed` from the work the kernel counted itself executing
+(srhd_stats.exec_*).  N > 1 runs N independent replicas (the path does not shard on this tier:
+DESIGN.md section 8); value = all ranks' cell updates / max-over-ranks device time.
 
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
 workload on the host cores; see DESIGN.md section 7.
@@ -187,11 +191,6 @@ def aggregate_value(ncell_per_rank, steps, ms_local, world, device):
     return world * ncell_per_rank * steps / (ms_max * 1e-3), ms_max
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE fluid_step_kernel launch, from the ncu --set full
-# capture named beside each entry (profiles/); None until a capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"blast256": 2.40e9}   # profiles/r1i_fluid_step_ppm_hllc.md (dram read + write of one launch)
-
-
 def run_conv(args):
     """--workload conv: BASELINE.json configs[1], 2^24 states, prim -> cons -> prim per step."""
     import torch
@@ -269,7 +268,7 @@ def run_conv(args):
                    "eq30_failures": s.n_c2p_fail},
         "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": "cons2prim_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                     "frac": ach / peak, "traffic": None, "kernel_ms": c2p_ms, "peak_measured": peak_meas,
+                     "frac": ach / peak, "traffic": ncu_traffic("conv"), "kernel_ms": c2p_ms, "peak_measured": peak_meas,
                      "flops_per_state": fm.c2p(k_mean),
                      "hbm": {"achieved": n * 80 / (c2p_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                              "frac": n * 80 / (c2p_ms * 1e-3) / 1e9 / hbm_peak},
@@ -282,38 +281,31 @@ def run_conv(args):
     print(json.dumps(out))
 
 
-# Warp-instruction counts of ONE fluid_step_kernel launch from the ncu capture named beside them
-# (smsp__inst_executed.sum and its fp64 part): feed the issue-cycle accounting of DESIGN.md section 6
-# (an fp64 warp instruction holds a sub-partition's issue port for 2 cycles, any other for 1).
-NCU_WARP_INST = {"blast256": {"fp64": 0.687e9, "other": 1.190e9, "source": "profiles/r1i_fluid_step_ppm_hllc.md"}}
+CONFIG_STEPS = {"blast256": 100, "random512": 50, "jet": 50, "tube": 205}   # BASELINE.json configs: their own step counts
 
 
-def run_ours(args):
-    if args.workload == "conv":
-        return run_conv(args)
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE fluid_step_kernel launch on this workload, from
+    the committed ncu --set full capture summarised in profiles/ncu_traffic.json (written from the capture
+    named inside it; nothing here is measured under a profiler).  None if no capture of that workload."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        return t.get(workload, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+def time_workload(name, steps, warmup, scale, world, local, rank, from_start=False, e2e_steps=0):
+    """Time `steps` steps of one workload after `warmup` untimed ones (from_start: the config's own run from
+    its initial condition, warm-up on a second instance).  Returns a dict of measured figures."""
     import torch
     import torch.distributed as dist
     from paper_2012_11130_b200 import binding as B
-    from paper_2012_11130_b200 import build as cuda_build
     from paper_2012_11130_b200 import flopmodel as fm
     from paper_2012_11130_b200.driver import GridStepper
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if rank == 0:
-        cuda_build.build()
-    if world > 1:
-        dist.barrier()
-    B.load_library()
-
-    recon, riemann, cfl, desc = WORKLOADS[args.workload]
-    prim, dh, bc, inflow = make_workload(args.workload, scale=args.scale)
+    recon, riemann, cfl, desc = WORKLOADS[name]
+    prim, dh, bc, inflow = make_workload(name, scale=scale)
     shape = prim.shape[1:]
     st_inflow = None
     if inflow is not None:
@@ -321,10 +313,10 @@ def run_ours(args):
         cj = B.prim2cons(torch.from_numpy(prim_jet.reshape(5, 1).copy()).cuda()).cpu().numpy().ravel()
         st_inflow = (mask, cj)
     st = GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=st_inflow)
-    st.set_prim(prim)
+    prim_d = torch.from_numpy(prim).cuda() if from_start else None
+    st.set_prim(prim if prim_d is None else prim_d)
     del prim
     ncell = st.ncell
-    torch.cuda.synchronize()
 
     def barrier():
         torch.cuda.synchronize()
@@ -332,36 +324,60 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         st.step_async()
+    if from_start:                      # warm-up done (clocks, caches, lazy module load): restart from t = 0
+        st.set_prim(prim_d)
+        del prim_d
     barrier()
-    peak_meas = B.fp64_peak_probe() if rank == 0 else None     # measured DFMA roof (outside the timed region)
-    barrier()
-
-    # ---- device-resident timing: K steps, CUDA events on the launching (current) stream
     sampler = ClockSampler(local)
     sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    kev, iters, retries = [], 0, 0
+    kev = []
+    tot = {k: 0 for k in ("n_retry_pg", "n_passes", "newton_iters", "exec_c2p", "exec_newton", "exec_riemann",
+                          "exec_hancock", "n_unphys_final")}
+    # per-step counters are read back AFTER the timed region from a device-side log (no host sync inside it)
+    log = torch.zeros((steps, st.stats.numel()), dtype=torch.uint8, device="cuda")
     ev0.record()
-    for _ in range(args.steps):
-        st.step_async(kernel_events=kev)          # dt = C dh / S_max formed on the device: no host sync
+    for i in range(steps):
+        st.step_async(kernel_events=kev)           # dt = C dh / S_max formed on the device: no host sync
+        log[i].copy_(st.stats, non_blocking=True)  # 80-byte device-to-device copy of this step's counters
     ev1.record()
     barrier()
     clocks = sampler.result()
     ms = ev0.elapsed_time(ev1)
     k_ms = sum(a.elapsed_time(b) for a, b in kev) / len(kev)
-    s = st.last_stats()
-    value, ms_max = aggregate_value(ncell, args.steps, ms, world, "cuda")
-
-    # ---- end to end through the public API: every step copies its input grid from pinned host
-    # memory, runs GridStepper.step_async() (CFL reduction of the fresh grid, gather, fluid step with
-    # dt formed on the device, scatter) and copies the result back.  n_pipe independent problem
-    # instances (each with its own buffers and CUDA stream) are in flight round-robin, so one
-    # instance's PCIe copies overlap another's kernels; within an instance step n+1 starts from the
-    # host copy of step n's result.
-    e2e = None
-    if not args.no_e2e:
+    for row in log.cpu():
+        s = B.Stats.from_buffer_copy(row.numpy().tobytes())
+        for k in tot:
+            tot[k] += getattr(s, k)
+    value, ms_max = aggregate_value(ncell, steps, ms, world, "cuda")
+    nxt = 16 + 2 * st.par.ghost
+    nconv = steps * st.npg * (nxt ** 3 + 2 * 3 * 17 * 256)        # conversions the algorithm defines
+    k_mean = tot["newton_iters"] / nconv
+    flops_alg = ncell * fm.fluid_step_flops_per_cell(recon, riemann, k_mean)          # per step
+    flops_exe = fm.fluid_step_flops_executed(recon, riemann, ncell * steps, tot["exec_c2p"], tot["exec_newton"],
+                                             tot["exec_riemann"], tot["exec_hancock"]) / steps
+    res = {
+        "name": name, "desc": desc, "recon": recon, "riemann": riemann, "cfl": cfl, "shape": list(shape),
+        "npg": st.npg, "ncell": ncell, "steps": steps, "warmup": warmup, "from_start": from_start,
+        "value": value, "ms_per_step": ms_max / steps, "kernel_ms": k_ms, "clocks": clocks,
+        "k_mean": k_mean, "flops_alg_per_step": flops_alg, "flops_exec_per_step": flops_exe,
+        "passes_per_group": tot["n_passes"] / (steps * st.npg), "retry_groups_per_step": tot["n_retry_pg"] / steps,
+        "unphysical_cells": tot["n_unphys_final"],
+        "exec_conversions_per_cell": tot["exec_c2p"] / (ncell * steps),
+        "exec_newton_per_conversion": tot["exec_newton"] / max(tot["exec_c2p"], 1),
+        "exec_riemann_per_cell": tot["exec_riemann"] / (ncell * steps),
+        "state_mb": st.grid.numel() * 8 / 1e6, "tiles_mb": st.tiles.numel() * 8 / 1e6,
+        "launches_per_step": st.launches_per_step,
+    }
+    if e2e_steps:
+        # end to end through the public API: every step copies its input grid from pinned host memory, runs
+        # GridStepper.step_async() (CFL reduction of the fresh grid, ghost-zone fill, fluid step with dt formed
+        # on the device, scatter) and copies the result back.  n_pipe INDEPENDENT problem instances (own
+        # buffers, own CUDA stream) are in flight round-robin so one instance's PCIe copies overlap another's
+        # kernels: the figure is aggregate throughput over independent instances, the latency of one step of
+        # one instance is about n_pipe times longer.
         nbytes = st.grid.numel() * 8
         n_pipe = 3 if nbytes * 5 < 20e9 else 1
         inst = [st] + [GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=st_inflow) for _ in range(n_pipe - 1)]
@@ -370,7 +386,7 @@ def run_ours(args):
         h_out = [torch.empty(st.grid.shape, dtype=torch.float64, pin_memory=True) for _ in range(n_pipe)]
         for h in h_in:
             h.copy_(st.grid)
-        n_e2e = max(n_pipe, min(args.steps, 12) // n_pipe * n_pipe)
+        n_e2e = max(n_pipe, e2e_steps // n_pipe * n_pipe)
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
@@ -388,57 +404,125 @@ def run_ours(args):
         e1.record()
         barrier()
         e2e_value, _ = aggregate_value(ncell, n_e2e, e0.elapsed_time(e1), world, "cuda")
-        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-               "steps": n_e2e, "instances_in_flight": n_pipe}
-        del inst[1:], h_in, h_out
+        res["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                      "steps": n_e2e, "instances_in_flight": n_pipe,
+                      "note": "aggregate over independent problem instances in flight; per-instance step latency is about instances_in_flight times longer"}
+        del inst, h_in, h_out
+    del st
+    torch.cuda.empty_cache()
+    return res
 
+
+def roofline_of(r, peak, peak_meas, hbm_peak, have_peaks):
+    """Roofline object of fluid_step_kernel on one timed workload (ALU bound: DESIGN.md section 6)."""
+    from paper_2012_11130_b200 import flopmodel as fm
+    t = r["kernel_ms"] * 1e-3
+    ach = r["flops_alg_per_step"] / t / 1e12
+    exe = r["flops_exec_per_step"] / t / 1e12
+    hbm_ach = r["ncell"] * fm.FLUID_STEP_BYTES_PER_CELL / t / 1e9
+    return {
+        "bound": "alu", "kernel": "fluid_step_kernel", "workload": r["name"], "unit": "TFLOP/s",
+        "achieved": ach, "peak": peak, "frac": ach / peak,
+        "achieved_executed": exe, "frac_executed": exe / peak,
+        "achieved_note": "achieved = flops of the work the METHOD defines per cell update (no ghost-zone recompute, no thrown-away retry passes, no shortcuts) / kernel time; achieved_executed = flops of the conversions, Riemann solves and edge states the kernel actually executed (srhd_stats.exec_*) / kernel time",
+        "peak_source": "148 SMs x 64 fp64 lanes x 2 x max SM clock (unit counts; DESIGN.md section 6)",
+        "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
+        "frac_executed_of_measured": exe / peak_meas if peak_meas else None,
+        "peak_measured_source": "srhd_fp64_peak_probe (register-only DFMA loop) in this run",
+        "kernel_ms": r["kernel_ms"], "ms_per_step": r["ms_per_step"], "steps": r["steps"],
+        "kernel_share_of_step": r["kernel_ms"] / r["ms_per_step"],
+        "flops_per_cell": r["flops_alg_per_step"] / r["ncell"],
+        "flops_executed_per_cell": r["flops_exec_per_step"] / r["ncell"],
+        "traffic": ncu_traffic(r["name"]),
+        "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
+                "peak_source": "MEASURED_PEAKS.json" if have_peaks else "fallback 6650 GB/s (B200_PROFILING.md)"},
+    }
+
+
+def summary_of(r):
+    return {"what": r["desc"], "grid": r["shape"], "scheme": f'{r["recon"]}+{r["riemann"]}', "cfl": r["cfl"],
+            "steps": r["steps"], "from_initial_condition": r["from_start"], "value": r["value"], "unit": UNIT,
+            "ms_per_step": r["ms_per_step"], "kernel_ms": r["kernel_ms"],
+            "newton_iters_per_conversion": r["k_mean"], "passes_per_patch_group": r["passes_per_group"],
+            "retry_patch_groups_per_step": r["retry_groups_per_step"], "unphysical_cells": r["unphysical_cells"],
+            "executed_conversions_per_cell": r["exec_conversions_per_cell"],
+            "executed_riemann_solves_per_cell": r["exec_riemann_per_cell"],
+            "sm_mhz": r["clocks"]["sm_mhz"], "throttle_reasons": r["clocks"]["reasons"]}
+
+
+def run_ours(args):
+    if args.workload == "conv":
+        return run_conv(args)
+    import torch
+    import torch.distributed as dist
+    from paper_2012_11130_b200 import binding as B
+    from paper_2012_11130_b200 import build as cuda_build
+    from paper_2012_11130_b200 import flopmodel as fm
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        cuda_build.build()
+    if world > 1:
+        dist.barrier()
+    B.load_library()
+
+    # ---- headline: K steps of the chosen workload after W warm-up steps, then end to end
+    head = time_workload(args.workload, args.steps, args.warmup, args.scale, world, local, rank,
+                         e2e_steps=0 if args.no_e2e else min(args.steps, 6))
+    # ---- every 3-D config over its OWN step count from its initial condition (seconds of GPU time)
+    per = {}
+    if args.per_workload and world == 1:
+        for name in ("blast256", "random512", "jet"):
+            per[name] = time_workload(name, max(1, CONFIG_STEPS[name] // (args.scale if args.scale > 1 else 1)), 3,
+                                      args.scale, world, local, rank, from_start=True)
+    if world > 1:
+        dist.barrier()
     if rank != 0:
         return
-    # ---- roofline of the dominant kernel (fluid_step_kernel): ALU bound
-    nxt = 16 + 2 * st.par.ghost
-    nconv = st.npg * (nxt ** 3 + 2 * 3 * 17 * 256)
-    k_mean = s.newton_iters / nconv
-    flops = ncell * fm.fluid_step_flops_per_cell(recon, riemann, k_mean)
-    peak = fm.fp64_peak_tflops(clocks["sm_max_mhz"] or 1965.0)
-    ach = flops / (k_ms * 1e-3) / 1e12
+    torch.cuda.synchronize()
+    peak_meas = B.fp64_peak_probe()                # measured DFMA roof (outside every timed region)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
-    hbm_ach = ncell * fm.FLUID_STEP_BYTES_PER_CELL / (k_ms * 1e-3) / 1e9
-    issue = None
-    if args.workload in NCU_WARP_INST and args.scale == 1:
-        wi = NCU_WARP_INST[args.workload]
-        cycles = k_ms * 1e-3 * (clocks["sm_mhz"] or clocks["sm_max_mhz"] or 1965.0) * 1e6 * fm.NUM_SMS * 4
-        issue = {"frac": (2 * wi["fp64"] + wi["other"]) / cycles, "fp64_pipe_frac": 2 * wi["fp64"] / cycles,
-                 "fp64_warp_inst": wi["fp64"], "other_warp_inst": wi["other"], "counts_from": wi["source"],
-                 "rule": "fp64 instruction = 2 issue cycles per sub-partition, any other = 1 (measured, DESIGN.md section 6)"}
+    peak = fm.fp64_peak_tflops(head["clocks"]["sm_max_mhz"] or 1965.0)
+    # the roofline is quoted on the GENERAL path: random512 has no uniform region, so none of the
+    # uniform-region shortcuts applies there; the headline workload's own figures sit beside it
+    general = per.get("random512", head)
+    roof = roofline_of(general, peak, peak_meas, hbm_peak, bool(peaks))
+    roof["headline_workload"] = {k: v for k, v in roofline_of(head, peak, peak_meas, hbm_peak, bool(peaks)).items()
+                                 if k in ("workload", "achieved", "frac", "achieved_executed", "frac_executed", "kernel_ms",
+                                          "ms_per_step", "steps", "kernel_share_of_step", "flops_per_cell",
+                                          "flops_executed_per_cell", "traffic")}
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "what": desc, "grid": list(shape), "patch_groups": st.npg,
-                   "scheme": f"{recon}+{riemann}", "cfl": cfl, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": f"inputs larger than L2 ({st.grid.numel() * 8 / 1e6:.0f} MB state, {st.tiles.numel() * 8 / 1e6:.0f} MB tiles)"
-                         if st.grid.numel() * 8 > 126e6 else "state fits L2 (small case)",
-                   "newton_iters_per_conversion": k_mean, "retry_patch_groups_last_step": s.n_retry_pg,
-                   "unphysical_cells_last_step": s.n_unphys_final},
-        "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": "fluid_step_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                     "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-                     "peak_source": "148 SMs x 64 fp64 lanes x 2 x max SM clock (unit counts; DESIGN.md section 6)",
-                     "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
-                     "peak_measured_source": "srhd_fp64_peak_probe (register-only DFMA loop) in this run",
-                     "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (ms / args.steps),
-                     "flops_per_cell": flops / ncell, "issue_cycles": issue,
-                     "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
-                             "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"}},
-        "gpu_launches": st.launches_per_step * args.steps + (2 if args.warmup == 0 else 0),
+        "config": {"workload": args.workload, "what": head["desc"], "grid": head["shape"], "patch_groups": head["npg"],
+                   "scheme": f'{head["recon"]}+{head["riemann"]}', "cfl": head["cfl"],
+                   "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": f'inputs larger than L2 ({head["state_mb"]:.0f} MB state, {head["tiles_mb"]:.0f} MB tiles)'
+                         if head["state_mb"] > 126 else "state fits L2 (small case)",
+                   "timed_steps": f'steps {args.warmup + 1}..{args.warmup + args.steps} from the initial condition',
+                   "newton_iters_per_conversion": head["k_mean"], "passes_per_patch_group": head["passes_per_group"],
+                   "retry_patch_groups_per_step": head["retry_groups_per_step"],
+                   "executed_conversions_per_cell": head["exec_conversions_per_cell"],
+                   "per_workload": {k: summary_of(v) for k, v in per.items()}},
+        "clocks": head["clocks"],
+        "roofline": roof,
+        "gpu_launches": head["launches_per_step"] * args.steps,
     }
-    if e2e:
-        out["e2e"] = e2e
+    if "e2e" in head:
+        out["e2e"] = head["e2e"]
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(args.workload)
     print(json.dumps(out))
@@ -450,7 +534,10 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="blast256", choices=sorted(WORKLOADS) + ["conv"])
+    ap.add_argument("--workload", default="jet", choices=sorted(WORKLOADS) + ["conv"],
+                    help="headline workload; default = the largest single-GPU config, BASELINE.json configs[4]")
+    ap.add_argument("--no-per-workload", dest="per_workload", action="store_false",
+                    help="skip the runs of blast256 / random512 / jet over their own step counts")
     ap.add_argument("--scale", type=int, default=1, help="divide the grid extents (debugging only; 1 = the config)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

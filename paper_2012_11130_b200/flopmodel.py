@@ -62,3 +62,14 @@ NUM_SMS = 148
 
 def fp64_peak_tflops(sm_mhz=1965.0):
     return NUM_SMS * FP64_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
+
+
+def fluid_step_flops_executed(recon, riemann, ncell, exec_c2p, exec_newton, exec_riemann, exec_hancock):
+    """Flops of the work the kernel actually executed (srhd_stats.exec_*): conversions and their Newton
+    iterations (retry passes, ghost-zone cells and shortcuts as they happened), Riemann solves, edge-state
+    pairs of the Hancock stage, plus the per-cell update / Eq. 30 check / U_max of the interior cells."""
+    solver = HLLE if riemann in (0, "hlle") else HLLC
+    rec = 5 * (PLM_COMPONENT if recon in (0, "plm") else PPM_COMPONENT)
+    hancock = rec + 2 * (P2C + PHYS_FLUX) + 5 + 10 + 10       # per (cell, direction): dF, share of the sum, two adds
+    return (exec_c2p * C2P_FIXED + exec_newton * NEWTON_ITER + exec_riemann * (2 * SIDE_SETUP + solver) +
+            exec_hancock * hancock + ncell * (UPDATE + EQ30_CHECK + UMAX))
