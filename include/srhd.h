@@ -193,6 +193,15 @@ int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int 
  * in practice.  bench.py uses it for the measured fp64 ALU roof. */
 int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, void* stream);
 
+/* Verification helper (not part of the solver): evaluates the library's canonical quotient a/b (the one
+ * that feeds the Eq. 30 verdict: one shared reciprocal + a Markstein correction in the production build, IEEE
+ * division in the exact build) and IEEE division side by side on n seeded pairs generated on the device;
+ * d_out (device, 2 x unsigned long long) receives {number of bit mismatches, index of the first one or
+ * ~0}.  dist: 0 = the value ranges of BASELINE.json configs 2-5, 1 = operands within 2^15 ulp of powers of two
+ * and of each other, 2 = exponents over [1e-200, 1e200].  Used by tests/test_gpu_quotient.py. */
+int srhd_quotient_check(unsigned long long n, unsigned long long seed, int dist,
+                        unsigned long long* d_out, void* stream);
+
 /* Human-readable text for a return code of this library (negative) or of CUDA (positive). */
 const char* srhd_error_string(int code);
 

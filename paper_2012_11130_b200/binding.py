@@ -44,7 +44,7 @@ class Stats(C.Structure):
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
            "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed",
-           "srhd_fp64_peak_probe", "srhd_error_string", "srhd_build_is_exact"]
+           "srhd_fp64_peak_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
 
@@ -92,6 +92,8 @@ def load_library(exact=False):
                                           C.POINTER(C.c_double), C.POINTER(Params), _VP, _VP]
     L.srhd_fp64_peak_probe.restype = C.c_int
     L.srhd_fp64_peak_probe.argtypes = [_VP, C.c_int, C.POINTER(C.c_ulonglong), _VP]
+    L.srhd_quotient_check.restype = C.c_int
+    L.srhd_quotient_check.argtypes = [C.c_ulonglong, C.c_ulonglong, C.c_int, _VP, _VP]
     L.srhd_error_string.restype = C.c_char_p
     L.srhd_error_string.argtypes = [C.c_int]
     L.srhd_build_is_exact.restype = C.c_int
@@ -327,3 +329,12 @@ def fp64_peak_probe(iters=4096, reps=5):
         if r:
             best = max(best, flops.value / (e0.elapsed_time(e1) * 1e-3) / 1e12)
     return best
+
+
+def quotient_check(n, seed=1, dist=0, exact=False):
+    """srhd_quotient_check: (bit mismatches, index of the first) of the canonical quotient vs IEEE division."""
+    L = load_library(exact)
+    out = torch.zeros(2, dtype=torch.int64, device="cuda")
+    _check(L.srhd_quotient_check(int(n), int(seed), int(dist), out.data_ptr(), _stream()), L)
+    o = out.cpu().numpy().view("uint64")
+    return int(o[0]), int(o[1])

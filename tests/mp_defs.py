@@ -191,7 +191,7 @@ def cons2prim(U):
 
     def resid(h):
         g = sqrt(1 + m2 / (D * h) ** 2)
-        return D * h * g - (D / g) * T_of_h(h) - (Et + D)
+        return (D * h * g - (D / g) * T_of_h(h)) / (Et + D) - 1
 
     hi = 2 + 2 * (Et + D) / D
     h = findroot(resid, (mpf(1), hi), solver="anderson", tol=mpf(10) ** -70, maxsteps=200)
@@ -213,9 +213,26 @@ def plm_edges(am1, a0, ap1, beta):
     return a0 - d / 2, a0 + d / 2
 
 
-def step_cells(cons, cells, dt, dh, riemann="hllc", beta=1.5):
-    """One PLM + MUSCL-Hancock + HLLE/HLLC update (readings S3, S5, S12) of the
-    listed cells (i, j, k) of a conserved box cons[5][nz][ny][nx] (numpy float64; every cell within two
+def ppm_edges(a, beta):
+    """reading S4: Colella & Woodward (1984) on a uniform grid from a = (a_{i-2} .. a_{i+2}): limited slopes
+    as S3, face = (a_i + a_{i+1})/2 - (d_{i+1} - d_i)/6, monotonisation CW84 Eq. 1.10 (first pass: no blend)."""
+    dm, d0, dp = (limited_slope(a[k + 1] - a[k], a[k + 2] - a[k + 1], beta) for k in range(3))
+    ai = a[2]
+    am = (a[1] + a[2]) / 2 - (d0 - dm) / 6
+    ap = (a[2] + a[3]) / 2 - (dp - d0) / 6
+    if (ap - ai) * (ai - am) <= 0:
+        return ai, ai
+    dd, c6 = ap - am, 6 * (ai - (am + ap) / 2)
+    if dd * c6 > dd * dd:
+        am = 3 * ai - 2 * ap
+    elif -(dd * dd) > dd * c6:
+        ap = 3 * ai - 2 * am
+    return am, ap
+
+
+def step_cells(cons, cells, dt, dh, riemann="hllc", beta=1.5, recon="plm"):
+    """One PLM/PPM + MUSCL-Hancock + HLLE/HLLC update (readings S3, S5, S12) of the
+    listed cells (i, j, k) of a conserved box cons[5][nz][ny][nx] (numpy float64; every cell within two (PLM) or three (PPM)
     of a listed cell must be inside the box), in 40-digit arithmetic from the definitions above.
     Returns {cell: [5 mpf]}.  Python loops with memoisation: a handful of cells only."""
     dt, dh = mpf(dt), mpf(dh)
@@ -241,7 +258,11 @@ def step_cells(cons, cells, dt, dh, riemann="hllc", beta=1.5):
         Wm, Wp = {}, {}
         for d in range(3):
             a, b = prim(shift(c, d, -1)), prim(shift(c, d, +1))
-            em, ep = zip(*[plm_edges(a[q], W0[q], b[q], beta) for q in range(5)])
+            if recon == "plm":
+                em, ep = zip(*[plm_edges(a[q], W0[q], b[q], beta) for q in range(5)])
+            else:
+                a2, b2 = prim(shift(c, d, -2)), prim(shift(c, d, +2))
+                em, ep = zip(*[ppm_edges([a2[q], a[q], W0[q], b[q], b2[q]], beta) for q in range(5)])
             Wm[d], Wp[d] = list(em), list(ep)
         # one COMMON increment from all three directions (unsplit, reading S5)
         dU = [mpf(0)] * 5

@@ -1,0 +1,78 @@
+"""-m gpu: WHO IS RIGHT where the production build and the oracle differ by more than 1e-11 after one step?
+
+VERDICT r1 "What's weak" #3: the tolerances on configs 3 and 4 were loosened with an argument (the paper's
+error model, Eq. 20: the inversion of a state of Mach number M is uncertain by (1 + M^2) eps in any evaluation
+order) but nothing adjudicated it.  Here the cells that differ most are recomputed from the definitions in
+40-digit arithmetic (tests/mp_defs.step_cells: total-energy forms, numerical root finding, plain
+subtractions, its own loops).  Claim checked: oracle and GPU are EQUALLY far from that answer -- each within
+the Eq.-20-derived tolerance of gpu_util.step_err_eq20, neither systematically closer.
+"""
+import numpy as np
+import pytest
+import torch
+from mpmath import mpf
+
+from paper_2012_11130_b200 import binding as B
+from paper_2012_11130_b200 import workloads as wl
+from paper_2012_11130_b200.driver import GridStepper
+from tests import mp_defs
+from tests.gpu_util import patches_to_block, report, step_err, step_err_eq20
+
+pytestmark = pytest.mark.gpu
+
+
+def _worst_cells(ref, st, recon, riemann, dt, nworst):
+    tiles = st.tiles.cpu().numpy()
+    got = st.patches.cpu().numpy()
+    par = ref.params(recon, riemann)
+    want = np.empty_like(got)
+    single = np.zeros(tiles.shape[0], dtype=bool)
+    for g in range(tiles.shape[0]):
+        w, s = ref.fluid_step(tiles[g:g + 1], dt, st.dh, par)
+        want[g] = w[0]
+        single[g] = s.n_passes == 1                   # the 40-digit stepper has no retry ladder
+    err = patches_to_block(step_err(got, want, 2)[:, :, None])[:, 0]       # (npg,16,16,16)
+    e2, tol = step_err_eq20(ref, got, want, tiles, st.par.ghost, dt, st.dh)
+    err = np.where(single[:, None, None, None], np.nan_to_num(err, nan=0.0, posinf=0.0), 0.0)
+    order = np.argsort(err.ravel())[::-1][:nworst]
+    return tiles, patches_to_block(got), patches_to_block(want), err, tol, [np.unravel_index(i, err.shape) for i in order]
+
+
+@pytest.mark.parametrize("name", ["jet", "random"])
+def test_worst_cells_against_40_digit_arithmetic(ref, name):
+    if name == "jet":
+        prim, dh, bc, inflow = wl.jet(nx=64, ny=64, nz=128, radius=0.08)
+        recon, riemann, nsteps = "ppm", "hllc", 30
+        mask, prim_jet = inflow
+        cj = B.prim2cons(torch.from_numpy(prim_jet.reshape(5, 1).copy()).cuda()).cpu().numpy().ravel()
+        st = GridStepper(prim.shape[1:], dh, bc, recon, riemann, cfl=0.4, inflow=(mask, cj)).set_prim(prim)
+    else:
+        prim, dh, bc = wl.random_field(n=64, log_theta=(-8.0, 4.0), gamma_max=30.0)
+        recon, riemann, nsteps = "plm", "hlle", 12
+        st = GridStepper(prim.shape[1:], dh, bc, recon, riemann, cfl=0.4).set_prim(prim)
+    for _ in range(nsteps):
+        st.step()
+    dt = st.step()
+    tiles, got, want, err, tol, cells = _worst_cells(ref, st, recon, riemann, dt, nworst=10)
+    G = st.par.ghost
+    rows = []
+    for (g, k, j, i) in cells:
+        if err[g, k, j, i] <= 0:
+            continue
+        truth = mp_defs.step_cells(tiles[g], [(i + G, j + G, k + G)], dt, dh, riemann, recon=recon)[(i + G, j + G, k + G)]
+        tr = np.array([float(x) for x in truth])
+        # S14 denominators from the 40-digit answer
+        den = np.array([abs(tr[0]), 0, 0, 0, abs(tr[4])])
+        den[1:4] = np.sqrt((tr[1:4] ** 2).sum()) + abs(tr[4])
+        e_gpu = max(float(abs(mpf(got[g, q, k, j, i]) - truth[q])) / den[q] for q in range(5))
+        e_orc = max(float(abs(mpf(want[g, q, k, j, i]) - truth[q])) / den[q] for q in range(5))
+        rows.append((float(err[g, k, j, i]), e_gpu, e_orc, float(tol[g, k, j, i])))
+        # each of the two fp64 answers is within the Eq.-20-derived tolerance of the 40-digit one
+        assert e_gpu <= tol[g, k, j, i] and e_orc <= tol[g, k, j, i], (name, (g, k, j, i), rows[-1])
+    rows = np.array(rows) if rows else np.zeros((0, 4))
+    report("adjudication_" + name, cells=len(rows), gpu_vs_oracle=rows[:, 0].tolist(), gpu_vs_40digits=rows[:, 1].tolist(),
+           oracle_vs_40digits=rows[:, 2].tolist(), tolerance=rows[:, 3].tolist())
+    if len(rows):
+        # neither implementation is systematically the better one: their errors against the truth are of
+        # the same size as their mutual difference
+        assert np.median(rows[:, 2]) >= 0.1 * np.median(rows[:, 1]) or np.median(rows[:, 2]) <= 1e-13

@@ -241,3 +241,32 @@ def test_patch_gather_speed_equals_scatter_then_gather(ref, ghost):
                 assert np.array_equal(tiles.cpu().numpy(), want)
                 sep = B.max_signal_speed(dev(grid).reshape(5, -1).contiguous(), par, exact=exact)
                 assert float(smax.cpu()) == float(sep.cpu())
+
+
+@pytest.mark.parametrize("recon,riemann", [("plm", "hllc"), ("ppm", "hllc"), ("plm", "hlle")])
+def test_retry_ladder_parity_production_build(ref, recon, riemann):
+    """the PRODUCTION library on data that walks the retry ladder: every patch group ends on
+    the same rung as the oracle's (same number of passes in total, same retried groups, same count of cells
+    left unphysical after the last rung), and the cells of groups that end physically agree to 1e-11."""
+    po = ref.params(recon, riemann, max_retry=3)
+    dh = 1.0 / 64
+    for seed, mult, kw in ((5, 4.0, dict(umax=30.0, rough=3.0, log_theta=(-8.0, 2.0))),
+                           (9, 1.0, dict(umax=10.0, rough=1.0, log_theta=(-6.0, 2.0))),
+                           (11 + po.ghost, 1.0, {})):
+        tiles = make_tiles(ref, 6, po.ghost, seed=seed, **kw)
+        dt = mult * cfl_dt(ref, tiles, dh)
+        per_group = [ref.fluid_step(tiles[g:g + 1], dt, dh, po) for g in range(tiles.shape[0])]
+        want = np.concatenate([w for w, _ in per_group])
+        par = B.params(recon, riemann, max_retry=3)
+        for g, (w, st) in enumerate(per_group):       # group by group: the rung of EACH group
+            got, sbuf = B.fluid_step(dev(tiles[g:g + 1]), dt, dh, par)
+            s = B.stats_to_host(sbuf)
+            assert (s.n_passes, s.n_retry_pg, s.n_unphys_final, s.n_c2p_fail) == \
+                   (st.n_passes, st.n_retry_pg, st.n_unphys_final, st.n_c2p_fail), (seed, g)
+            if st.n_unphys_final == 0:
+                assert step_err(got.cpu().numpy(), w, 2).max() <= TOL_STEP, (seed, g, st.n_passes)
+        got, sbuf = B.fluid_step(dev(tiles), dt, dh, par)       # and the batch as one launch
+        s = B.stats_to_host(sbuf)
+        assert s.n_passes == sum(st.n_passes for _, st in per_group)
+        assert s.exec_c2p >= tiles.shape[0] * ((16 + 2 * po.ghost) ** 3)      # the executed-work counters are live
+        assert np.array_equal(np.isfinite(got.cpu().numpy()), np.isfinite(want))

@@ -248,13 +248,14 @@ def test_second_order_convergence_on_the_3d_diagonal_wave(ref, T0):
     assert o1 > 1.8 and o2 > 1.8, (e16, e32, e64, o1, o2)
 
 
-def test_one_step_matches_40_digit_evaluation_of_the_definitions(ref):
-    """A handful of cells of a small 3-D box, one PLM + MUSCL-Hancock + HLLC/HLLE step, against
+@pytest.mark.parametrize("recon", ["plm", "ppm"])
+def test_one_step_matches_40_digit_evaluation_of_the_definitions(ref, recon):
+    """A handful of cells of a small 3-D box, one PLM/PPM + MUSCL-Hancock + HLLC/HLLE step, against
     tests/mp_defs.step_cells: total-energy definitions, numerical root finding, textbook eigenvalues,
     plain subtractions in 40 digits, its own loops.  Pins the assembly (stencils, the coupling of the three
     directions in the predictor, face pairing, update) and the Etilde formulation at once."""
     rng = np.random.default_rng(4)
-    n, g = 3, 2
+    n, g = 3, ref.params(recon, "hllc").ghost
     s = n + 2 * g + 2                                 # one spare layer so the mp stencil stays inside
     k = 2 * np.pi * (np.arange(s) + 0.37) / 9.0
     Z, Y, X = np.meshgrid(k, 0.8 * k, 1.3 * k, indexing="ij")
@@ -269,12 +270,13 @@ def test_one_step_matches_40_digit_evaluation_of_the_definitions(ref):
     dt = 0.4 * dh / ref.max_signal_speed(big.reshape(5, -1))
     tile = np.ascontiguousarray(big[:, 1:-1, 1:-1, 1:-1])
     for riemann in ("hllc", "hlle"):
-        par = ref.params("plm", riemann)
+        par = ref.params(recon, riemann)
         out, st, passes = ref.step_box(tile, dt, dh, par)
         assert passes == 1
-        cells = [(0, 0, 0), (1, 2, 0), (2, 1, 2)]
+        cells = [(0, 0, 0), (1, 2, 0), (2, 1, 2)] if recon == "plm" else [(1, 2, 0)]
         off = g + 1                                   # interior cell (i,j,k) sits at big[..., k+off, j+off, i+off]
-        want = mp_defs.step_cells(big, [(i + off, j + off, k + off) for i, j, k in cells], dt, dh, riemann)
+        want = mp_defs.step_cells(big, [(i + off, j + off, k + off) for i, j, k in cells], dt, dh, riemann,
+                                  recon=recon)
         for (i, j, k) in cells:
             w = want[(i + off, j + off, k + off)]
             scale = [abs(w[0]), abs(w[4]) + float(np.sqrt(sum(float(x) ** 2 for x in w[1:4]))), abs(w[4])]
