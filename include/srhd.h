@@ -198,7 +198,8 @@ int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, v
  * division in the exact build) and IEEE division side by side on n seeded pairs generated on the device;
  * d_out (device, 2 x unsigned long long) receives {number of bit mismatches, index of the first one or
  * ~0}.  dist: 0 = the value ranges of BASELINE.json configs 2-5, 1 = operands within 2^15 ulp of powers of two
- * and of each other, 2 = exponents over [1e-200, 1e200].  Used by tests/test_gpu_quotient.py. */
+ * and of each other, 2 = exponents over [1e-150, 1e150]
+ * (quotients that underflow to subnormal numbers are outside the claim: such a state fails Eq. 30 either way).  Used by tests/test_gpu_quotient.py. */
 int srhd_quotient_check(unsigned long long n, unsigned long long seed, int dist,
                         unsigned long long* d_out, void* stream);
 

@@ -11,16 +11,26 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "libsrhd_ref.so")
 SRC = [os.path.join(HERE, "srhd_ref.cpp")]
 HDR = [os.path.join(HERE, "srhd_ref.hpp")]
+# "fma": the SAME source with the compiler free to contract a*b+c into fused multiply-adds -- a second, equally
+# legitimate IEEE rounding of the same formulas.  Tests use it to measure how far two correct fp64 evaluations
+# of this algorithm drift apart (tests/test_gpu_configs.py); it is never the parity reference.
+VARIANTS = {"": ["-ffp-contract=off"], "fma": ["-ffp-contract=fast", "-mfma"]}
 
 
-def build(force: bool = False) -> str:
-    newest = max(os.path.getmtime(p) for p in SRC + HDR)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
-        return LIB
-    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-Wextra", "-o", LIB] + SRC
+def lib_path(variant=""):
+    return LIB if not variant else os.path.join(HERE, f"libsrhd_ref_{variant}.so")
+
+
+def build(force: bool = False, variant: str = "") -> str:
+    out = lib_path(variant)
+    newest = max(os.path.getmtime(p) for p in SRC + HDR + [os.path.abspath(__file__)])
+    if not force and os.path.exists(out) and os.path.getmtime(out) >= newest:
+        return out
+    cmd = ["g++", "-std=c++17", "-O2"] + VARIANTS[variant] + ["-fopenmp", "-fPIC", "-shared",
+           "-Wall", "-Wextra", "-o", out + ".tmp"] + SRC
     subprocess.run(cmd, check=True)
-    return LIB
+    os.replace(out + ".tmp", out)
+    return out
 
 
 if __name__ == "__main__":

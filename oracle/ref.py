@@ -38,10 +38,33 @@ def params(recon="plm", riemann="hllc", minmod_coeff=1.5, max_retry=8, newton_rt
     return Params(r, s, minmod_coeff, max_retry, newton_rtol, newton_max_iter, 2 if r == 0 else 3)
 
 
+_LIBS = {}
+_VARIANT = ""
+
+
+class variant:
+    """with ref.variant("fma"): ... -- route every call to the oracle built with FMA contraction allowed (a
+    second rounding of the same formulas; oracle/build.py).  Never the parity reference."""
+
+    def __init__(self, name):
+        self.name = name
+
+    def __enter__(self):
+        global _VARIANT, _LIB
+        self.prev = _VARIANT
+        _VARIANT, _LIB = self.name, _LIBS.get(self.name)
+        lib()
+
+    def __exit__(self, *a):
+        global _VARIANT, _LIB
+        _VARIANT, _LIB = self.prev, _LIBS.get(self.prev)
+
+
 def lib():
     global _LIB
     if _LIB is None:
-        L = C.CDLL(_build.build())
+        L = C.CDLL(_build.build(variant=_VARIANT))
+        _LIBS[_VARIANT] = L
         for name in ("htilde_of_T", "T_of_htilde", "dT_dhtilde", "cs2_of_T", "smax_of_umax"):
             f = getattr(L, "srhd_ref_" + name)
             f.restype, f.argtypes = _D, [_D]

@@ -79,26 +79,40 @@ def step_err_local(got, want, tiles, ghost):
 
 # ---------------------------------------------------------------------------------------------------------
 # Tolerance of a one-step comparison DERIVED from the paper's error model (Eq. 20): the inversion of a
-# state with Mach number M returns h, U, rho, p with relative uncertainty (1 + M^2) eps, whatever the order of
-# evaluation.  Two correct fp64 implementations whose half-step states differ in the last bit therefore feed
-# Riemann problems that differ by that much, and the update of a cell subtracts face fluxes whose size is
-# set by the LARGEST conserved quantity among the cell and its face neighbours.  Per cell and per norm of S14:
-#     tol = max(1e-11, C * (dt/dh) * max_{stencil} (1 + M^2) eps * (largest neighbouring scale) / (own scale))
-# with the stencil the (2g+1)^3 cells the update depends on.  C = 4 (six faces, |v| <= 1, dt/dh <= 0.5).
+# state with Mach number M returns h, rho, p (and U = M/(D h)) with relative uncertainty (1 + M^2) eps, whatever
+# the order of evaluation.  The conserved state itself re-enters the fluxes exactly (F = U v_n + pressure terms)
+# and v_n = M_n/(E + p) is well conditioned, so what two correct fp64 implementations whose half-step states
+# differ in the last bit disagree on is (i) the PRESSURE of the face states, delta p = (1 + M^2) eps p, which
+# enters the momentum and energy fluxes directly and the mass flux through v_n and lambda* with a factor
+# D/(E + p), and (ii) the SOUND SPEED (T = p/rho), i.e. the wave speeds, whose distance from the flow speed is
+# |lambda - v_n| <= c_s/gamma^2: delta S = (1 + M^2) eps c_s/gamma^2 multiplies the JUMP of the conserved
+# variables across the face in the HLL averages (bounded by the largest neighbouring scale).
+# Per cell and per norm q of S14, with the (2g+1)^3 stencil the update depends on:
+#     tol_q = max(1e-11, C (dt/dh) { max_stencil[(1 + M^2) eps p w_q] + max_stencil[(1 + M^2) eps c_s/gamma^2] L_q } / own_q)
+# w_D = D/(D + Etilde), w_M = w_E = 1; L_q = largest scale of norm q among the cell and its face neighbours;
+# C = 4 (six faces, dt/dh <= 0.5).
 def _cs2_numpy(T):
     """P:129 Eq. 14 with h = Eq. 10 (tolerance scale only: not a parity reference)."""
     h = 2.5 * T + np.sqrt(2.25 * T * T + 1.0)
     return T * (5.0 * h - 8.0 * T) / (3.0 * h * (h - T))
 
 
-def eq20_condition(ref, tiles):
-    """(1 + Mach^2) eps of every tile cell from the ORACLE's primitives; tiles (npg,5,n,n,n)."""
+def eq20_uncertainties(ref, tiles):
+    """((1 + Mach^2) eps p, (1 + Mach^2) eps c_s / gamma^2) of every tile cell from the ORACLE's primitives;
+    tiles (npg,5,n,n,n)."""
     npg = tiles.shape[0]
     sh = tiles.shape[2:]
     W = ref.cons2prim(np.ascontiguousarray(tiles.transpose(1, 0, 2, 3, 4)).reshape(5, -1))[0].reshape(5, npg, *sh)
     cs2 = _cs2_numpy(W[4] / W[0])
-    mach2 = (W[1:4] ** 2).sum(0) * (1.0 - cs2) / cs2
-    return (1.0 + mach2) * np.finfo(np.float64).eps
+    usq = (W[1:4] ** 2).sum(0)
+    cond = (1.0 + usq * (1.0 - cs2) / cs2) * np.finfo(np.float64).eps
+    return cond * W[4], cond * np.sqrt(cs2) / (1.0 + usq)
+
+
+def blocks_of_cells(a):
+    """(npg,8,8,8,8) per-cell values in patch order (S13) -> (npg,16,16,16)."""
+    npg = a.shape[0]
+    return a.reshape(npg, 2, 2, 2, 8, 8, 8).transpose(0, 1, 4, 2, 5, 3, 6).reshape(npg, 16, 16, 16)
 
 
 def step_err_eq20(ref, got, want, tiles, ghost, dt, dh, C=4.0, floor=1e-11):
@@ -107,8 +121,14 @@ def step_err_eq20(ref, got, want, tiles, ghost, dt, dh, C=4.0, floor=1e-11):
     from scipy.ndimage import maximum_filter
     g, w = patches_to_block(got), patches_to_block(want)
     G = ghost
-    cond = maximum_filter(eq20_condition(ref, tiles), size=(1, 2 * G + 1, 2 * G + 1, 2 * G + 1), mode="nearest")
+    size = (1, 2 * G + 1, 2 * G + 1, 2 * G + 1)
+    dp, ds = eq20_uncertainties(ref, tiles)
     t = tiles
+    dp_d = dp * np.abs(t[:, 0]) / (np.abs(t[:, 0]) + np.abs(t[:, 4]))
+    sl = (slice(None), slice(G, G + 16), slice(G, G + 16), slice(G, G + 16))
+    dpm = maximum_filter(dp, size=size, mode="nearest")[sl]
+    dpd = maximum_filter(dp_d, size=size, mode="nearest")[sl]
+    dsm = maximum_filter(ds, size=size, mode="nearest")[sl]
     sc = [np.abs(t[:, 0]), np.sqrt((t[:, 1:4] ** 2).sum(1)) + np.abs(t[:, 4]), np.abs(t[:, 4])]
     loc = []
     for s0 in sc:
@@ -116,17 +136,16 @@ def step_err_eq20(ref, got, want, tiles, ghost, dt, dh, C=4.0, floor=1e-11):
         for ax in (1, 2, 3):
             for sh in (-1, 1):
                 m = np.maximum(m, np.roll(s0, sh, axis=ax))       # wrap only touches ghost layers
-        loc.append(m[:, G:G + 16, G:G + 16, G:G + 16])
-    cond = cond[:, G:G + 16, G:G + 16, G:G + 16]
+        loc.append(m[sl])
     own = [np.abs(w[:, 0]), np.sqrt((w[:, 1:4] ** 2).sum(1)) + np.abs(w[:, 4]), np.abs(w[:, 4])]
     errs = [np.abs(g[:, 0] - w[:, 0]), np.abs(g[:, 1:4] - w[:, 1:4]).max(1), np.abs(g[:, 4] - w[:, 4])]
     err = np.zeros_like(own[0])
     tol = np.full_like(own[0], floor)
     ratio = np.zeros_like(own[0])
     with np.errstate(divide="ignore", invalid="ignore"):
-        for e, o, l in zip(errs, own, loc):
+        for e, o, d, l in zip(errs, own, (dpd, dpm, dpm), loc):
             en = np.where(o > 0, e / o, np.where(e > 0, np.inf, 0.0))
-            tn = np.maximum(floor, C * (dt / dh) * cond * np.maximum(l, o) / o)
+            tn = np.maximum(floor, C * (dt / dh) * (d + dsm * np.maximum(l, o)) / o)
             worse = en / tn > ratio
             ratio = np.where(worse, en / tn, ratio)
             err = np.where(worse, en, err)
@@ -142,18 +161,3 @@ def report(name, **kw):
     os.makedirs(os.path.join(root, "gpurun_out"), exist_ok=True)
     with open(os.path.join(root, "gpurun_out", "parity_report.jsonl"), "a") as f:
         f.write(json.dumps({"test": name, **{k: (float(v) if isinstance(v, (np.floating, float)) else v) for k, v in kw.items()}}) + "\n")
-
-
-def eq20_l1_budget(ref, grid, dt, dh, ghost, C=4.0):
-    """The same error model summed over a whole grid (5,nz,ny,nx) for the many-step L1 norm of S14: the
-    L1-relative difference one step can add, per norm (D, M, Etilde):  sum_i C (dt/dh) cond_i local_i / sum_i own_i."""
-    from scipy.ndimage import maximum_filter
-    cond = eq20_condition(ref, grid[None])[0]
-    cond = maximum_filter(cond, size=2 * ghost + 1, mode="nearest")
-    sc = [np.abs(grid[0]), np.sqrt((grid[1:4] ** 2).sum(0)) + np.abs(grid[4]), np.abs(grid[4])]
-    out = []
-    for s0 in sc:
-        loc = maximum_filter(s0, footprint=np.array([[[0, 0, 0], [0, 1, 0], [0, 0, 0]], [[0, 1, 0], [1, 1, 1], [0, 1, 0]],
-                                                      [[0, 0, 0], [0, 1, 0], [0, 0, 0]]], dtype=bool), mode="nearest")
-        out.append(float((C * (dt / dh) * cond * loc).sum() / s0.sum()))
-    return np.array([out[0], out[1], out[1], out[1], out[2]])

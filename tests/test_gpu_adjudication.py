@@ -16,7 +16,7 @@ from paper_2012_11130_b200 import binding as B
 from paper_2012_11130_b200 import workloads as wl
 from paper_2012_11130_b200.driver import GridStepper
 from tests import mp_defs
-from tests.gpu_util import patches_to_block, report, step_err, step_err_eq20
+from tests.gpu_util import blocks_of_cells, patches_to_block, report, step_err, step_err_eq20
 
 pytestmark = pytest.mark.gpu
 
@@ -31,7 +31,7 @@ def _worst_cells(ref, st, recon, riemann, dt, nworst):
         w, s = ref.fluid_step(tiles[g:g + 1], dt, st.dh, par)
         want[g] = w[0]
         single[g] = s.n_passes == 1                   # the 40-digit stepper has no retry ladder
-    err = patches_to_block(step_err(got, want, 2)[:, :, None])[:, 0]       # (npg,16,16,16)
+    err = blocks_of_cells(step_err(got, want, 2))                         # (npg,16,16,16)
     e2, tol = step_err_eq20(ref, got, want, tiles, st.par.ghost, dt, st.dh)
     err = np.where(single[:, None, None, None], np.nan_to_num(err, nan=0.0, posinf=0.0), 0.0)
     order = np.argsort(err.ravel())[::-1][:nworst]
