@@ -84,11 +84,12 @@ def step_err_local(got, want, tiles, ghost):
 # and v_n = M_n/(E + p) is well conditioned, so what two correct fp64 implementations whose half-step states
 # differ in the last bit disagree on is (i) the PRESSURE of the face states, delta p = (1 + M^2) eps p, which
 # enters the momentum and energy fluxes directly and the mass flux through v_n and lambda* with a factor
-# D/(E + p), and (ii) the SOUND SPEED (T = p/rho), i.e. the wave speeds, whose distance from the flow speed is
-# |lambda - v_n| <= c_s/gamma^2: delta S = (1 + M^2) eps c_s/gamma^2 multiplies the JUMP of the conserved
-# variables across the face in the HLL averages (bounded by the largest neighbouring scale).
+# D/(E + p), and (ii) the SOUND SPEED (T = p/rho), i.e. the wave speeds: in the two-wave averages the weights
+# (v_L - S_L)/(S_R - S_L) and (S_R - v_R)/(S_R - S_L) are ratios of sound-speed-sized numbers, uncertain by
+# (1 + M^2) eps RELATIVELY, and they multiply S U with |S| <~ c_s wherever the averages are used at all
+# (a supersonic face takes the upwind flux): delta F ~ (1 + M^2) eps c_s times the largest neighbouring scale.
 # Per cell and per norm q of S14, with the (2g+1)^3 stencil the update depends on:
-#     tol_q = max(1e-11, C (dt/dh) { max_stencil[(1 + M^2) eps p w_q] + max_stencil[(1 + M^2) eps c_s/gamma^2] L_q } / own_q)
+#     tol_q = max(1e-11, C (dt/dh) { max_stencil[(1 + M^2) eps p w_q] + max_stencil[(1 + M^2) eps c_s] L_q } / own_q)
 # w_D = D/(D + Etilde), w_M = w_E = 1; L_q = largest scale of norm q among the cell and its face neighbours;
 # C = 4 (six faces, dt/dh <= 0.5).
 def _cs2_numpy(T):
@@ -98,7 +99,7 @@ def _cs2_numpy(T):
 
 
 def eq20_uncertainties(ref, tiles):
-    """((1 + Mach^2) eps p, (1 + Mach^2) eps c_s / gamma^2) of every tile cell from the ORACLE's primitives;
+    """((1 + Mach^2) eps p, (1 + Mach^2) eps c_s) of every tile cell from the ORACLE's primitives;
     tiles (npg,5,n,n,n)."""
     npg = tiles.shape[0]
     sh = tiles.shape[2:]
@@ -106,7 +107,7 @@ def eq20_uncertainties(ref, tiles):
     cs2 = _cs2_numpy(W[4] / W[0])
     usq = (W[1:4] ** 2).sum(0)
     cond = (1.0 + usq * (1.0 - cs2) / cs2) * np.finfo(np.float64).eps
-    return cond * W[4], cond * np.sqrt(cs2) / (1.0 + usq)
+    return cond * W[4], cond * np.sqrt(cs2)
 
 
 def blocks_of_cells(a):
