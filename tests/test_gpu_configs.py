@@ -132,7 +132,7 @@ def _oracle_tiles_from_prim(ref, prim, bc, ghost, idx, inflow=None):
     return out
 
 
-frac_bad = []      # per compared step: fraction of cells above TOL_STEP (filled by _sampled_full_size)
+frac_bad = []      # per compared step: fraction of cells above TOL_STEP in the plain per-cell S14 norm
 
 
 def _sampled_full_size(ref, st, recon, riemann, nsteps, nsample, seed, always=(), prim0=None, inflow0=None, tag=""):
@@ -187,7 +187,7 @@ def _sampled_full_size(ref, st, recon, riemann, nsteps, nsample, seed, always=()
                worst_local_scale_norm=local.max(), retried_groups=int(ost.n_retry_pg))
         assert (err <= tol).all(), (tag, n, float((err / tol).max()))
         worst = max(worst, float((err / tol).max()))
-        frac_bad.append(float((tol > TOL_STEP).mean()))
+        frac_bad.append(float((blocks_of_cells(plain) > TOL_STEP).mean()))
         checked += len(idx)
         ladder += int(ost.n_retry_pg)
     return worst, checked, ladder
@@ -200,7 +200,7 @@ def test_config2_blast_full_size_sampled(ref):
     worst, checked, ladder = _sampled_full_size(ref, st, "ppm", "hllc", nsteps=12, nsample=96, seed=1, always=centre,
                                                 prim0=prim, tag="blast256")
     assert checked >= 250 and worst <= 1.0, (worst, checked, ladder)
-    assert max(frac_bad) <= 1e-2, frac_bad      # the tolerance IS the north-star 1e-11 on all but 1 % of the cells
+    assert max(frac_bad) == 0.0, frac_bad       # and EVERY sampled cell meets the north-star 1e-11 per cell (S14)
 
 
 def test_config3_random_field_full_size_sampled(ref):
@@ -212,10 +212,11 @@ def test_config3_random_field_full_size_sampled(ref):
     assert ladder > 0          # this workload does exercise the retry ladder
     # Cold, fast cells of this field reach Mach ~1e7: by the paper's own error model (Eq. 20) the inversion of
     # a half-step state carries (1 + Mach^2) eps, which no evaluation order avoids (the exact build above IS
-    # bit-identical).  Every cell is held to the tolerance derived from that model; it is the north-star
-    # 1e-11 on all but a small fraction of the cells, which the report records.
+    # bit-identical).  Every cell is held to the tolerance derived from that model (gpu_util.step_err_eq20);
+    # measured: the first step from the raw random field leaves 0.36 % of the cells above the north-star
+    # 1e-11 (worst 6e-10), every later step none.
     assert checked >= 250 and worst <= 1.0, (worst, checked, ladder)
-    assert max(frac_bad) <= 0.05, frac_bad
+    assert frac_bad[0] <= 1e-2 and max(frac_bad[1:]) == 0.0, frac_bad
 
 
 def test_config4_jet_full_size_sampled(ref):
@@ -227,7 +228,7 @@ def test_config4_jet_full_size_sampled(ref):
                                                 prim0=prim, inflow0=inflow, tag="jet")
     del prim
     assert checked >= 250 and worst <= 1.0, (worst, checked, ladder)
-    assert max(frac_bad) <= 1e-2, frac_bad
+    assert max(frac_bad) == 0.0, frac_bad       # and EVERY sampled cell meets the north-star 1e-11 per cell (S14)
     assert float(st.grid[3].abs().max()) > 0            # the jet entered the box
 
 
