@@ -19,7 +19,7 @@ class Params(C.Structure):
     """srhd_ref_params; defaults are the readings S2/S3/S9 of DESIGN.md."""
     _fields_ = [("recon", C.c_int), ("riemann", C.c_int), ("minmod_coeff", C.c_double),
                 ("max_retry", C.c_int), ("newton_rtol", C.c_double), ("newton_max_iter", C.c_int),
-                ("ghost", C.c_int)]
+                ("ghost", C.c_int), ("integrator", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -32,10 +32,11 @@ class Stats(C.Structure):
 
 
 def params(recon="plm", riemann="hllc", minmod_coeff=1.5, max_retry=8, newton_rtol=1e-15,
-           newton_max_iter=20):
+           newton_max_iter=20, integrator="mhm"):
     r = {"plm": 0, "ppm": 1}[recon] if isinstance(recon, str) else int(recon)
     s = {"hlle": 0, "hllc": 1}[riemann] if isinstance(riemann, str) else int(riemann)
-    return Params(r, s, minmod_coeff, max_retry, newton_rtol, newton_max_iter, 2 if r == 0 else 3)
+    v = {"mhm": 0, "vl": 1}[integrator] if isinstance(integrator, str) else int(integrator)
+    return Params(r, s, minmod_coeff, max_retry, newton_rtol, newton_max_iter, (2 if r == 0 else 3) + v, v)
 
 
 _LIBS = {}

@@ -506,6 +506,168 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
   return pass + 1;
 }
 
+// ---------------------------------------------------------------- VL integrator (reading S18) ------
+// "VL (Falle 1991; van Leer 2006)": van Leer's predictor-corrector.  For one box, pass k of the same retry
+// ladder as above (the coefficient only enters the reconstruction of stage V4):
+//   V1  W = C2P(U) for every tile cell                                                        (as O5a)
+//   V2  first-order fluxes F1 at every face between cells c and c+n with all indices in -(g-1)..n+g-2:
+//       the Riemann solver on the CELL-CENTRE states (piecewise constant)
+//   V3  predictor: Uh = U - dt/(2 dh) ((F1x+ - F1x-) + (F1y+ - F1y-)) + (F1z+ - F1z-)) for those cells;
+//       Wh = C2P(Uh)  (an Eq. 30 violation fails the pass, S15)
+//   V4  PLM / PPM edge values of Wh (coefficient beta_k), UL/UR = P2C of the edge primitives
+//   V5  second-order fluxes F2 = Riemann(edge states) at every face touching an interior cell
+//   V6  Unew = U - dt/dh ((F2x+ - F2x-) + (F2y+ - F2y-)) + (F2z+ - F2z-));  Eq. 30 check, retry (S9, S10)
+// Stages V1-V3 do not depend on the pass.  Ghost width: one more than MUSCL-Hancock (PLM 3, PPM 4).
+int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt, double dh,
+                const srhd_ref_params& par, srhd_ref_stats& st, double* flux_keep = nullptr) {
+  const int g = par.ghost;
+  Box b{nx, ny, nz, g, nx + 2 * g, ny + 2 * g, nz + 2 * g, 0};
+  b.cstride = (size_t)b.sx * b.sy * b.sz;
+  const size_t np = b.cstride;
+  const int stp[3] = {1, b.sx, b.sx * b.sy};
+  const int ext[3] = {nx, ny, nz};
+  // V1
+  std::vector<double> Wc(5 * np);
+  double umax = 0.0;
+  for (int k = -g; k < nz + g; ++k)
+    for (int j = -g; j < ny + g; ++j)
+      for (int i = -g; i < nx + g; ++i) {
+        const size_t c = b.at(i, j, k);
+        double U[5], W[5];
+        for (int q = 0; q < 5; ++q) U[q] = cons_in[q * np + c];
+        int it = 0;
+        const bool phys = cons2prim(U, W, par.newton_rtol, par.newton_max_iter, &it, nullptr);
+        st.newton_iters += (unsigned long long)it;
+        for (int q = 0; q < 5; ++q) Wc[q * np + c] = W[q];
+        const bool interior = i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz;
+        if (interior) {
+          if (!phys) ++st.n_c2p_fail;
+          umax = std::max(umax, umax_of_prim(W));
+        }
+      }
+  st.max_speed = std::max(st.max_speed, smax_of_umax(umax));
+  // V2: first-order fluxes; F1[(d*5+q)*np + c] = flux through the face between c and c + n_d
+  const int lo = -(g - 1), hx = nx + g - 2, hy = ny + g - 2, hz = nz + g - 2;   // cells that get a predictor
+  std::vector<double> F1(3 * 5 * np, 0.0);
+  for (int d = 0; d < 3; ++d)
+    for (int k = lo - (d == 2); k <= hz; ++k)
+      for (int j = lo - (d == 1); j <= hy; ++j)
+        for (int i = lo - (d == 0); i <= hx; ++i) {
+          const size_t c = b.at(i, j, k), cr = c + stp[d];
+          double UL[5], UR[5], WL[5], WR[5], F[5];
+          for (int q = 0; q < 5; ++q) {
+            UL[q] = cons_in[q * np + c];
+            UR[q] = cons_in[q * np + cr];
+            WL[q] = Wc[q * np + c];
+            WR[q] = Wc[q * np + cr];
+          }
+          riemann_flux(par.riemann, d, WL, UL, WR, UR, F);
+          for (int q = 0; q < 5; ++q) F1[(d * 5 + q) * np + c] = F[q];
+        }
+  // V3: predictor and its primitives
+  std::vector<double> Wh(5 * np, 0.0);
+  unsigned long long half_fail = 0, half_iters = 0;
+  const double hdt = dt / (2.0 * dh);
+  for (int k = lo; k <= hz; ++k)
+    for (int j = lo; j <= hy; ++j)
+      for (int i = lo; i <= hx; ++i) {
+        const size_t c = b.at(i, j, k);
+        double Uh[5], W[5];
+        for (int q = 0; q < 5; ++q) {
+          const double dfx = F1[(0 * 5 + q) * np + c] - F1[(0 * 5 + q) * np + c - stp[0]];
+          const double dfy = F1[(1 * 5 + q) * np + c] - F1[(1 * 5 + q) * np + c - stp[1]];
+          const double dfz = F1[(2 * 5 + q) * np + c] - F1[(2 * 5 + q) * np + c - stp[2]];
+          Uh[q] = cons_in[q * np + c] - hdt * ((dfx + dfy) + dfz);
+        }
+        int it = 0;
+        if (!cons2prim(Uh, W, par.newton_rtol, par.newton_max_iter, &it, nullptr)) ++half_fail;   // S15
+        half_iters += (unsigned long long)it;
+        for (int q = 0; q < 5; ++q) Wh[q * np + c] = W[q];
+      }
+  st.newton_iters += half_iters;
+  std::vector<double> Um(3 * 5 * np), Up(3 * 5 * np), Wm(3 * 5 * np), Wp(3 * 5 * np);
+  std::vector<double> Flux(3 * 5 * np);
+  const int K = par.max_retry;
+  double beta = par.minmod_coeff;
+  unsigned long long cell_fail = 0;
+  int pass = 0;
+  for (;; ++pass) {
+    if (pass > 0) beta = (pass <= K) ? beta * 0.75 : 0.0;     // P:273, reading S9
+    cell_fail = 0;
+    // V4: edge states of the cells that are face-adjacent to the interior
+    for (int k = -1; k <= nz; ++k)
+      for (int j = -1; j <= ny; ++j)
+        for (int i = -1; i <= nx; ++i) {
+          const int nout = (i < 0 || i >= nx) + (j < 0 || j >= ny) + (k < 0 || k >= nz);
+          if (nout > 1) continue;
+          const size_t c = b.at(i, j, k);
+          for (int d = 0; d < 3; ++d) {
+            double wm[5], wp[5], um[5], up[5];
+            for (int q = 0; q < 5; ++q) {
+              double a[5];
+              for (int m = -2; m <= 2; ++m)
+                a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0 : Wh[q * np + c + (ptrdiff_t)m * stp[d]];
+              recon_1d(par.recon, a, beta, par.minmod_coeff, wm[q], wp[q]);
+            }
+            prim2cons(wm, um);
+            prim2cons(wp, up);
+            for (int q = 0; q < 5; ++q) {
+              Wm[(d * 5 + q) * np + c] = wm[q];
+              Wp[(d * 5 + q) * np + c] = wp[q];
+              Um[(d * 5 + q) * np + c] = um[q];
+              Up[(d * 5 + q) * np + c] = up[q];
+            }
+          }
+        }
+    // V5
+    for (int d = 0; d < 3; ++d) {
+      int l3[3] = {0, 0, 0}, h3[3] = {nx - 1, ny - 1, nz - 1};
+      l3[d] = -1;
+      for (int k = l3[2]; k <= h3[2]; ++k)
+        for (int j = l3[1]; j <= h3[1]; ++j)
+          for (int i = l3[0]; i <= h3[0]; ++i) {
+            const size_t c = b.at(i, j, k), cr = c + stp[d];
+            double UL[5], UR[5], WL[5], WR[5], F[5];
+            for (int q = 0; q < 5; ++q) {
+              UL[q] = Up[(d * 5 + q) * np + c];
+              WL[q] = Wp[(d * 5 + q) * np + c];
+              UR[q] = Um[(d * 5 + q) * np + cr];
+              WR[q] = Wm[(d * 5 + q) * np + cr];
+            }
+            riemann_flux(par.riemann, d, WL, UL, WR, UR, F);
+            for (int q = 0; q < 5; ++q) Flux[(d * 5 + q) * np + c] = F[q];
+          }
+    }
+    // V6
+    const double dtdh = dt / dh;
+    const size_t no = (size_t)nx * ny * nz;
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          const size_t c = b.at(i, j, k);
+          double Un[5];
+          for (int q = 0; q < 5; ++q) {
+            const double dfx = Flux[(0 * 5 + q) * np + c] - Flux[(0 * 5 + q) * np + c - stp[0]];
+            const double dfy = Flux[(1 * 5 + q) * np + c] - Flux[(1 * 5 + q) * np + c - stp[1]];
+            const double dfz = Flux[(2 * 5 + q) * np + c] - Flux[(2 * 5 + q) * np + c - stp[2]];
+            Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);
+            cons_out[q * no + ((size_t)k * ny + j) * nx + i] = Un[q];
+          }
+          if (!is_physical(Un)) ++cell_fail;
+        }
+    (void)ext;
+    // the predictor does not depend on beta: if IT failed, no rung can cure it -- go straight to the last
+    // rung's verdict (accept and count), like a face failure in the beta = 0 pass of MUSCL-Hancock (S15)
+    if (cell_fail == 0 || beta == 0.0) break;
+  }
+  if (flux_keep) std::copy(Flux.begin(), Flux.end(), flux_keep);
+  if (pass > 0) ++st.n_retry_pg;
+  st.n_passes += (unsigned long long)(pass + 1);
+  st.n_c2p_fail += half_fail;
+  st.n_unphys_final += cell_fail;
+  return pass + 1;
+}
+
 // index of the source cell for ghost index i under a boundary type (reading S11)
 inline int map_index(int i, int n, int bc_lo, int bc_hi) {
   if (i < 0) return (bc_lo == 0) ? ((i % n) + n) % n : 0;
@@ -615,7 +777,7 @@ int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, i
                       double dh, const srhd_ref_params* par, srhd_ref_stats* stats) {
   srhd_ref_stats st;
   std::memset(&st, 0, sizeof(st));
-  const int passes = step_box(cons_in, cons_out, nx, ny, nz, dt, dh, *par, st);
+  const int passes = (par->integrator == 1 ? step_box_vl : step_box)(cons_in, cons_out, nx, ny, nz, dt, dh, *par, st, nullptr);
   if (stats) *stats = st;
   return passes;
 }
@@ -649,7 +811,8 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
     std::memset(&st, 0, sizeof(st));
     std::vector<double> box((size_t)5 * 4096);
     std::vector<double> fl(flux_out ? (size_t)3 * in_pg : 0);
-    step_box(cons_in + pg * in_pg, box.data(), 16, 16, 16, dt, dh, *par, st, flux_out ? fl.data() : nullptr);
+    (par->integrator == 1 ? step_box_vl : step_box)(cons_in + pg * in_pg, box.data(), 16, 16, 16, dt, dh, *par, st,
+                                                    flux_out ? fl.data() : nullptr);
     if (flux_out) {
       const int g = par->ghost;
       const size_t np = (size_t)nxt * nxt * nxt;

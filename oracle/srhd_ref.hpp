@@ -29,7 +29,8 @@ struct srhd_ref_params {
   int    max_retry;        // K reductions by 0.75, then beta = 0    (K: reading S9)
   double newton_rtol;      // stop when |delta| <= rtol*|htilde|     (reading S2)
   int    newton_max_iter;  // iteration cap                          (reading S2)
-  int    ghost;            // 2 (PLM) or 3 (PPM)
+  int    ghost;            // MUSCL-Hancock: 2 (PLM) or 3 (PPM); VL: one more
+  int    integrator;       // 0 MUSCL-Hancock (Toro 2011), 1 VL (Falle 1991; van Leer 2006)   (reading S18)
 };
 
 struct srhd_ref_stats {

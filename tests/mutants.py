@@ -15,7 +15,7 @@ import tempfile
 from concurrent.futures import ThreadPoolExecutor
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-PINS = "tests/test_oracle_pins_r2.py"
+PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_vl.py"]
 
 # (name, cited passage, old text, new text, pytest node ids / -k expression that must fail)
 MUTANTS = [
@@ -67,6 +67,13 @@ MUTANTS = [
      "if ((face_fail == 0 && cell_fail == 0) || beta == 0.0) break;",
      "if ((cell_fail == 0) || beta == 0.0) break;",
      "test_retry_ladder_equals"),
+    ("VL: predictor advanced by a full step", "P:225, reading S18",
+     "Uh[q] = cons_in[q * np + c] - hdt * ((dfx + dfy) + dfz);", "Uh[q] = cons_in[q * np + c] - 2.0 * hdt * ((dfx + dfy) + dfz);",
+     "test_vl_second_order or test_vl_equals"),
+    ("VL: corrector reconstructs the OLD primitives (predictor ignored)", "P:225, reading S18",
+     "a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0 : Wh[q * np + c + (ptrdiff_t)m * stp[d]];",
+     "a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0 : Wc[q * np + c + (ptrdiff_t)m * stp[d]];",
+     "test_vl_second_order"),
     ("update: flux difference with the wrong sign in z", "Eq. 4a, reading S12",
      "Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);",
      "Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) - dfz);",
@@ -86,7 +93,7 @@ def run_mutant(m):
         with open(os.path.join(tmp, "oracle", "srhd_ref.cpp"), "w") as f:
             f.write(src.replace(old, new))
         env = dict(os.environ, SRHD_TEST_ORACLE_ROOT=tmp, SRHD_TEST_SKIP_CUDA_BUILD="1", OMP_NUM_THREADS="2")
-        r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider", PINS, "-k", kexpr],
+        r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider"] + PINS + ["-k", kexpr],
                            cwd=ROOT, env=env, capture_output=True, text=True, timeout=600)
         tail = (r.stdout.strip().splitlines() or [""])[-1]
         if r.returncode == 1:
