@@ -44,6 +44,8 @@ extern "C" {
 #define SRHD_RECON_PPM   1
 #define SRHD_RIEMANN_HLLE 0
 #define SRHD_RIEMANN_HLLC 1
+#define SRHD_INTEGRATOR_MHM 0   /* MUSCL-Hancock (Toro 2011), the fused hot path                 */
+#define SRHD_INTEGRATOR_VL  1   /* VL: van Leer predictor-corrector (Falle 1991; van Leer 2006; S18) */
 
 #define SRHD_REFINE_NONE   0   /* no gradient criterion */
 #define SRHD_REFINE_D      1   /* Q = D        (conserved: no root finding)            */
@@ -63,7 +65,8 @@ typedef struct {
   int    max_retry;        /* K reductions of beta by 0.75, then beta = 0; default 8 (S9)     */
   double newton_rtol;      /* Newton-Raphson stop: |delta| <= rtol*|htilde|; default 1e-15 (S2)       */
   int    newton_max_iter;  /* iteration cap; default 20 (S2)                                          */
-  int    ghost;            /* ghost width of cons_in: must be 2 for PLM, 3 for PPM                    */
+  int    ghost;            /* ghost width of cons_in: MUSCL-Hancock 2 (PLM) / 3 (PPM); VL one more    */
+  int    integrator;       /* SRHD_INTEGRATOR_MHM (default) or SRHD_INTEGRATOR_VL             */
 } srhd_params;
 
 /* Per-call counters, DEVICE resident, zeroed by the callee at call start (on the stream). */
@@ -156,7 +159,9 @@ int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_ou
 int srhd_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
                       const srhd_params* params, unsigned char* flags, void* stream);
 
-/* Bytes of caller-provided scratch srhd_fluid_step needs: 0, the step is fully fused. */
+/* Bytes of scratch a srhd_fluid_step call uses: 0 for MUSCL-Hancock (fully fused); for the VL integrator
+ * the two primitive tiles its stages communicate through, which the call allocates and frees itself in
+ * stream order (cudaMallocAsync / cudaFreeAsync on `stream`): informational, nothing for the caller to provide. */
 size_t srhd_workspace_bytes(int npg, const srhd_params* params);
 
 /* Harness helpers for a uniform grid (reading S11, S13; NOT part of the paper's solver: they stand in

@@ -17,6 +17,7 @@ _VP = C.c_void_p
 
 RECON = {"plm": 0, "ppm": 1}
 RIEMANN = {"hlle": 0, "hllc": 1}
+INTEGRATOR = {"mhm": 0, "vl": 1}
 BC = {"periodic": 0, "outflow": 1}
 
 
@@ -24,7 +25,7 @@ class Params(C.Structure):
     """srhd_params (include/srhd.h)."""
     _fields_ = [("recon", C.c_int), ("riemann", C.c_int), ("minmod_coeff", C.c_double),
                 ("max_retry", C.c_int), ("newton_rtol", C.c_double), ("newton_max_iter", C.c_int),
-                ("ghost", C.c_int)]
+                ("ghost", C.c_int), ("integrator", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -103,7 +104,7 @@ def load_library(exact=False):
 
 
 def params(recon="plm", riemann="hllc", minmod_coeff=None, max_retry=None, newton_rtol=None,
-           newton_max_iter=None, exact=False):
+           newton_max_iter=None, exact=False, integrator="mhm"):
     """srhd_default_params + overrides."""
     p = Params()
     r = RECON[recon] if isinstance(recon, str) else int(recon)
@@ -117,6 +118,9 @@ def params(recon="plm", riemann="hllc", minmod_coeff=None, max_retry=None, newto
         p.newton_rtol = newton_rtol
     if newton_max_iter is not None:
         p.newton_max_iter = newton_max_iter
+    v = INTEGRATOR[integrator] if isinstance(integrator, str) else int(integrator)
+    p.integrator = v                    # the VL integrator needs one more layer of ghost zones (include/srhd.h)
+    p.ghost += v
     return p
 
 

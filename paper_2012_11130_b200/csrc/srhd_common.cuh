@@ -16,7 +16,8 @@ inline int check_params(const srhd_params* p) {
   if (!p) return SRHD_ERR_NULL_POINTER;
   if (p->recon != SRHD_RECON_PLM && p->recon != SRHD_RECON_PPM) return SRHD_ERR_BAD_PARAMS;
   if (p->riemann != SRHD_RIEMANN_HLLE && p->riemann != SRHD_RIEMANN_HLLC) return SRHD_ERR_BAD_PARAMS;
-  if (p->ghost != (p->recon == SRHD_RECON_PLM ? 2 : 3)) return SRHD_ERR_BAD_PARAMS;
+  if (p->integrator != SRHD_INTEGRATOR_MHM && p->integrator != SRHD_INTEGRATOR_VL) return SRHD_ERR_BAD_PARAMS;
+  if (p->ghost != (p->recon == SRHD_RECON_PLM ? 2 : 3) + p->integrator) return SRHD_ERR_BAD_PARAMS;
   if (!(p->minmod_coeff >= 0.0) || !(p->minmod_coeff <= 2.0)) return SRHD_ERR_BAD_PARAMS;
   if (p->max_retry < 0 || p->max_retry > 64) return SRHD_ERR_BAD_PARAMS;
   if (!(p->newton_rtol >= 0.0) || p->newton_max_iter < 1) return SRHD_ERR_BAD_PARAMS;

@@ -591,9 +591,19 @@ int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int 
 
 }  // namespace srhd
 
+namespace srhd {   // srhd_vl.cu
+int vl_step(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
+            const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
+            double min_speed);
+size_t vl_workspace_bytes(int npg, const srhd_params* p);
+}  // namespace srhd
+
 using namespace srhd;
 
-extern "C" size_t srhd_workspace_bytes(int, const srhd_params*) { return 0; }
+extern "C" size_t srhd_workspace_bytes(int npg, const srhd_params* params) {
+  if (check_params(params) != SRHD_OK || params->integrator == SRHD_INTEGRATOR_MHM) return 0;
+  return vl_workspace_bytes(npg, params);
+}
 
 static int fluid_step_impl(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt,
                            double dh, const srhd_params* params, srhd_stats* stats, void* stream,
@@ -616,6 +626,8 @@ static int fluid_step_impl(const double* cons_in, double* cons_out, double* flux
     if (e != cudaSuccess) return (int)e;
   }
   if (npg == 0) return SRHD_OK;
+  if (params->integrator == SRHD_INTEGRATOR_VL)
+    return vl_step(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed);
   if (params->recon == SRHD_RECON_PLM) {
     return params->riemann == SRHD_RIEMANN_HLLE
                ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed)

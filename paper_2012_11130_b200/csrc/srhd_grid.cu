@@ -12,7 +12,7 @@ struct GridBC {
 };
 
 // source index of ghost index i along an axis of n cells (S11): periodic wraps, outflow clamps.
-// |ghost offset| <= 3 < 16 <= n, so one conditional add replaces the modulo.
+// |ghost offset| <= 4 < 16 <= n, so one conditional add replaces the modulo.
 SRHD_DEV int map_index(int i, int n, int bc_lo, int bc_hi) {
   if (i < 0) return (bc_lo == SRHD_BC_PERIODIC) ? i + n : 0;
   if (i >= n) return (bc_hi == SRHD_BC_PERIODIC) ? i - n : n - 1;
@@ -216,7 +216,7 @@ extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int
                                 const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
                                 void* stream) {
   if (!grid || !cons_in || !bc) return SRHD_ERR_NULL_POINTER;
-  if (ghost != 2 && ghost != 3) return SRHD_ERR_BAD_PARAMS;
+  if (ghost < 2 || ghost > 4) return SRHD_ERR_BAD_PARAMS;
   const int ce = check_extents(nx, ny, nz);
   if (ce) return ce;
   GridBC b;
@@ -230,6 +230,9 @@ extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   if (ghost == 2)
     grid_gather_kernel<2><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
+                                                                                            b, inflow_mask);
+  else if (ghost == 4)
+    grid_gather_kernel<4><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
                                                                                             b, inflow_mask);
   else
     grid_gather_kernel<3><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
@@ -287,6 +290,9 @@ extern "C" int srhd_patch_gather_speed(const double* patches, double* cons_in, i
   if (params->ghost == 2)
     patch_gather_speed_kernel<2><<<npg, 256, 0, st>>>(patches, cons_in, nx, ny, nz, b, inflow_mask, rtol,
                                                       params->newton_max_iter, d_max_speed);
+  else if (params->ghost == 4)
+    patch_gather_speed_kernel<4><<<npg, 256, 0, st>>>(patches, cons_in, nx, ny, nz, b, inflow_mask, rtol,
+                                                      params->newton_max_iter, d_max_speed);
   else
     patch_gather_speed_kernel<3><<<npg, 256, 0, st>>>(patches, cons_in, nx, ny, nz, b, inflow_mask, rtol,
                                                       params->newton_max_iter, d_max_speed);
@@ -303,6 +309,7 @@ extern "C" void srhd_default_params(srhd_params* p, int recon, int riemann) {
   p->newton_rtol = 1e-15;
   p->newton_max_iter = 20;
   p->ghost = (recon == SRHD_RECON_PLM) ? 2 : 3;
+  p->integrator = SRHD_INTEGRATOR_MHM;
 }
 
 extern "C" const char* srhd_error_string(int code) {

@@ -99,6 +99,9 @@ extern "C" int srhd_refine_flags(const double* cons_in, int npg, int quantity, d
   if (params->ghost == 2)
     refine_flags_kernel<2><<<npg, kRefineThreads, 0, st>>>(cons_in, quantity, c_q, mom_over_d, rtol,
                                                            params->newton_max_iter, flags);
+  else if (params->ghost == 4)
+    refine_flags_kernel<4><<<npg, kRefineThreads, 0, st>>>(cons_in, quantity, c_q, mom_over_d, rtol,
+                                                           params->newton_max_iter, flags);
   else
     refine_flags_kernel<3><<<npg, kRefineThreads, 0, st>>>(cons_in, quantity, c_q, mom_over_d, rtol,
                                                            params->newton_max_iter, flags);

@@ -1,0 +1,96 @@
+"""-m gpu parity of the VL integrator (reading S18; csrc/srhd_vl.cu) with the oracle's: exact build
+bit for bit (outputs, patch-face fluxes, counters), production build to the north-star tolerances, through
+the same C-ABI calls and the same uniform-grid stepper as the MUSCL-Hancock path."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2012_11130_b200 import binding as B
+from paper_2012_11130_b200 import workloads as wl
+from paper_2012_11130_b200.driver import GridStepper
+from tests.gpu_util import l1_rel, step_err
+
+pytestmark = pytest.mark.gpu
+COMBOS = [("plm", "hlle"), ("plm", "hllc"), ("ppm", "hlle"), ("ppm", "hllc")]
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_tiles(ref, npg, ghost, seed, **kw):
+    prim = wl.random_patch_groups(npg, ghost, seed=seed, **kw)
+    nxt = 16 + 2 * ghost
+    cons = ref.prim2cons(prim.transpose(1, 0, 2, 3, 4).reshape(5, -1))
+    return np.ascontiguousarray(cons.reshape(5, npg, nxt, nxt, nxt).transpose(1, 0, 2, 3, 4))
+
+
+@pytest.mark.parametrize("recon,riemann", COMBOS)
+def test_vl_one_step_parity(ref, recon, riemann):
+    po = ref.params(recon, riemann, integrator="vl")
+    npg, dh = 5, 1.0 / 64
+    tiles = make_tiles(ref, npg, po.ghost, seed=21 + po.ghost)
+    dt = 0.4 * dh / ref.max_signal_speed(tiles.transpose(1, 0, 2, 3, 4).reshape(5, -1))
+    want, wflux, st = ref.fluid_step_fluxes(tiles, dt, dh, po)
+    pe = B.params(recon, riemann, exact=True, integrator="vl")
+    assert pe.ghost == po.ghost
+    got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, dh, pe, exact=True)
+    s = B.stats_to_host(sbuf)
+    assert np.array_equal(got.cpu().numpy(), want), float(np.nanmax(step_err(got.cpu().numpy(), want, 2)))
+    assert np.array_equal(gflux.cpu().numpy(), wflux)
+    assert s.algorithm_dict() == st.as_dict()
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, B.params(recon, riemann, integrator="vl"))
+    s = B.stats_to_host(sbuf)
+    err = step_err(got.cpu().numpy(), want, 2)
+    assert err.max() <= 1e-11, err.max()
+    assert (s.n_passes, s.n_retry_pg, s.n_unphys_final, s.n_c2p_fail) == (st.n_passes, st.n_retry_pg, st.n_unphys_final, st.n_c2p_fail)
+    assert abs(s.max_speed - st.max_speed) <= 1e-13 * st.max_speed
+
+
+@pytest.mark.parametrize("recon", ["plm", "ppm"])
+def test_vl_retry_ladder_parity(ref, recon):
+    po = ref.params(recon, "hllc", max_retry=3, integrator="vl")
+    npg, dh = 4, 1.0 / 64
+    tiles = make_tiles(ref, npg, po.ghost, seed=5, umax=30.0, rough=3.0, log_theta=(-8.0, 2.0))
+    dt = 4.0 * 0.4 * dh / ref.max_signal_speed(tiles.transpose(1, 0, 2, 3, 4).reshape(5, -1))
+    want, st = ref.fluid_step(tiles, dt, dh, po)
+    assert st.n_retry_pg > 0
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, B.params(recon, "hllc", max_retry=3, exact=True, integrator="vl"), exact=True)
+    assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+    assert B.stats_to_host(sbuf).algorithm_dict() == st.as_dict()
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, B.params(recon, "hllc", max_retry=3, integrator="vl"))
+    s = B.stats_to_host(sbuf)
+    assert (s.n_passes, s.n_retry_pg, s.n_unphys_final) == (st.n_passes, st.n_retry_pg, st.n_unphys_final)
+
+
+def test_vl_multi_step_on_the_grid_stepper(ref):
+    """blast 64^3 x 40 steps and the TM tube to t = 0.1 with the VL integrator through GridStepper (ghost-zone
+    fill with one more layer, dt on the device): L1 <= 1e-9 production, bit-identical exact build."""
+    prim, dh, bc = wl.blast_wave(n=64)
+    par = ref.params("plm", "hllc", integrator="vl")
+    for exact, nsteps in ((False, 40), (True, 10)):
+        st = GridStepper(prim.shape[1:], dh, bc, "plm", "hllc", cfl=0.4, exact=exact, integrator="vl").set_prim(prim)
+        o = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+        for _ in range(nsteps):
+            dt = st.step()
+            o, _ = ref.grid_step_tiled(o, dt, dh, par, bc)
+        g = st.grid.cpu().numpy()
+        if exact:
+            assert np.array_equal(g, o)
+        else:
+            assert l1_rel(g, o).max() <= 1e-9, l1_rel(g, o)
+    prim, dh, bc = wl.shock_tube()
+    st = GridStepper(prim.shape[1:], dh, bc, "plm", "hllc", cfl=0.5, integrator="vl").set_prim(prim)
+    o = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    while st.t < 0.1:
+        dt = st.step(0.1)
+        o, _ = ref.grid_step_tiled(o, dt, dh, par, bc)
+    assert l1_rel(st.grid.cpu().numpy(), o).max() <= 1e-9
+    # the asynchronous path (dt formed on the device) gives the same bits as the host-dt path
+    a = GridStepper(prim.shape[1:], dh, bc, "plm", "hllc", cfl=0.5, integrator="vl").set_prim(prim)
+    b = GridStepper(prim.shape[1:], dh, bc, "plm", "hllc", cfl=0.5, integrator="vl").set_prim(prim)
+    for _ in range(3):
+        a.step()
+        b.step_async()
+    torch.cuda.synchronize()
+    assert torch.equal(a.grid, b.grid)
