@@ -198,6 +198,12 @@ int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int 
  * in practice.  bench.py uses it for the measured fp64 ALU roof. */
 int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, void* stream);
 
+/* Measurement helper: srhd_fp64_peak_probe's DFMA loop with `ffma_per_8_dfma` (0, 4, 8, 12 or 16) independent
+ * single-precision FMAs interleaved per 8 DFMA.  *dfma_flops (HOST pointer) = flops of the DFMA part only.
+ * Timed by the caller; shows how issue slots are shared between the fp64 pipe and everything else
+ * (output kept under profiles/). */
+int srhd_issue_probe(double* d_sink, int iters, int ffma_per_8_dfma, unsigned long long* dfma_flops, void* stream);
+
 /* Verification helper (not part of the solver): evaluates the library's canonical quotient a/b (the one
  * that feeds the Eq. 30 verdict: one shared reciprocal + a Markstein correction in the production build, IEEE
  * division in the exact build) and IEEE division side by side on n seeded pairs generated on the device;

@@ -45,7 +45,7 @@ class Stats(C.Structure):
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
            "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed",
-           "srhd_fp64_peak_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact"]
+           "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
 
@@ -93,6 +93,8 @@ def load_library(exact=False):
                                           C.POINTER(C.c_double), C.POINTER(Params), _VP, _VP]
     L.srhd_fp64_peak_probe.restype = C.c_int
     L.srhd_fp64_peak_probe.argtypes = [_VP, C.c_int, C.POINTER(C.c_ulonglong), _VP]
+    L.srhd_issue_probe.restype = C.c_int
+    L.srhd_issue_probe.argtypes = [_VP, C.c_int, C.c_int, C.POINTER(C.c_ulonglong), _VP]
     L.srhd_quotient_check.restype = C.c_int
     L.srhd_quotient_check.argtypes = [C.c_ulonglong, C.c_ulonglong, C.c_int, _VP, _VP]
     L.srhd_error_string.restype = C.c_char_p
@@ -342,3 +344,32 @@ def quotient_check(n, seed=1, dist=0, exact=False):
     _check(L.srhd_quotient_check(int(n), int(seed), int(dist), out.data_ptr(), _stream()), L)
     o = out.cpu().numpy().view("uint64")
     return int(o[0]), int(o[1])
+
+
+def issue_probe(iters=2048, reps=3):
+    """srhd_issue_probe timed with CUDA events: {FFMA per 8 DFMA: DFMA TFLOP/s}.  `python -m
+    paper_2012_11130_b200.binding issue_probe` prints the table kept under profiles/."""
+    L = load_library(False)
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    out = {}
+    for ni in (0, 4, 8, 12, 16):
+        flops, best = C.c_ulonglong(0), 0.0
+        for r in range(reps + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            _check(L.srhd_issue_probe(sink.data_ptr(), iters, ni, C.byref(flops), _stream()), L)
+            e1.record()
+            e1.synchronize()
+            if r:
+                best = max(best, flops.value / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        out[ni] = best
+    return out
+
+
+if __name__ == "__main__":
+    import sys
+    if sys.argv[1:] == ["issue_probe"]:
+        t = issue_probe()
+        print("| FFMA per 8 DFMA | DFMA TFLOP/s | relative to 0 | 16/(16+NI) |\n|---|---|---|---|")
+        for ni, v in t.items():
+            print(f"| {ni} | {v:.2f} | {v / t[0]:.3f} | {16 / (16 + ni):.3f} |")

@@ -350,6 +350,56 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double* __restrict__ sin
 }
 }  // namespace srhd
 
+// ---- issue-port probe: the same DFMA loop with NI independent FFMA interleaved per 8 DFMA.  If an fp64
+// warp instruction held only the fp64 pipe, up to 8 FFMA per 8 DFMA would issue in its shadow for free; the
+// measured DFMA rate instead falls as 16/(16 + NI): every fp64 warp instruction occupies its scheduler's issue
+// port for two cycles and any other instruction for one, with no overlap.
+namespace srhd {
+template <int NI>
+__global__ void __launch_bounds__(256) issue_probe_kernel(double* __restrict__ sink, int iters, double a, double b,
+                                                          float fa, float fb) {
+  double x[8];
+  float y[16];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = 1.0 + 1e-3 * (threadIdx.x + k);
+#pragma unroll
+  for (int k = 0; k < 16; ++k) y[k] = 1.0f + 1e-3f * (threadIdx.x + k);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(x[k], a, b);
+#pragma unroll
+      for (int k = 0; k < NI; ++k) y[k] = fmaf(y[k], fa, fb);
+    }
+  }
+  double acc = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc += x[k];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) acc += y[k];
+  if (acc == 12345.678) sink[0] = acc;    // never true
+}
+}  // namespace srhd
+
+extern "C" int srhd_issue_probe(double* d_sink, int iters, int ffma_per_8_dfma, unsigned long long* dfma_flops,
+                                void* stream) {
+  if (!d_sink) return SRHD_ERR_NULL_POINTER;
+  if (iters < 1) return SRHD_ERR_BAD_SIZE;
+  const int grid = srhd::kNumSMs * 8, block = 256;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  switch (ffma_per_8_dfma) {
+    case 0: srhd::issue_probe_kernel<0><<<grid, block, 0, st>>>(d_sink, iters, 0.999999, 1e-6, 0.99999f, 1e-6f); break;
+    case 4: srhd::issue_probe_kernel<4><<<grid, block, 0, st>>>(d_sink, iters, 0.999999, 1e-6, 0.99999f, 1e-6f); break;
+    case 8: srhd::issue_probe_kernel<8><<<grid, block, 0, st>>>(d_sink, iters, 0.999999, 1e-6, 0.99999f, 1e-6f); break;
+    case 12: srhd::issue_probe_kernel<12><<<grid, block, 0, st>>>(d_sink, iters, 0.999999, 1e-6, 0.99999f, 1e-6f); break;
+    case 16: srhd::issue_probe_kernel<16><<<grid, block, 0, st>>>(d_sink, iters, 0.999999, 1e-6, 0.99999f, 1e-6f); break;
+    default: return SRHD_ERR_BAD_PARAMS;
+  }
+  if (dfma_flops) *dfma_flops = 2ull * 32ull * (unsigned long long)iters * (unsigned long long)grid * block;
+  return (int)cudaGetLastError();
+}
+
 extern "C" int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, void* stream) {
   if (!d_sink) return SRHD_ERR_NULL_POINTER;
   if (iters < 1) return SRHD_ERR_BAD_SIZE;
