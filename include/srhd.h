@@ -159,6 +159,34 @@ int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_ou
 int srhd_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
                       const srhd_params* params, unsigned char* flags, void* stream);
 
+/* Flux correction at coarse-fine interfaces with the paper's guard (section 3.3(4)): the coarse cells
+ * next to the interface were updated with the coarse flux through it (flux_out of srhd_fluid_step_fluxes); this
+ * call swaps that flux for the fine one (already averaged over the fine faces and sub-steps by the driver):
+ *     lo face: U' = U + dt/dh (F_fine - F_coarse),    hi face: U' = U - dt/dh (F_fine - F_coarse),
+ * and "if unphysical results are found after this flux correction, we simply ignore the correction on the
+ * failed cells": U' that fails Eq. 30 is dropped and counted.
+ *   patches     : device, [np][5][8][8][8] (cons_out layout, updated in place)
+ *   flux_coarse, flux_fine : device, [nf][5][8][8], in-face layout of flux_out
+ *   face_patch, face_id    : device, [nf] ints: patch index, face 0 x-lo .. 5 z-hi
+ *   d_n_skipped : device, one unsigned long long (zeroed by the call): cells whose correction was ignored
+ * Faces are processed class by class (x-lo, x-hi, y-lo, ...), so a cell on a patch edge is corrected through
+ * one face after the other, in that order; within a class a (patch, face) pair may appear once. */
+int srhd_flux_correction(double* patches, const double* flux_coarse, const double* flux_fine,
+                         const int* face_patch, const int* face_id, int nf, double dt, double dh,
+                         unsigned long long* d_n_skipped, void* stream);
+
+/* Ghost-zone interpolation with the primitive-variable fallback (section 3.3(3)): every coarse cell with six
+ * neighbours gives its 2^3 children Q -+ d_x/4 -+ d_y/4 -+ d_z/4 with the limited slopes of reading S3
+ * (coefficient minmod_coeff) on the CONSERVED variables (conservative); where a child fails Eq. 30 the
+ * same interpolation is done on the PRIMITIVE variables of the seven cells and converted back ("Eq. 30 is
+ * always satisfied ... ghost zones do not affect conservation").
+ *   coarse: device, [5][nz][ny][nx];  fine: device, [5][2(nz-2)][2(ny-2)][2(nx-2)]
+ *   fallback: device, (nz-2)(ny-2)(nx-2) bytes, 1 where the fallback was used (may be NULL)
+ *   d_n_fallback: device, one unsigned long long (zeroed by the call) */
+int srhd_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine, double minmod_coeff,
+                      const srhd_params* params, unsigned char* fallback, unsigned long long* d_n_fallback,
+                      void* stream);
+
 /* Bytes of scratch a srhd_fluid_step call uses: 0 for MUSCL-Hancock (fully fused); for the VL integrator
  * the two primitive tiles its stages communicate through, which the call allocates and frees itself in
  * stream order (cudaMallocAsync / cudaFreeAsync on `stream`): informational, nothing for the caller to provide. */

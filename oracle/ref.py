@@ -238,6 +238,33 @@ def refine_flags(cons_in, par, quantity="rho", c_q=0.3, mom_over_d=0.0):
     return flags
 
 
+def flux_correction(patches, flux_coarse, flux_fine, face_patch, face_id, dt, dh):
+    """(corrected copy of patches (np,5,8,8,8), number of skipped cells)."""
+    out = _f64(patches).copy()
+    fc, ff = _f64(flux_coarse), _f64(flux_fine)
+    fp = np.ascontiguousarray(face_patch, dtype=np.int32)
+    fi = np.ascontiguousarray(face_id, dtype=np.int32)
+    f = lib().srhd_ref_flux_correction
+    f.restype = C.c_ulonglong
+    ip = C.POINTER(C.c_int)
+    n = f(_p(out), _p(fc), _p(ff), fp.ctypes.data_as(ip), fi.ctypes.data_as(ip), C.c_int(len(fp)), _D(dt), _D(dh))
+    return out, int(n)
+
+
+def ghost_interp(coarse, beta, par=None):
+    """coarse (5,nz,ny,nx) -> (fine (5,2(nz-2),2(ny-2),2(nx-2)), fallback flags (nz-2,ny-2,nx-2), count)."""
+    coarse = _f64(coarse)
+    par = par or params()
+    _, nz, ny, nx = coarse.shape
+    fine = np.empty((5, 2 * (nz - 2), 2 * (ny - 2), 2 * (nx - 2)))
+    fb = np.zeros((nz - 2, ny - 2, nx - 2), dtype=np.uint8)
+    f = lib().srhd_ref_ghost_interp
+    f.restype = C.c_ulonglong
+    n = f(_p(coarse), C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(fine), _D(beta), C.byref(par),
+          fb.ctypes.data_as(C.POINTER(C.c_ubyte)))
+    return fine, fb, int(n)
+
+
 def _bc(bc):
     m = {"periodic": 0, "outflow": 1}
     return (C.c_int * 6)(*[m[b] if isinstance(b, str) else int(b) for b in bc])

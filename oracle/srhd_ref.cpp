@@ -922,6 +922,103 @@ void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny,
 }
 
 
+// ---- coarse-fine hooks of the AMR driver (section 3.3(3), section 3.3(4)) ------------------
+// Flux correction with the "skip if unphysical" rule: the coarse cells next to a coarse-fine
+// interface were updated with the coarse flux through that face; the correction swaps it for the fine
+// fluxes (already averaged over the fine faces and sub-steps by the caller):
+//   lo face:  U' = U + dt/dh (F_fine - F_coarse)        hi face:  U' = U - dt/dh (F_fine - F_coarse)
+// If U' fails Eq. 30 the correction is ignored for that cell (counted).  Faces are processed class by class
+// (all x-lo faces, then x-hi, y-lo, ... ): a cell on a patch edge is corrected through one face after the other.
+//   patches [np][5][8][8][8]; flux_coarse, flux_fine [nf][5][8][8] (in-face layout of flux_out); face_patch,
+//   face_id [nf] (0 x-lo, 1 x-hi, 2 y-lo, 3 y-hi, 4 z-lo, 5 z-hi).  Returns the number of skipped cells.
+unsigned long long srhd_ref_flux_correction(double* patches, const double* flux_coarse, const double* flux_fine,
+                                            const int* face_patch, const int* face_id, int nf, double dt, double dh) {
+  unsigned long long skipped = 0;
+  const double dtdh = dt / dh;
+  for (int cls = 0; cls < 6; ++cls)
+    for (int f = 0; f < nf; ++f) {
+      if (face_id[f] != cls) continue;
+      const int d = cls >> 1, hi = cls & 1;
+      double* P = patches + (size_t)face_patch[f] * 5 * 512;
+      for (int a = 0; a < 8; ++a)
+        for (int bb = 0; bb < 8; ++bb) {
+          int i, j, k;
+          if (d == 0) { i = hi ? 7 : 0; j = bb; k = a; }
+          else if (d == 1) { i = bb; j = hi ? 7 : 0; k = a; }
+          else { i = bb; j = a; k = hi ? 7 : 0; }
+          const size_t c = (size_t)k * 64 + j * 8 + i;
+          double Un[5];
+          for (int q = 0; q < 5; ++q) {
+            const double dF = flux_fine[((size_t)f * 5 + q) * 64 + a * 8 + bb] - flux_coarse[((size_t)f * 5 + q) * 64 + a * 8 + bb];
+            Un[q] = hi ? P[q * 512 + c] - dtdh * dF : P[q * 512 + c] + dtdh * dF;
+          }
+          if (is_physical(Un)) { for (int q = 0; q < 5; ++q) P[q * 512 + c] = Un[q]; }
+          else ++skipped;                                   // "we simply ignore the correction"
+        }
+    }
+  return skipped;
+}
+
+// Ghost-zone interpolation with the primitive-variable fallback: every coarse cell that has all six
+// neighbours gives its 2^3 children  Q_child = ((Q + sx dx/4) + sy dy/4) + sz dz/4,  s = -+1, with the limited
+// slopes d of reading S3 (coefficient beta) -- on the CONSERVED variables (conservative: the children average to
+// the parent).  If any child fails Eq. 30, the same interpolation is done on the PRIMITIVE variables of the
+// seven cells and the children are converted back (always physical; "ghost zones do not affect conservation").
+//   coarse [5][nz][ny][nx];  fine [5][2(nz-2)][2(ny-2)][2(nx-2)];  fallback (may be null) [nz-2][ny-2][nx-2] bytes.
+unsigned long long srhd_ref_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine, double beta,
+                                         const srhd_ref_params* par, unsigned char* fallback) {
+  const size_t n = (size_t)nx * ny * nz;
+  const int fx = 2 * (nx - 2), fy = 2 * (ny - 2), fz = 2 * (nz - 2);
+  const size_t nf = (size_t)fx * fy * fz;
+  const ptrdiff_t stp[3] = {1, nx, (ptrdiff_t)nx * ny};
+  unsigned long long nfb = 0;
+  for (int k = 1; k < nz - 1; ++k)
+    for (int j = 1; j < ny - 1; ++j)
+      for (int i = 1; i < nx - 1; ++i) {
+        const size_t c = ((size_t)k * ny + j) * nx + i;
+        double Q[7][5];                                       // cell, x-, x+, y-, y+, z-, z+
+        for (int q = 0; q < 5; ++q) {
+          Q[0][q] = coarse[q * n + c];
+          for (int d = 0; d < 3; ++d) {
+            Q[1 + 2 * d][q] = coarse[q * n + c - stp[d]];
+            Q[2 + 2 * d][q] = coarse[q * n + c + stp[d]];
+          }
+        }
+        double child[8][5];
+        bool ok = true, fell_back = false;
+        for (int pass = 0; pass < 2; ++pass) {                // 0: conserved variables, 1: primitive variables
+          double V[7][5];
+          for (int m = 0; m < 7; ++m) {
+            if (pass == 0) for (int q = 0; q < 5; ++q) V[m][q] = Q[m][q];
+            else cons2prim(Q[m], V[m], par->newton_rtol, par->newton_max_iter, nullptr, nullptr);
+          }
+          double sl[3][5];
+          for (int d = 0; d < 3; ++d)
+            for (int q = 0; q < 5; ++q)
+              sl[d][q] = 0.25 * limited_slope(V[0][q] - V[1 + 2 * d][q], V[2 + 2 * d][q] - V[0][q], beta);
+          ok = true;
+          for (int ch = 0; ch < 8; ++ch) {
+            double v[5];
+            for (int q = 0; q < 5; ++q) {
+              const double ax = (ch & 1) ? sl[0][q] : -sl[0][q], ay = (ch & 2) ? sl[1][q] : -sl[1][q],
+                           az = (ch & 4) ? sl[2][q] : -sl[2][q];
+              v[q] = ((V[0][q] + ax) + ay) + az;
+            }
+            if (pass == 0) { for (int q = 0; q < 5; ++q) child[ch][q] = v[q]; ok = ok && is_physical(v); }
+            else prim2cons(v, child[ch]);
+          }
+          if (ok) break;
+          if (pass == 0) { ++nfb; fell_back = true; }
+        }
+        if (fallback) fallback[((size_t)(k - 1) * (ny - 2) + (j - 1)) * (nx - 2) + (i - 1)] = fell_back ? 1 : 0;
+        for (int ch = 0; ch < 8; ++ch) {
+          const int I = 2 * (i - 1) + (ch & 1), J = 2 * (j - 1) + ((ch >> 1) & 1), Kk = 2 * (k - 1) + (ch >> 2);
+          for (int q = 0; q < 5; ++q) fine[q * nf + ((size_t)Kk * fy + J) * fx + I] = child[ch][q];
+        }
+      }
+  return nfb;
+}
+
 // ---- refinement criteria (section 3.1; Eq. 33; reading S17: centred differences) --
 // quantity: 0 none, 1 D, 2 Etilde, 3 rho, 4 Lorentz factor.  flags[pg*8 + p], patch p as in S13.
 void srhd_ref_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,

@@ -111,6 +111,16 @@ void srhd_ref_grid_gather(const double* grid, double* cons_in, int nx, int ny, i
                           const double* inflow_cons);
 void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz);
 
+// --- coarse-fine hooks (section 3.3(3), section 3.3(4)); see srhd_ref.cpp for layouts ------------
+// flux correction of the coarse cells next to a coarse-fine interface, skipped where the corrected cell fails
+// Eq. 30; returns the number of skipped cells
+unsigned long long srhd_ref_flux_correction(double* patches, const double* flux_coarse, const double* flux_fine,
+                                            const int* face_patch, const int* face_id, int nf, double dt, double dh);
+// 2x ghost-zone interpolation of conserved variables with the primitive-variable fallback; returns the number
+// of coarse cells that fell back
+unsigned long long srhd_ref_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine, double beta,
+                                         const srhd_ref_params* par, unsigned char* fallback);
+
 // --- refinement criteria of the SRHD module (section 3.1; Eq. 33) -----------------
 // per 8^3 patch of ghosted patch-group tiles: flag = any cell with
 //   (|dQ_x| + |dQ_y| + |dQ_z|) / (2|Q|) > c_q  (centred differences over two cells: reading S17)

@@ -44,7 +44,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_flux_correction", "srhd_ghost_interp", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed",
            "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -79,6 +79,10 @@ def load_library(exact=False):
     L.srhd_fluid_step_cfl.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, _VP, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_refine_flags.restype = C.c_int
     L.srhd_refine_flags.argtypes = [_VP, C.c_int, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
+    L.srhd_flux_correction.restype = C.c_int
+    L.srhd_flux_correction.argtypes = [_VP, _VP, _VP, _VP, _VP, C.c_int, _D, _D, _VP, _VP]
+    L.srhd_ghost_interp.restype = C.c_int
+    L.srhd_ghost_interp.argtypes = [_VP, C.c_int, C.c_int, C.c_int, _VP, _D, C.POINTER(Params), _VP, _VP, _VP]
     L.srhd_workspace_bytes.restype = C.c_size_t
     L.srhd_workspace_bytes.argtypes = [C.c_int, C.POINTER(Params)]
     L.srhd_grid_gather.restype = C.c_int
@@ -249,6 +253,38 @@ def refine_flags(cons_in, par, quantity="rho", c_q=0.3, mom_over_d=0.0, flags=No
     _check(L.srhd_refine_flags(cons_in.data_ptr(), npg, q, float(c_q), float(mom_over_d), C.byref(par),
                                flags.data_ptr(), _stream()), L)
     return flags
+
+
+def flux_correction(patches, flux_coarse, flux_fine, face_patch, face_id, dt, dh, exact=False):
+    """srhd_flux_correction (in place on patches (np,5,8,8,8)); returns a 1-element int64 device tensor: skipped cells."""
+    L = load_library(exact)
+    _dev(patches, "patches"), _dev(flux_coarse, "flux_coarse"), _dev(flux_fine, "flux_fine")
+    for t, nm in ((face_patch, "face_patch"), (face_id, "face_id")):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+            raise SrhdError(f"{nm} must be a contiguous int32 CUDA tensor")
+    nf = face_patch.numel()
+    if tuple(flux_coarse.shape) != (nf, 5, 8, 8) or tuple(flux_fine.shape) != (nf, 5, 8, 8) or face_id.numel() != nf:
+        raise SrhdError("flux_coarse / flux_fine must have shape (nf,5,8,8) and face_id nf entries")
+    if patches.dim() != 5 or tuple(patches.shape[1:]) != (5, 8, 8, 8) or (nf and int(face_patch.max()) >= patches.shape[0]):
+        raise SrhdError("patches must have shape (np,5,8,8,8) and face_patch must index it")
+    out = torch.zeros(1, dtype=torch.int64, device=patches.device)
+    _check(L.srhd_flux_correction(patches.data_ptr(), flux_coarse.data_ptr(), flux_fine.data_ptr(), face_patch.data_ptr(),
+                                  face_id.data_ptr(), nf, float(dt), float(dh), out.data_ptr(), _stream()), L)
+    return out
+
+
+def ghost_interp(coarse, minmod_coeff, par=None, exact=False):
+    """srhd_ghost_interp: coarse (5,nz,ny,nx) -> (fine (5,2(nz-2),2(ny-2),2(nx-2)), fallback flags uint8, count tensor)."""
+    L = load_library(exact)
+    coarse = _dev(coarse, "coarse")
+    par = par or params(exact=exact)
+    _, nz, ny, nx = coarse.shape
+    fine = torch.empty((5, 2 * (nz - 2), 2 * (ny - 2), 2 * (nx - 2)), dtype=torch.float64, device=coarse.device)
+    fb = torch.zeros((nz - 2, ny - 2, nx - 2), dtype=torch.uint8, device=coarse.device)
+    cnt = torch.zeros(1, dtype=torch.int64, device=coarse.device)
+    _check(L.srhd_ghost_interp(coarse.data_ptr(), nx, ny, nz, fine.data_ptr(), float(minmod_coeff), C.byref(par),
+                               fb.data_ptr(), cnt.data_ptr(), _stream()), L)
+    return fine, fb, cnt
 
 
 def _bc(bc):
