@@ -32,7 +32,11 @@ def test_flux_correction_parity_and_skip_rule(ref):
         n = B.flux_correction(d, dev(fc), dev(ff), dev(np.array(fp), torch.int32), dev(np.array(fi), torch.int32), 0.3, 1.0,
                               exact=exact)
         assert int(n.cpu()) == skipped
-        assert np.array_equal(d.cpu().numpy(), want)                   # adds and one multiply: bit for bit in both builds
+        g = d.cpu().numpy()
+        if exact:
+            assert np.array_equal(g, want)
+        else:                                                           # the production build contracts U - dtdh*dF into an fma
+            assert (np.abs(g - want) <= 4e-16 * (np.abs(want) + 0.3 * np.abs(ff - fc).max())).all()
 
 
 def test_ghost_interp_parity_with_fallback(ref):
