@@ -88,6 +88,8 @@ typedef struct {
   unsigned long long exec_newton;     /* Newton-Raphson iterations executed                           */
   unsigned long long exec_riemann;    /* HLLE / HLLC solves executed                                  */
   unsigned long long exec_hancock;    /* (cell, direction) edge-state pairs reconstructed + converted */
+  unsigned long long n_uniform_pg;    /* patch groups whose whole tile held one state bit for bit and took
+                                         the uniform-tile path (the result is the input; see srhd_fluid.cu) */
 } srhd_stats;
 
 /* Fill *p with the defaults above for the given recon / riemann choice (host pointer). */
@@ -187,9 +189,10 @@ int srhd_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine
                       const srhd_params* params, unsigned char* fallback, unsigned long long* d_n_fallback,
                       void* stream);
 
-/* Bytes of scratch a srhd_fluid_step call uses: 0 for MUSCL-Hancock (fully fused); for the VL integrator
- * the two primitive tiles its stages communicate through, which the call allocates and frees itself in
- * stream order (cudaMallocAsync / cudaFreeAsync on `stream`): informational, nothing for the caller to provide. */
+/* Bytes of scratch a srhd_fluid_step call uses: for MUSCL-Hancock one byte per patch group (the flags by
+ * which the uniform-tile pre-pass tells the main kernel which groups it has already written); for the VL
+ * integrator the two primitive tiles its stages communicate through.  The call allocates and frees them itself
+ * in stream order (cudaMallocAsync / cudaFreeAsync on `stream`): informational, nothing for the caller to provide. */
 size_t srhd_workspace_bytes(int npg, const srhd_params* params);
 
 /* Harness helpers for a uniform grid (reading S11, S13; NOT part of the paper's solver: they stand in

@@ -33,14 +33,15 @@ class Stats(C.Structure):
     _fields_ = [("n_c2p_fail", C.c_ulonglong), ("n_retry_pg", C.c_ulonglong),
                 ("n_unphys_final", C.c_ulonglong), ("newton_iters", C.c_ulonglong),
                 ("max_speed", C.c_double), ("n_passes", C.c_ulonglong), ("exec_c2p", C.c_ulonglong),
-                ("exec_newton", C.c_ulonglong), ("exec_riemann", C.c_ulonglong), ("exec_hancock", C.c_ulonglong)]
+                ("exec_newton", C.c_ulonglong), ("exec_riemann", C.c_ulonglong), ("exec_hancock", C.c_ulonglong),
+                ("n_uniform_pg", C.c_ulonglong)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
     def algorithm_dict(self):
         """The counters the algorithm defines (everything but the executed-work figures)."""
-        return {k: getattr(self, k) for k, _ in self._fields_ if not k.startswith("exec_")}
+        return {k: getattr(self, k) for k, _ in self._fields_ if not k.startswith("exec_") and k != "n_uniform_pg"}
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",

@@ -151,14 +151,116 @@ SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
   return false;
 }
 
+// Uniform tiles (undisturbed ambient gas ahead of a blast wave or a jet): every cell of the tile, ghost zones
+// included, holds the same five doubles bit for bit.  Then the whole algorithm collapses to values that
+// one thread can form: W0 = C2P(U0) for every tile cell; all slopes vanish, so every edge state is
+// U1 = P2C(W0) and every flux difference of the half step is +0 (U1 + (-0) = U1); every face solves the same
+// Riemann problem F_d(U1, U1); every update is U0 - dt/dh ((F-F) + (F-F) + (F-F)) = U0.  This pre-pass (one
+// CTA per patch group, launched ahead of fluid_step_kernel on the same stream) streams such a tile once from
+// HBM (16-byte loads, compared as bit patterns), writes the 8 patches, adds what the march would have counted
+// to the counters and sets handled[pg] = 1, which makes the main kernel's CTA return at once.  Anything unusual
+// (a state that fails Eq. 30, a non-finite flux) is left to the main kernel; a tile that is not uniform is
+// dropped at its first 4 KB.  It is a kernel of its own, not a branch of the main one: a data-dependent early
+// exit there makes nvcc guard every warp collective of the march with a divergence test (BRA.DIV; measured
+// +25 % kernel time on data without a single uniform tile).
+constexpr int kScanThreads = 256;
+template <int G, int RS>
+__global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
+    const double* __restrict__ cons_in, double* __restrict__ cons_out, double* __restrict__ flux_out, double dt,
+    double dh, double rtol, int max_iter, srhd_stats* __restrict__ stats, const double* __restrict__ d_smax,
+    double cfl, double min_speed, unsigned char* __restrict__ handled) {
+  using P = Plan<G>;
+  constexpr int NT = kScanThreads, T3 = P::T3;
+  constexpr int H = T3 / 2;                                  // 16-byte words per component
+  static_assert(T3 % 2 == 0, "tile components must be whole 16-byte words");
+  const int tid = threadIdx.x;
+  const double* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
+  double* __restrict__ out = cons_out + (size_t)blockIdx.x * 8 * 5 * 512;
+  double* __restrict__ fout = flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr;
+  if (tid == 0) handled[blockIdx.x] = 0;
+  const double2* __restrict__ t2 = reinterpret_cast<const double2*>(tile);
+  unsigned long long ref[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) ref[q] = (unsigned long long)__double_as_longlong(__ldg(tile + (size_t)q * T3));
+  auto differs = [&](int w, double2 v) {
+    const int q = w / H;
+    const unsigned long long r = (q == 0) ? ref[0] : (q == 1) ? ref[1] : (q == 2) ? ref[2] : (q == 3) ? ref[3] : ref[4];
+    return ((unsigned long long)__double_as_longlong(v.x) != r) || ((unsigned long long)__double_as_longlong(v.y) != r);
+  };
+  if (__syncthreads_or(differs(tid, __ldg(t2 + tid)) ? 1 : 0)) return;      // the first 4 KB settle most tiles
+  for (int base = NT; base < 5 * H; base += 8 * NT) {
+    double2 v[8];
+    int w[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      w[u] = min(base + u * NT + tid, 5 * H - 1);
+      v[u] = __ldg(t2 + w[u]);
+    }
+    bool diff = false;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) diff = diff || differs(w[u], v[u]);
+    if (__syncthreads_or(diff ? 1 : 0)) return;
+  }
+  if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);      // as the main kernel (srhd_fluid_step_cfl)
+  const double dtdh = dt / dh;
+  double U0[1][5], W0[1][5], U1[1][5], W1[1][5], F[3][5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U0[0][q] = __longlong_as_double((long long)ref[q]);
+  bool ph0[1], ph1[1];
+  int it0[1], it1[1];
+  Aux a0[1], a1[1], ae;
+  cons2prim_multi<1>(U0, W0, a0, rtol, max_iter, ph0, it0);
+  prim2cons_aux(W0[0], U1[0], ae);
+  cons2prim_multi<1>(U1, W1, a1, rtol, max_iter, ph1, it1);
+  bool ok = ph0[0] && ph1[0] && is_physical(U0[0]) && (fabs(dtdh) <= DBL_MAX);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    riemann_flux<RS>(d, W1[0], U1[0], a1[0], W1[0], U1[0], a1[0], F[d], true);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) ok = ok && (fabs(F[d][q]) <= DBL_MAX);
+  }
+  if (!ok) return;                                           // every thread computed the same verdict
+  double2* __restrict__ o2 = reinterpret_cast<double2*>(out);
+  for (int w = tid; w < 8 * 5 * 256; w += NT) {              // out[patch][component][512]
+    const int q = (w >> 8) % 5;
+    const double u = (q == 0) ? U0[0][0] : (q == 1) ? U0[0][1] : (q == 2) ? U0[0][2] : (q == 3) ? U0[0][3] : U0[0][4];
+    o2[w] = make_double2(u, u);
+  }
+  if (fout) {
+    for (int w = tid; w < 8 * 6 * 5 * 64; w += NT) {         // flux_out[patch][face][component][64]
+      const int q = (w >> 6) % 5, d = ((w / 320) % 6) >> 1;
+      double f = 0.0;
+#pragma unroll
+      for (int dd = 0; dd < 3; ++dd)
+#pragma unroll
+        for (int qq = 0; qq < 5; ++qq) f = (dd == d && qq == q) ? F[dd][qq] : f;
+      fout[w] = f;
+    }
+  }
+  if (tid == 0) {
+    handled[blockIdx.x] = 1;
+    if (stats) {
+      atomicAdd(&stats->newton_iters, (unsigned long long)T3 * (unsigned)it0[0] +
+                                          (unsigned long long)(2 * 3 * 17 * 256) * (unsigned)it1[0]);
+      atomicAdd(&stats->n_passes, 1ull);
+      atomicAdd(&stats->exec_newton, (unsigned long long)(it0[0] + it1[0]));
+      atomicAdd(&stats->exec_c2p, 2ull);
+      atomicAdd(&stats->exec_riemann, SRHD_EXACT ? 3ull : 0ull);
+      atomicAdd(&stats->n_uniform_pg, 1ull);
+      atomic_max_nonneg(&stats->max_speed, smax_of_umax(umax_of_prim(W0[0], a0[0])));
+    }
+  }
+}
+
 template <int G, int RS>
 __global__ void __launch_bounds__(kFluidThreads, 1)
 fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out,
                   double* __restrict__ flux_out, double dt, double dh, double beta0, int max_retry, double rtol,
                   int max_iter, srhd_stats* __restrict__ stats, const double* __restrict__ d_smax, double cfl,
-                  double min_speed) {
+                  double min_speed, const unsigned char* __restrict__ handled) {
   using P = Plan<G>;
   constexpr int NT = kFluidThreads, NW = NT / 32;
+  if (handled[blockIdx.x]) return;              // a uniform tile: uniform_tiles_kernel wrote its result
   constexpr int NXT = P::NXT, PL = P::PL, T3 = P::T3, R = P::R;
   constexpr int NP1 = (PL + 31) / 32;           // cons2prim chunks per tile plane
   constexpr int NXY = 2 * P::NFXY / 32;         // x and y face chunks per plane (544 faces = 17 x 32)
@@ -235,6 +337,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);   // Eq. 28 formed on the device (srhd_fluid_step_cfl)
   const double hdt = dt / (2.0 * dh);
   const double dtdh = dt / dh;
+
   unsigned long long my_iters = 0;     // iterations of the algorithm's conversions (centre cells + accepted pass)
   unsigned long long ex_newton = 0;    // executed work (every pass, shortcuts taken into account)
   unsigned ex_c2p = 0, ex_riemann = 0, ex_hancock = 0;
@@ -356,6 +459,11 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
             }
             continue;
           }
+          // `has` differs from lane to lane and nvcc likes to test it BEFORE the warp-uniform warp_flat (jump
+          // threading), which sends the two groups of lanes to the shuffles below along different paths: a
+          // diverged warp executes every shuffle through the slow collective path (measured: +25 % kernel time).
+          // The explicit convergence point keeps the lanes together whatever the compiler does above it.
+          __syncwarp();
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
             const double fx = __shfl_sync(0xffffffffu, dF[q], hbase);
@@ -583,10 +691,18 @@ int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int 
   const size_t smem = Plan<G>::bytes;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
-  kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, flux_out, dt, dh, p->minmod_coeff, p->max_retry,
-                                         newton_stop_rtol(p->newton_rtol), p->newton_max_iter, stats, d_smax, cfl,
-                                         min_speed);
-  return (int)cudaGetLastError();
+  // one byte per patch group between the two kernels, allocated and freed in stream order
+  unsigned char* handled = nullptr;
+  e = cudaMallocAsync(reinterpret_cast<void**>(&handled), (size_t)npg, st);
+  if (e != cudaSuccess) return (int)e;
+  const double rtol = newton_stop_rtol(p->newton_rtol);
+  uniform_tiles_kernel<G, RS><<<npg, kScanThreads, 0, st>>>(cons_in, cons_out, flux_out, dt, dh, rtol,
+                                                            p->newton_max_iter, stats, d_smax, cfl, min_speed, handled);
+  kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, flux_out, dt, dh, p->minmod_coeff, p->max_retry, rtol,
+                                         p->newton_max_iter, stats, d_smax, cfl, min_speed, handled);
+  e = cudaGetLastError();
+  const cudaError_t e2 = cudaFreeAsync(handled, st);
+  return (int)(e != cudaSuccess ? e : e2);
 }
 
 }  // namespace srhd
@@ -601,7 +717,8 @@ size_t vl_workspace_bytes(int npg, const srhd_params* p);
 using namespace srhd;
 
 extern "C" size_t srhd_workspace_bytes(int npg, const srhd_params* params) {
-  if (check_params(params) != SRHD_OK || params->integrator == SRHD_INTEGRATOR_MHM) return 0;
+  if (check_params(params) != SRHD_OK || npg <= 0) return 0;
+  if (params->integrator == SRHD_INTEGRATOR_MHM) return (size_t)npg;   // the uniform-tile flags, one byte per group
   return vl_workspace_bytes(npg, params);
 }
 

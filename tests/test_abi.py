@@ -55,7 +55,7 @@ def test_defaults_and_error_strings():
     L = b.load_library()
     for code in range(-6, 1):
         assert len(L.srhd_error_string(code)) > 1
-    assert L.srhd_workspace_bytes(10, C.byref(p)) == 0
+    assert L.srhd_workspace_bytes(10, C.byref(p)) == 10   # MUSCL-Hancock: one flag byte per patch group
 
 
 def test_argument_errors_without_gpu():

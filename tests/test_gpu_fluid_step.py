@@ -270,3 +270,47 @@ def test_retry_ladder_parity_production_build(ref, recon, riemann):
         assert s.n_passes == sum(st.n_passes for _, st in per_group)
         assert s.exec_c2p >= tiles.shape[0] * ((16 + 2 * po.ghost) ** 3)      # the executed-work counters are live
         assert np.array_equal(np.isfinite(got.cpu().numpy()), np.isfinite(want))
+
+
+@pytest.mark.parametrize("recon,riemann", COMBOS)
+def test_uniform_tile_path_parity(ref, recon, riemann):
+    """Tiles that hold ONE state bit for bit take the uniform-tile path of the kernel (srhd_stats.n_uniform_pg):
+    output, patch-boundary fluxes and every algorithm counter must be what the oracle's full march gives.  Tiles
+    that differ from uniform in one cell (first / last tile cell, one interior cell), and a uniform state that fails
+    Eq. 30, must take the general path and match too."""
+    po = ref.params(recon, riemann)
+    nxt, dh = 16 + 2 * po.ghost, 1.0 / 64
+    states = np.array([[0.7, 3.0e2, -1.0e2, 5.0e1, 1e-4],        # fast and cold
+                       [1.0, 0.0, 0.0, 0.0, 1e-6],               # ambient gas at rest (blast / jet configs)
+                       [2.5e-3, -0.4, 0.3, 2.0, 40.0]])          # hot
+    cons = ref.prim2cons(states.T.copy())                         # (5, 3)
+    npg = 7
+    tiles = np.empty((npg, 5, nxt, nxt, nxt))
+    for pg in range(npg):
+        tiles[pg] = cons[:, pg % 3][:, None, None, None]
+    tiles[3, 0, 0, 0, 0] *= 1.0 + 2.0 ** -52                      # one ulp in the first tile cell
+    tiles[4, 4, -1, -1, -1] *= 1.0 + 2.0 ** -52                   # ... in the last one
+    tiles[5, 2, nxt // 2, nxt // 2, nxt // 2] += 1e-3             # one interior cell
+    tiles[6, 4] = -1e-9                                           # uniform but unphysical (Etilde < 0): general path
+    dt = 0.4 * dh
+    want, wflux, st = ref.fluid_step_fluxes(tiles, dt, dh, po)
+    pe = B.params(recon, riemann, exact=True)
+    got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, dh, pe, exact=True)
+    s = B.stats_to_host(sbuf)
+    assert s.n_uniform_pg == 3
+    assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+    assert np.array_equal(gflux.cpu().numpy(), wflux, equal_nan=True)
+    assert s.algorithm_dict() == st.as_dict()
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, pe, exact=True)  # without flux output
+    assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+    assert B.stats_to_host(sbuf).algorithm_dict() == st.as_dict()
+    # production build: the uniform tiles reproduce their input bit for bit, the rest to the step tolerance
+    got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, dh, B.params(recon, riemann))
+    s = B.stats_to_host(sbuf)
+    got = got.cpu().numpy()
+    assert s.n_uniform_pg == 3
+    assert np.array_equal(got[:3], want[:3])
+    assert step_err(got[:6], want[:6], 2).max() <= TOL_STEP
+    fscale = np.abs(wflux[:3]).max(axis=(1, 2, 3, 4, 5), keepdims=True)
+    assert (np.abs(gflux.cpu().numpy()[:3] - wflux[:3]) / fscale).max() <= 1e-13
+    assert (s.n_retry_pg, s.n_passes) == (st.n_retry_pg, st.n_passes)
