@@ -222,6 +222,24 @@ int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int 
                             const unsigned char* inflow_mask, const double* inflow_cons,
                             const srhd_params* params, double* d_max_speed, void* stream);
 
+/* One whole step of a uniform grid kept in the patch layout: srhd_patch_gather_speed + srhd_fluid_step_cfl behind
+ * one call, with the uniform-tile test done on the way (same results, bit for bit, as the two calls).
+ *   patches_in : device, [npg][8][5][8][8][8], the current state (cons_out of the previous step)
+ *   patches_out: device, same shape, the new state; must not be patches_in (neighbouring groups still read it)
+ *   cons_in    : device scratch for the ghosted tiles, [npg][5][nxt]^3, nxt = 16 + 2*params->ghost; only the
+ *                tiles of groups that are not uniform are written
+ *   flux_out   : as srhd_fluid_step_fluxes, may be NULL
+ *   d_max_speed: device, one double: receives S_max of the CURRENT state (Eq. 26-27); the step then uses
+ *                dt = cfl * dh / max(S_max, min_speed) (Eq. 28) without a host round trip
+ * A patch group whose whole tile (ghost zones after the boundary mapping included) holds one state bit for bit is
+ * finished by the first kernel: its new patches are its old ones (srhd_stats.n_uniform_pg counts them), so its
+ * state crosses HBM once in and once out and no tile is materialised for it; every other group goes through
+ * fluid_step_kernel as in srhd_fluid_step_cfl.  Boundary arguments as srhd_grid_gather; errors as the two calls. */
+int srhd_grid_step_cfl(const double* patches_in, double* patches_out, double* cons_in, double* flux_out,
+                       int nx, int ny, int nz, const int* bc, const unsigned char* inflow_mask,
+                       const double* inflow_cons, double cfl, double dh, double min_speed,
+                       const srhd_params* params, srhd_stats* stats, double* d_max_speed, void* stream);
+
 /* Measurement helper (not part of the solver): launches a register-only DFMA loop that fills every
  * fp64 lane of the GPU (148 x 8 CTAs x 256 threads, 32*iters dependent-chain DFMA per thread in 8
  * independent chains) on `stream`; *flops (HOST pointer, may be NULL) receives the flop count of the

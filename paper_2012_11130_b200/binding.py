@@ -45,7 +45,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_flux_correction", "srhd_ghost_interp", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed",
+           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_flux_correction", "srhd_ghost_interp", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed", "srhd_grid_step_cfl",
            "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact"]
 
 _LIBS = {}
@@ -96,6 +96,10 @@ def load_library(exact=False):
     L.srhd_patch_gather_speed.restype = C.c_int
     L.srhd_patch_gather_speed.argtypes = [_VP, _VP, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), _VP,
                                           C.POINTER(C.c_double), C.POINTER(Params), _VP, _VP]
+    L.srhd_grid_step_cfl.restype = C.c_int
+    L.srhd_grid_step_cfl.argtypes = [_VP, _VP, _VP, _VP, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), _VP,
+                                     C.POINTER(C.c_double), C.c_double, C.c_double, C.c_double, C.POINTER(Params),
+                                     _VP, _VP, _VP]
     L.srhd_fp64_peak_probe.restype = C.c_int
     L.srhd_fp64_peak_probe.argtypes = [_VP, C.c_int, C.POINTER(C.c_ulonglong), _VP]
     L.srhd_issue_probe.restype = C.c_int
@@ -355,6 +359,35 @@ def patch_gather_speed(patches, shape, par, bc, inflow=None, cons_in=None, out=N
     _check(L.srhd_patch_gather_speed(patches.data_ptr(), cons_in.data_ptr(), nx, ny, nz, _bc(bc), mask_ptr, icons,
                                      C.byref(par), out.data_ptr(), _stream()), L)
     return cons_in, out
+
+
+def grid_step_cfl(patches_in, patches_out, cons_in, shape, cfl, dh, par, bc, inflow=None, min_speed=0.0,
+                  flux_out=None, stats=None, out=None, exact=False):
+    """srhd_grid_step_cfl: one whole step of a uniform grid in the patch layout (patches_in -> patches_out);
+    cons_in is the tile scratch (npg,5,nxt,nxt,nxt); returns (patches_out, S_max tensor, stats)."""
+    L = load_library(exact)
+    patches_in, patches_out, cons_in = _dev(patches_in, "patches_in"), _dev(patches_out, "patches_out"), _dev(cons_in, "cons_in")
+    nz, ny, nx = shape
+    npg = (nx // 16) * (ny // 16) * (nz // 16)
+    nxt = 16 + 2 * par.ghost
+    if tuple(patches_in.shape) != (npg, 8, 5, 8, 8, 8) or tuple(patches_out.shape) != (npg, 8, 5, 8, 8, 8):
+        raise SrhdError(f"patches must have shape ({npg}, 8, 5, 8, 8, 8)")
+    if tuple(cons_in.shape) != (npg, 5, nxt, nxt, nxt):
+        raise SrhdError(f"cons_in must have shape ({npg}, 5, {nxt}, {nxt}, {nxt})")
+    if flux_out is not None and tuple(_dev(flux_out, "flux_out").shape) != (npg, 8, 6, 5, 8, 8):
+        raise SrhdError(f"flux_out must have shape ({npg}, 8, 6, 5, 8, 8)")
+    out = torch.empty(1, dtype=torch.float64, device=patches_in.device) if out is None else out
+    stats = new_stats(patches_in.device) if stats is None else stats
+    mask_ptr, icons = None, None
+    if inflow is not None:
+        mask, vals = inflow
+        mask_ptr = mask.data_ptr()
+        icons = (C.c_double * 5)(*[float(v) for v in vals])
+    _check(L.srhd_grid_step_cfl(patches_in.data_ptr(), patches_out.data_ptr(), cons_in.data_ptr(),
+                                None if flux_out is None else flux_out.data_ptr(), nx, ny, nz, _bc(bc), mask_ptr,
+                                icons, float(cfl), float(dh), float(min_speed), C.byref(par), stats.data_ptr(),
+                                out.data_ptr(), _stream()), L)
+    return patches_out, out, stats
 
 
 def fp64_peak_probe(iters=4096, reps=5):

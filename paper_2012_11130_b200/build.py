@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = ["srhd_convert.cu", "srhd_fluid.cu", "srhd_grid.cu", "srhd_refine.cu", "srhd_vl.cu", "srhd_amr.cu"]
-HEADERS = ["srhd_math.cuh", "srhd_common.cuh", os.path.join("..", "..", "include", "srhd.h")]
+HEADERS = ["srhd_math.cuh", "srhd_common.cuh", "srhd_uniform.cuh", os.path.join("..", "..", "include", "srhd.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared"]
 VARIANTS = {

@@ -19,6 +19,7 @@
 // beta <- 0.75 beta, finally with beta = 0.  Each cell's state crosses HBM once on the way
 // in (plus ghost layers) and once on the way out; the update re-reads its own cell through L2.
 #include "srhd_common.cuh"
+#include "srhd_uniform.cuh"
 
 namespace srhd {
 
@@ -151,18 +152,13 @@ SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
   return false;
 }
 
-// Uniform tiles (undisturbed ambient gas ahead of a blast wave or a jet): every cell of the tile, ghost zones
-// included, holds the same five doubles bit for bit.  Then the whole algorithm collapses to values that
-// one thread can form: W0 = C2P(U0) for every tile cell; all slopes vanish, so every edge state is
-// U1 = P2C(W0) and every flux difference of the half step is +0 (U1 + (-0) = U1); every face solves the same
-// Riemann problem F_d(U1, U1); every update is U0 - dt/dh ((F-F) + (F-F) + (F-F)) = U0.  This pre-pass (one
-// CTA per patch group, launched ahead of fluid_step_kernel on the same stream) streams such a tile once from
-// HBM (16-byte loads, compared as bit patterns), writes the 8 patches, adds what the march would have counted
-// to the counters and sets handled[pg] = 1, which makes the main kernel's CTA return at once.  Anything unusual
-// (a state that fails Eq. 30, a non-finite flux) is left to the main kernel; a tile that is not uniform is
-// dropped at its first 4 KB.  It is a kernel of its own, not a branch of the main one: a data-dependent early
-// exit there makes nvcc guard every warp collective of the march with a divergence test (BRA.DIV; measured
-// +25 % kernel time on data without a single uniform tile).
+// Uniform tiles (undisturbed ambient gas ahead of a blast wave or a jet; srhd_uniform.cuh): this pre-pass (one
+// CTA per patch group, launched ahead of fluid_step_kernel on the same stream) streams a tile once from HBM
+// (16-byte loads, compared as bit patterns); if every cell holds the same state it writes the 8 patches, adds
+// what the march would have counted to the counters and sets handled[pg] = 1, which makes the main kernel's CTA
+// return at once.  A tile that is not uniform is dropped at its first 4 KB.  It is a kernel of its own, not a
+// branch of the main one: a data-dependent early exit there makes nvcc guard every warp collective of the march
+// with a divergence test (BRA.DIV; measured +25 % kernel time on data without a single uniform tile).
 constexpr int kScanThreads = 256;
 template <int G, int RS>
 __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
@@ -175,8 +171,6 @@ __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
   static_assert(T3 % 2 == 0, "tile components must be whole 16-byte words");
   const int tid = threadIdx.x;
   const double* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
-  double* __restrict__ out = cons_out + (size_t)blockIdx.x * 8 * 5 * 512;
-  double* __restrict__ fout = flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr;
   if (tid == 0) handled[blockIdx.x] = 0;
   const double2* __restrict__ t2 = reinterpret_cast<const double2*>(tile);
   unsigned long long ref[5];
@@ -202,53 +196,17 @@ __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
     if (__syncthreads_or(diff ? 1 : 0)) return;
   }
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);      // as the main kernel (srhd_fluid_step_cfl)
-  const double dtdh = dt / dh;
-  double U0[1][5], W0[1][5], U1[1][5], W1[1][5], F[3][5];
+  if (!(fabs(dt / dh) <= DBL_MAX)) return;                   // U0 - (dt/dh) 0 = U0 needs a finite dt/dh
+  double U0[5];
 #pragma unroll
-  for (int q = 0; q < 5; ++q) U0[0][q] = __longlong_as_double((long long)ref[q]);
-  bool ph0[1], ph1[1];
-  int it0[1], it1[1];
-  Aux a0[1], a1[1], ae;
-  cons2prim_multi<1>(U0, W0, a0, rtol, max_iter, ph0, it0);
-  prim2cons_aux(W0[0], U1[0], ae);
-  cons2prim_multi<1>(U1, W1, a1, rtol, max_iter, ph1, it1);
-  bool ok = ph0[0] && ph1[0] && is_physical(U0[0]) && (fabs(dtdh) <= DBL_MAX);
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    riemann_flux<RS>(d, W1[0], U1[0], a1[0], W1[0], U1[0], a1[0], F[d], true);
-#pragma unroll
-    for (int q = 0; q < 5; ++q) ok = ok && (fabs(F[d][q]) <= DBL_MAX);
-  }
-  if (!ok) return;                                           // every thread computed the same verdict
-  double2* __restrict__ o2 = reinterpret_cast<double2*>(out);
-  for (int w = tid; w < 8 * 5 * 256; w += NT) {              // out[patch][component][512]
-    const int q = (w >> 8) % 5;
-    const double u = (q == 0) ? U0[0][0] : (q == 1) ? U0[0][1] : (q == 2) ? U0[0][2] : (q == 3) ? U0[0][3] : U0[0][4];
-    o2[w] = make_double2(u, u);
-  }
-  if (fout) {
-    for (int w = tid; w < 8 * 6 * 5 * 64; w += NT) {         // flux_out[patch][face][component][64]
-      const int q = (w >> 6) % 5, d = ((w / 320) % 6) >> 1;
-      double f = 0.0;
-#pragma unroll
-      for (int dd = 0; dd < 3; ++dd)
-#pragma unroll
-        for (int qq = 0; qq < 5; ++qq) f = (dd == d && qq == q) ? F[dd][qq] : f;
-      fout[w] = f;
-    }
-  }
+  for (int q = 0; q < 5; ++q) U0[q] = __longlong_as_double((long long)ref[q]);
+  UniformResult r;
+  if (!uniform_eval<RS>(U0, rtol, max_iter, r)) return;      // every thread computed the same verdict
+  uniform_write(cons_out + (size_t)blockIdx.x * 8 * 5 * 512,
+                flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr, U0, r, tid, NT);
   if (tid == 0) {
     handled[blockIdx.x] = 1;
-    if (stats) {
-      atomicAdd(&stats->newton_iters, (unsigned long long)T3 * (unsigned)it0[0] +
-                                          (unsigned long long)(2 * 3 * 17 * 256) * (unsigned)it1[0]);
-      atomicAdd(&stats->n_passes, 1ull);
-      atomicAdd(&stats->exec_newton, (unsigned long long)(it0[0] + it1[0]));
-      atomicAdd(&stats->exec_c2p, 2ull);
-      atomicAdd(&stats->exec_riemann, SRHD_EXACT ? 3ull : 0ull);
-      atomicAdd(&stats->n_uniform_pg, 1ull);
-      atomic_max_nonneg(&stats->max_speed, smax_of_umax(umax_of_prim(W0[0], a0[0])));
-    }
+    uniform_count(stats, T3, r);
   }
 }
 
@@ -683,26 +641,43 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   }
 }
 
+// handled == nullptr: run the uniform-tile pre-pass first (flags in a stream-ordered scratch allocation);
+// else the caller has run a pre-pass of its own and only the march is launched
 template <int G, int RS>
 int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
                  const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-                 double min_speed) {
+                 double min_speed, const unsigned char* handled) {
   auto kern = fluid_step_kernel<G, RS>;
   const size_t smem = Plan<G>::bytes;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
-  // one byte per patch group between the two kernels, allocated and freed in stream order
-  unsigned char* handled = nullptr;
-  e = cudaMallocAsync(reinterpret_cast<void**>(&handled), (size_t)npg, st);
-  if (e != cudaSuccess) return (int)e;
   const double rtol = newton_stop_rtol(p->newton_rtol);
-  uniform_tiles_kernel<G, RS><<<npg, kScanThreads, 0, st>>>(cons_in, cons_out, flux_out, dt, dh, rtol,
-                                                            p->newton_max_iter, stats, d_smax, cfl, min_speed, handled);
+  unsigned char* scratch = nullptr;
+  if (!handled) {
+    e = cudaMallocAsync(reinterpret_cast<void**>(&scratch), (size_t)npg, st);
+    if (e != cudaSuccess) return (int)e;
+    uniform_tiles_kernel<G, RS><<<npg, kScanThreads, 0, st>>>(cons_in, cons_out, flux_out, dt, dh, rtol,
+                                                              p->newton_max_iter, stats, d_smax, cfl, min_speed, scratch);
+    handled = scratch;
+  }
   kern<<<npg, kFluidThreads, smem, st>>>(cons_in, cons_out, flux_out, dt, dh, p->minmod_coeff, p->max_retry, rtol,
                                          p->newton_max_iter, stats, d_smax, cfl, min_speed, handled);
   e = cudaGetLastError();
-  const cudaError_t e2 = cudaFreeAsync(handled, st);
+  const cudaError_t e2 = scratch ? cudaFreeAsync(scratch, st) : cudaSuccess;
   return (int)(e != cudaSuccess ? e : e2);
+}
+
+int fluid_march(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
+                const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
+                double min_speed, const unsigned char* handled) {
+  if (p->recon == SRHD_RECON_PLM) {
+    return p->riemann == SRHD_RIEMANN_HLLE
+               ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, p, stats, st, d_smax, cfl, min_speed, handled)
+               : launch_fluid<2, 1>(cons_in, cons_out, flux_out, npg, dt, dh, p, stats, st, d_smax, cfl, min_speed, handled);
+  }
+  return p->riemann == SRHD_RIEMANN_HLLE
+             ? launch_fluid<3, 0>(cons_in, cons_out, flux_out, npg, dt, dh, p, stats, st, d_smax, cfl, min_speed, handled)
+             : launch_fluid<3, 1>(cons_in, cons_out, flux_out, npg, dt, dh, p, stats, st, d_smax, cfl, min_speed, handled);
 }
 
 }  // namespace srhd
@@ -745,14 +720,7 @@ static int fluid_step_impl(const double* cons_in, double* cons_out, double* flux
   if (npg == 0) return SRHD_OK;
   if (params->integrator == SRHD_INTEGRATOR_VL)
     return vl_step(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed);
-  if (params->recon == SRHD_RECON_PLM) {
-    return params->riemann == SRHD_RIEMANN_HLLE
-               ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed)
-               : launch_fluid<2, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed);
-  }
-  return params->riemann == SRHD_RIEMANN_HLLE
-             ? launch_fluid<3, 0>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed)
-             : launch_fluid<3, 1>(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed);
+  return fluid_march(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed, nullptr);
 }
 
 extern "C" int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,

@@ -2,6 +2,7 @@
 // the scatter of updated patches back to the grid.  They stand in for the AMR driver's ghost-zone
 // preparation, are pure data movement (no arithmetic) and are timed as part of a step.
 #include "srhd_common.cuh"
+#include "srhd_uniform.cuh"
 
 namespace srhd {
 
@@ -201,6 +202,122 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* _
   if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax_out, umax);
 }
 
+// One whole step of a uniform grid kept in the patch layout, first kernel (srhd_grid_step_cfl): patch_gather_speed_kernel
+// with the uniform-tile test of srhd_uniform.cuh in front of it.  Phase 1 reads the (16+2g)^3 tile cells of the
+// group from the source patches WITHOUT writing them and compares them, as bit patterns, with the group's first
+// cell (it stops at the first chunk that shows a difference).  A uniform group is finished here: its 8 patches
+// of the NEW state are the old ones (srhd_uniform.cuh), written straight to patches_out, its counters and its
+// U_max come from one conversion, handled[pg] = 1 -- the state of such a group crosses HBM once in and once out
+// and no tile is ever materialised.  Any other group gets its tile and the U_max of its 4096 cells exactly as
+// patch_gather_speed_kernel does it, and handled[pg] = 0 leaves it to fluid_step_kernel.
+template <int G, int RS>
+__global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __restrict__ patches,
+                                                            double* __restrict__ patches_out,
+                                                            double* __restrict__ cons_in,
+                                                            double* __restrict__ flux_out, int nx, int ny, int nz,
+                                                            GridBC b, const unsigned char* __restrict__ mask,
+                                                            double rtol, int max_iter, double* __restrict__ umax_out,
+                                                            srhd_stats* __restrict__ stats,
+                                                            unsigned char* __restrict__ handled) {
+  constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
+  __shared__ int ax[nxt], ay[nxt], mx[nxt], my[nxt];
+  __shared__ long long az[nxt];               // -1 - offset for a plane below z = 0 of an inflow boundary
+  const int px = nx / 16, py = ny / 16;
+  const int pg = blockIdx.x, tid = threadIdx.x;
+  const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
+  if (tid < nxt) {
+    const int t = tid;
+    const int X = map_index(gx * 16 + t - G, nx, b.bc[0], b.bc[1]);
+    const int Y = map_index(gy * 16 + t - G, ny, b.bc[2], b.bc[3]);
+    const int kk = gz * 16 + t - G;
+    const int Z = map_index(kk, nz, b.bc[4], b.bc[5]);
+    ax[t] = (X >> 4) * 20480 + ((X >> 3) & 1) * 2560 + (X & 7);
+    ay[t] = (Y >> 4) * px * 20480 + ((Y >> 3) & 1) * 2 * 2560 + (Y & 7) * 8;
+    mx[t] = X;
+    my[t] = Y * nx;
+    const long long off = (long long)(Z >> 4) * px * py * 20480 + ((Z >> 3) & 1) * 4 * 2560 + (Z & 7) * 64;
+    az[t] = (b.has_inflow && kk < 0) ? -1 - off : off;
+  }
+  if (tid == 0) handled[pg] = 0;
+  __syncthreads();
+  const double* __restrict__ own = patches + (size_t)pg * 8 * 5 * 512;
+  // the five doubles of tile cell c as the gather would write them
+  auto tile_cell = [&](int c, double v[5]) {
+    const int k = c / nrow, r = c - k * nrow, j = r / nxt, i = r - j * nxt;
+    long long z = az[k];
+    bool inflow = false;
+    if (z < 0) {
+      z = -1 - z;
+      inflow = mask[my[j] + mx[i]] != 0;
+    }
+    const double* __restrict__ sp = patches + z + ay[j] + ax[i];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) v[q] = inflow ? b.inflow[q] : __ldg(sp + q * 512);
+  };
+  // ---- phase 1: is the tile one state?
+  double U0[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U0[q] = __ldg(own + q * 512);
+  bool uniform = true;
+  for (int c0 = tid; c0 < t3; c0 += 2 * 256) {
+    double v[2][5];
+    bool diff = false;
+#pragma unroll
+    for (int u = 0; u < 2; ++u) tile_cell(min(c0 + u * 256, t3 - 1), v[u]);
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
+#pragma unroll
+      for (int q = 0; q < 5; ++q) diff = diff || (__double_as_longlong(v[u][q]) != __double_as_longlong(U0[q]));
+    if (__syncthreads_or(diff ? 1 : 0)) {
+      uniform = false;
+      break;
+    }
+  }
+  if (uniform) {
+    UniformResult r;
+    if (uniform_eval<RS>(U0, rtol, max_iter, r)) {           // every thread computed the same verdict
+      uniform_write(patches_out + (size_t)pg * 8 * 5 * 512,
+                    flux_out ? flux_out + (size_t)pg * 8 * 6 * 5 * 64 : nullptr, U0, r, tid, 256);
+      if (tid == 0) {
+        handled[pg] = 1;
+        uniform_count(stats, t3, r);
+        atomic_max_nonneg(umax_out, r.umax);
+      }
+      return;
+    }
+  }
+  // ---- phase 2 (any other group): the tile and U_max of the group's own cells, as patch_gather_speed_kernel
+  double* __restrict__ dst = cons_in + (size_t)pg * 5 * t3;
+  for (int c0 = tid; c0 < t3; c0 += 2 * 256) {
+    double v[2][5];
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
+      if (c0 + u * 256 < t3) tile_cell(c0 + u * 256, v[u]);
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int c = c0 + u * 256;
+      if (c < t3) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) dst[(size_t)q * t3 + c] = v[u][q];
+      }
+    }
+  }
+  double umax = 0.0;
+  for (int c = tid; c < 4096; c += 256) {
+    const size_t so = (size_t)(c >> 9) * 5 * 512 + (c & 511);
+    double U[1][5], W[1][5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) U[0][q] = __ldg(own + so + (size_t)q * 512);
+    bool phys[1];
+    int it[1];
+    Aux aux[1];
+    cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
+    umax = fmax(umax, umax_of_prim(W[0], aux[0]));
+  }
+  umax = warp_max(umax);
+  if ((tid & 31) == 0) atomic_max_nonneg(umax_out, umax);
+}
+
 __global__ void smax_finish_kernel2(double* v) { *v = smax_of_umax(*v); }   // Eq. 27 once, after the max
 
 }  // namespace srhd
@@ -298,6 +415,75 @@ extern "C" int srhd_patch_gather_speed(const double* patches, double* cons_in, i
                                                       params->newton_max_iter, d_max_speed);
   smax_finish_kernel2<<<1, 1, 0, st>>>(d_max_speed);
   return (int)cudaGetLastError();
+}
+
+template <int G, int RS>
+static void launch_prepass(const double* patches, double* patches_out, double* cons_in, double* flux_out, int nx,
+                           int ny, int nz, const GridBC& b, const unsigned char* mask, double rtol, int max_iter,
+                           double* umax_out, srhd_stats* stats, unsigned char* handled, cudaStream_t st) {
+  const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  patch_prepass_kernel<G, RS><<<npg, 256, 0, st>>>(patches, patches_out, cons_in, flux_out, nx, ny, nz, b, mask, rtol,
+                                                   max_iter, umax_out, stats, handled);
+}
+
+extern "C" int srhd_grid_step_cfl(const double* patches_in, double* patches_out, double* cons_in, double* flux_out,
+                                  int nx, int ny, int nz, const int* bc, const unsigned char* inflow_mask,
+                                  const double* inflow_cons, double cfl, double dh, double min_speed,
+                                  const srhd_params* params, srhd_stats* stats, double* d_max_speed, void* stream) {
+  if (!patches_in || !patches_out || !cons_in || !bc || !d_max_speed) return SRHD_ERR_NULL_POINTER;
+  const int pc = check_params(params);
+  if (pc) return pc;
+  const int ce = check_extents(nx, ny, nz);
+  if (ce) return ce;
+  if (!(cfl > 0.0) || !std::isfinite(cfl) || !(min_speed >= 0.0) || !(dh > 0.0) || !std::isfinite(dh))
+    return SRHD_ERR_BAD_STEP;
+  if (patches_in == patches_out) return SRHD_ERR_ALIAS;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  if (params->integrator != SRHD_INTEGRATOR_MHM) {           // no pre-pass for the VL kernels: the two plain calls
+    const int e = srhd_patch_gather_speed(patches_in, cons_in, nx, ny, nz, bc, inflow_mask, inflow_cons, params,
+                                          d_max_speed, stream);
+    if (e) return e;
+    return srhd_fluid_step_cfl(cons_in, patches_out, flux_out, npg, cfl, dh, d_max_speed, min_speed, params, stats,
+                               stream);
+  }
+  GridBC b;
+  for (int i = 0; i < 6; ++i) {
+    if (bc[i] != SRHD_BC_PERIODIC && bc[i] != SRHD_BC_OUTFLOW) return SRHD_ERR_BAD_PARAMS;
+    b.bc[i] = bc[i];
+  }
+  b.has_inflow = (inflow_mask != nullptr);
+  if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
+  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
+  cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(double), st);
+  if (e != cudaSuccess) return (int)e;
+  if (stats) {
+    e = cudaMemsetAsync(stats, 0, sizeof(srhd_stats), st);
+    if (e != cudaSuccess) return (int)e;
+  }
+  unsigned char* handled = nullptr;
+  e = cudaMallocAsync(reinterpret_cast<void**>(&handled), (size_t)npg, st);
+  if (e != cudaSuccess) return (int)e;
+  const double rtol = newton_stop_rtol(params->newton_rtol);
+  const int mi = params->newton_max_iter;
+  if (params->recon == SRHD_RECON_PLM) {
+    if (params->riemann == SRHD_RIEMANN_HLLE)
+      launch_prepass<2, 0>(patches_in, patches_out, cons_in, flux_out, nx, ny, nz, b, inflow_mask, rtol, mi, d_max_speed, stats, handled, st);
+    else
+      launch_prepass<2, 1>(patches_in, patches_out, cons_in, flux_out, nx, ny, nz, b, inflow_mask, rtol, mi, d_max_speed, stats, handled, st);
+  } else {
+    if (params->riemann == SRHD_RIEMANN_HLLE)
+      launch_prepass<3, 0>(patches_in, patches_out, cons_in, flux_out, nx, ny, nz, b, inflow_mask, rtol, mi, d_max_speed, stats, handled, st);
+    else
+      launch_prepass<3, 1>(patches_in, patches_out, cons_in, flux_out, nx, ny, nz, b, inflow_mask, rtol, mi, d_max_speed, stats, handled, st);
+  }
+  smax_finish_kernel2<<<1, 1, 0, st>>>(d_max_speed);
+  e = cudaGetLastError();
+  int rc = (int)e;
+  if (e == cudaSuccess)
+    rc = fluid_march(cons_in, patches_out, flux_out, npg, 1.0, dh, params, stats, st, d_max_speed, cfl, min_speed, handled);
+  const cudaError_t e2 = cudaFreeAsync(handled, st);
+  return rc ? rc : (int)e2;
 }
 
 extern "C" void srhd_default_params(srhd_params* p, int recon, int riemann) {

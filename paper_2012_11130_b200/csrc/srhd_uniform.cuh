@@ -1,0 +1,87 @@
+// srhd_uniform.cuh -- what one step does to a patch group whose whole tile (ghost zones included) holds ONE
+// state U0 bit for bit, shared by the two pre-passes that look for such tiles (uniform_tiles_kernel in
+// srhd_fluid.cu: tiles already gathered; patch_prepass_kernel in srhd_grid.cu: straight from the patches).
+//
+// The algorithm of srhd_fluid_step collapses (readings S3-S7, S12): W0 = C2P(U0) for every tile cell; all
+// slopes vanish, so every edge state is U1 = P2C(W0) and every flux difference of the half step is +0
+// (U1 + (-0) = U1); every face solves the same Riemann problem F_d(U1, U1); every update is
+// U0 - dt/dh ((F-F) + (F-F) + (F-F)) = U0 for any finite dt.  Anything unusual (a state that fails Eq. 30, a
+// non-finite flux) makes uniform_eval return false and the group takes the general march.
+#pragma once
+#include "srhd_common.cuh"
+
+namespace srhd {
+
+struct UniformResult {
+  int it0, it1;       // Newton-Raphson iterations of C2P(U0) and C2P(U1)
+  double umax;        // Eq. 26 of W0
+  double F[3][5];     // the Riemann flux of (U1, U1) along x, y, z
+};
+
+// every thread of the CTA calls this with the same U0 (the warp votes inside cons2prim_multi need whole warps)
+template <int RS>
+SRHD_DEV bool uniform_eval(const double U0in[5], double rtol, int max_iter, UniformResult& r) {
+  double U0[1][5], W0[1][5], U1[1][5], W1[1][5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U0[0][q] = U0in[q];
+  bool ph0[1], ph1[1];
+  int it0[1], it1[1];
+  Aux a0[1], a1[1], ae;
+  cons2prim_multi<1>(U0, W0, a0, rtol, max_iter, ph0, it0);
+  prim2cons_aux(W0[0], U1[0], ae);
+  cons2prim_multi<1>(U1, W1, a1, rtol, max_iter, ph1, it1);
+  bool ok = ph0[0] && ph1[0] && is_physical(U0[0]);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    riemann_flux<RS>(d, W1[0], U1[0], a1[0], W1[0], U1[0], a1[0], r.F[d], true);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) ok = ok && (fabs(r.F[d][q]) <= DBL_MAX);
+  }
+  r.it0 = it0[0];
+  r.it1 = it1[0];
+  r.umax = umax_of_prim(W0[0], a0[0]);
+  return ok;
+}
+
+// the 8 patches of the group (out[patch][component][512]) and, if asked for, the patch-boundary fluxes
+// (fout[patch][face][component][64]); NT threads, thread tid
+SRHD_DEV void uniform_write(double* __restrict__ out, double* __restrict__ fout, const double U0[5],
+                            const UniformResult& r, int tid, int NT) {
+  double2* __restrict__ o2 = reinterpret_cast<double2*>(out);
+  for (int w = tid; w < 8 * 5 * 256; w += NT) {
+    const int q = (w >> 8) % 5;
+    const double u = (q == 0) ? U0[0] : (q == 1) ? U0[1] : (q == 2) ? U0[2] : (q == 3) ? U0[3] : U0[4];
+    o2[w] = make_double2(u, u);
+  }
+  if (fout) {
+    for (int w = tid; w < 8 * 6 * 5 * 64; w += NT) {
+      const int q = (w >> 6) % 5, d = ((w / 320) % 6) >> 1;
+      double f = 0.0;
+#pragma unroll
+      for (int dd = 0; dd < 3; ++dd)
+#pragma unroll
+        for (int qq = 0; qq < 5; ++qq) f = (dd == d && qq == q) ? r.F[dd][qq] : f;
+      fout[w] = f;
+    }
+  }
+}
+
+// what the march would have counted for this group (one thread); tile_cells = (16 + 2 ghost)^3
+SRHD_DEV void uniform_count(srhd_stats* __restrict__ stats, int tile_cells, const UniformResult& r) {
+  if (!stats) return;
+  atomicAdd(&stats->newton_iters, (unsigned long long)tile_cells * (unsigned)r.it0 +
+                                      (unsigned long long)(2 * 3 * 17 * 256) * (unsigned)r.it1);
+  atomicAdd(&stats->n_passes, 1ull);
+  atomicAdd(&stats->exec_newton, (unsigned long long)(r.it0 + r.it1));
+  atomicAdd(&stats->exec_c2p, 2ull);
+  atomicAdd(&stats->exec_riemann, SRHD_EXACT ? 3ull : 0ull);
+  atomicAdd(&stats->n_uniform_pg, 1ull);
+  atomic_max_nonneg(&stats->max_speed, smax_of_umax(r.umax));
+}
+
+// srhd_fluid.cu: the march alone, for patch groups whose handled[] byte is 0 (the caller ran a pre-pass)
+int fluid_march(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
+                const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
+                double min_speed, const unsigned char* handled);
+
+}  // namespace srhd

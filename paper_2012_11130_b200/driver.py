@@ -2,12 +2,15 @@
 
 The state lives in the PATCH layout the solver writes (cons_out of srhd_fluid_step: 8^3 patches, as in
 the paper's AMR code); a uniform grid (5, nz, ny, nx) is only materialised when it is asked for.
-One step (collapsed onto the GPU), 3 launches:
+One step (collapsed onto the GPU):
     srhd_patch_gather_speed(patches) -> tiles, S_max   ghost-zone fill of every 16^3 patch group from the
                                                        neighbouring patches (stands in for P:219) fused
                                                        with the CFL reduction of that state (Eq. 26-27)
     srhd_fluid_step_cfl(tiles) -> patches              the fused MUSCL-Hancock update with
                                                        dt = C dh / S_max formed on the device (Eq. 28)
+step_async() issues both behind ONE call, srhd_grid_step_cfl (3 launches, patches double buffered), whose first
+kernel also finishes the patch groups that hold a single state (their new patches are their old ones) without
+ever materialising their tiles; fused=False keeps the two separate calls (same results bit for bit).
 The first step after set_prim / set_cons starts from the grid instead: srhd_max_signal_speed +
 srhd_grid_gather.  step() reads S_max back (one double) because the host wants t; step_async() does not
 synchronise.  Nothing here computes on the host except that scalar arithmetic; all buffers are torch
@@ -23,7 +26,7 @@ class GridStepper:
     """Owns the device buffers of one uniform grid of conserved variables."""
 
     def __init__(self, shape, dh, bc, recon="plm", riemann="hllc", cfl=0.4, inflow=None, exact=False,
-                 device="cuda", dt_speed="signal", **par_overrides):
+                 device="cuda", dt_speed="signal", fused=True, **par_overrides):
         nz, ny, nx = shape
         if nx % 16 or ny % 16 or nz % 16:
             raise B.SrhdError("grid extents must be multiples of 16 (whole patch groups)")
@@ -32,6 +35,7 @@ class GridStepper:
         if dt_speed not in ("signal", "light"):
             raise B.SrhdError("dt_speed must be 'signal' (Eq. 26-28) or 'light' (S_max replaced by c, P:229)")
         self.dt_speed = dt_speed
+        self.fused = bool(fused)   # step_async() through srhd_grid_step_cfl (False: the two separate calls)
         self.npg = (nx // 16) * (ny // 16) * (nz // 16)
         self.ncell = nx * ny * nz
         nxt = 16 + 2 * self.par.ghost
@@ -39,6 +43,7 @@ class GridStepper:
         self._grid = torch.empty((5, nz, ny, nx), **f64)
         self.tiles = torch.empty((self.npg, 5, nxt, nxt, nxt), **f64)
         self.patches = torch.empty((self.npg, 8, 5, 8, 8, 8), **f64)
+        self._patches_b = None    # second patch buffer, allocated by the first fused step (srhd_grid_step_cfl)
         self.smax = torch.zeros(1, **f64)
         self.stats = B.new_stats(device)
         self.inflow = None
@@ -56,7 +61,9 @@ class GridStepper:
         self.nstep = 0
         self._in_patches = False   # True: self.patches holds the current state (self._grid may be stale)
         self._grid_stale = False
-        self.launches_per_step = 3   # ghost-zone fill (+ speed), smax finish (signal) or plain gather, fluid step
+        # fused: pre-pass (ghost-zone fill + speed + uniform tiles), smax finish, march; else gather + speed, smax
+        # finish, uniform-tile scan, march
+        self.launches_per_step = 3 if self.fused else 4
 
     # ---- state in / out -------------------------------------------------------------------------
     @property
@@ -144,6 +151,16 @@ class GridStepper:
         the time matters."""
         if self.dt_speed == "light":
             return self.advance(self.cfl * self.dh, kernel_events)
+        if self._in_patches and self.fused:
+            # the whole step behind one call: uniform patch groups are finished by its first kernel straight
+            # from the patches (no tile), the others are gathered and marched; patches are double buffered
+            if self._patches_b is None:
+                self._patches_b = torch.empty_like(self.patches)
+            self._timed(kernel_events, lambda: B.grid_step_cfl(
+                self.patches, self._patches_b, self.tiles, self.shape, self.cfl, self.dh, self.par, self.bc,
+                self.inflow, min_speed=self.smax_inflow, stats=self.stats, out=self.smax, exact=self.exact))
+            self.patches, self._patches_b = self._patches_b, self.patches
+            return self._done()
         self._fill_tiles(need_speed=True)
         self._timed(kernel_events, lambda: B.fluid_step_cfl(self.tiles, self.cfl, self.dh, self.smax, self.par,
                                                             min_speed=self.smax_inflow, cons_out=self.patches,
