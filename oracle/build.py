@@ -14,7 +14,12 @@ HDR = [os.path.join(HERE, "srhd_ref.hpp")]
 # "fma": the SAME source with the compiler free to contract a*b+c into fused multiply-adds -- a second, equally
 # legitimate IEEE rounding of the same formulas.  Tests use it to measure how far two correct fp64 evaluations
 # of this algorithm drift apart (tests/test_gpu_configs.py); it is never the parity reference.
-VARIANTS = {"": ["-ffp-contract=off"], "fma": ["-ffp-contract=fast", "-mfma"]}
+# "gamma53" / "gamma43": the polytropic EoS of P:107 Eq. 11 with Gamma = 5/3 / 4/3; "orig": the paper's "original scheme"
+# (evolve the total energy E) for the A/B runs of Fig. 3 / Fig. 16 (srhd_ref.cpp header).
+VARIANTS = {"": ["-ffp-contract=off"], "fma": ["-ffp-contract=fast", "-mfma"],
+            "gamma53": ["-ffp-contract=off", "-DSRHD_REF_EOS=1", "-DSRHD_REF_GAMMA_NUM=5", "-DSRHD_REF_GAMMA_DEN=3"],
+            "gamma43": ["-ffp-contract=off", "-DSRHD_REF_EOS=1", "-DSRHD_REF_GAMMA_NUM=4", "-DSRHD_REF_GAMMA_DEN=3"],
+            "orig": ["-ffp-contract=off", "-DSRHD_REF_SCHEME=1"]}
 
 
 def lib_path(variant=""):

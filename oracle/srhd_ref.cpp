@@ -18,31 +18,79 @@
 #include <omp.h>
 #endif
 
+// Compile-time variants of the SAME source (oracle/build.py), mirrored by the CUDA builds:
+//   SRHD_REF_EOS    0  Taub-Mathews EoS (Eq. 10; the default, what the paper recommends)
+//                   1  polytropic EoS with a constant ratio of specific heats Gamma = NUM/DEN (Eq. 11; "we still
+//                      reserve this feature ... for fast computation of a pure non-relativistic or relativistic
+//                      gas"), Gamma = SRHD_REF_GAMMA_NUM / SRHD_REF_GAMMA_DEN (5/3 or 4/3)
+//   SRHD_REF_SCHEME 0  the paper's new scheme: the fifth conserved variable is the reduced energy Etilde = E - D
+//                      (Eq. 6), evolved by the flux (Etilde + p) v (Eq. 7), Eq. 15 solved from Etilde
+//                   1  the "original scheme" the paper compares against (section 4; App. B): the
+//                      fifth conserved variable is the total energy E (Eq. 5c), evolved by the flux M (Eq. 4c), the
+//                      left-hand side of Eq. 15 formed as (E/D)^2 - (|M|/D)^2 - 1 -- for the A/B runs of Fig. 3 and
+//                      Fig. 16 only
+#ifndef SRHD_REF_EOS
+#define SRHD_REF_EOS 0
+#endif
+#ifndef SRHD_REF_SCHEME
+#define SRHD_REF_SCHEME 0
+#endif
+#ifndef SRHD_REF_GAMMA_NUM
+#define SRHD_REF_GAMMA_NUM 5
+#define SRHD_REF_GAMMA_DEN 3
+#endif
+
 namespace {
 
 constexpr double kEps = DBL_EPSILON;  // eps_machine of Eq. 30 for double precision
+#if SRHD_REF_EOS == 1
+constexpr double kGnum = SRHD_REF_GAMMA_NUM, kGden = SRHD_REF_GAMMA_DEN;   // Gamma = kGnum / kGden
+constexpr double kG1 = kGnum / (kGnum - kGden);                             // Gamma / (Gamma - 1): 2.5 or 4, exact
+#endif
 
 // ---------------------------------------------------------------- O1: Taub-Mathews EoS ---------
 // P:185 Eq. 22: htilde = 2.5 T + 2.25 T^2 / (1 + sqrt(2.25 T^2 + 1))      (subtraction free)
+#if SRHD_REF_EOS == 0
 double htilde_of_T(double T) {
   const double a = 2.25 * T * T;
   return 2.5 * T + a / (1.0 + std::sqrt(a + 1.0));
 }
+#else
+// P:107 Eq. 11: h = 1 + Gamma/(Gamma-1) T
+double htilde_of_T(double T) { return kG1 * T; }
+#endif
 // P:148 Eq. 16: T = (2 ht^2 + 4 ht) / (5 ht + 5 + sqrt(9 ht^2 + 18 ht + 25))
+#if SRHD_REF_EOS == 0
 double T_of_htilde(double ht) {
   return (2.0 * ht * ht + 4.0 * ht) / (5.0 * ht + 5.0 + std::sqrt(9.0 * ht * ht + 18.0 * ht + 25.0));
 }
+#else
+double T_of_htilde(double ht) { return ht / kG1; }             // Eq. 11 inverted
+#endif
 // P:591 Eq. A2
+#if SRHD_REF_EOS == 0
 double dT_dhtilde(double ht) {
   const double s = std::sqrt(9.0 * ht * ht + 18.0 * ht + 25.0);
   const double den = 5.0 * ht + 5.0 + s;
   return (4.0 * ht + 4.0) / den - (2.0 * ht * ht + 4.0 * ht) * ((9.0 * ht + 9.0) / s + 5.0) / (den * den);
 }
+#else
+double dT_dhtilde(double) { return 1.0 / kG1; }
+#endif
 // P:129 Eq. 14 squared, with h = 1 + htilde(T) (Eq. 10 == 1 + Eq. 22)
+#if SRHD_REF_EOS == 0
 double cs2_of_T(double T) {
   const double h = 1.0 + htilde_of_T(T);
   return (T / (3.0 * h)) * ((5.0 * h - 8.0 * T) / (h - T));
 }
+#else
+// ideal gas with constant Gamma: c_s^2 = Gamma p / (rho h) = Gamma T / h (the paper prints Eq. 14 for the TM EoS
+// only; reading S19)
+double cs2_of_T(double T) {
+  const double h = 1.0 + htilde_of_T(T);
+  return (kGnum * T) / (kGden * h);
+}
+#endif
 // P:140-144 Eq. 15, right-hand side f(htilde) with musq = (|M|/D)^2, T = T(htilde) by Eq. 16
 double f_eq15(double ht, double T, double musq) {
   const double h = ht + 1.0;
@@ -58,6 +106,18 @@ double df_eqA1(double ht, double T, double dT, double musq) {
 }
 // initial guess.  A7 threshold; A6 hot branch; A4 cold branch in the corrected form
 // (reading G2: the positive root of A3; the printed numerator sqrt(...) is a typo).
+#if SRHD_REF_EOS == 1
+// App. A is specific to the TM EoS.  For Eq. 11, T = a htilde with a = (Gamma-1)/Gamma turns Eq. 15 into
+//   f = (1 - 2a + a^2 xi) htilde^2 + 2 (1 - a) htilde,   xi = h^2/(h^2 + mu^2) in [1/(1+mu^2), 1],
+// a quadratic in htilde for fixed xi.  Its positive root with the LOWER bound of xi is an upper bound of the true
+// root, from which Newton-Raphson on the increasing, convex f descends monotonically (reading S20).
+double htilde_guess(double L, double musq) {
+  const double a = 1.0 / kG1;
+  const double A = 1.0 - 2.0 * a + a * a / (1.0 + musq);
+  const double B = 1.0 - a;
+  return L / (B + std::sqrt(B * B + A * L));
+}
+#else
 double htilde_guess(double L, double musq) {
   const double s = 1.0 + musq;
   const double q = 43.0 * musq + 63.0;
@@ -65,6 +125,7 @@ double htilde_guess(double L, double musq) {
   if (L > r * r) return (4.0 / 3.0) * std::sqrt(L);                                   // A6
   return 125.0 * s * L / (75.0 * s + std::sqrt(125.0 * s * q * L + 5625.0 * s * s));  // A4 (G2)
 }
+#endif
 
 // ---------------------------------------------------------------- O2: prim -> cons --------------
 // P:641 Fig. 15 (right); Eq. 5a, 5b; Eq. 22, 23; Eq. 15 "with known |M|/D".
@@ -83,7 +144,12 @@ void prim2cons(const double W[5], double U[5]) {
   U[1] = Dh * Ux;                                             // Eq. 5b
   U[2] = Dh * Uy;
   U[3] = Dh * Uz;
+#if SRHD_REF_SCHEME == 0
   U[4] = D * ((musq + f) / (1.0 + std::sqrt(1.0 + musq + f)));  // Eq. 23
+#else
+  (void)f;
+  U[4] = Dh * gamma - p;                                        // original scheme: E = D h gamma - p (Eq. 5c)
+#endif
 }
 
 // ---------------------------------------------------------------- O3: cons -> prim --------------
@@ -103,7 +169,11 @@ bool cons2prim(const double U[5], double W[5], double rtol, int max_iter, int* i
   const double x = dpos ? Et / Dc : 0.0;
   const double ux = Mx / Dc, uy = My / Dc, uz = Mz / Dc;
   const double musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
+#if SRHD_REF_SCHEME == 0
   double L = std::fma(x, x + 2.0, -musq);                     // left-hand side of Eq. 15 / Eq. 30
+#else
+  double L = std::fma(x, x, -musq) - 1.0;                     // original scheme: (E/D)^2 - (|M|/D)^2 - 1
+#endif
   if (!(L > kEps)) {
     phys = false;
     L = kEps;
@@ -142,7 +212,11 @@ bool is_physical(const double U[5]) {
   const double x = Et / D;
   const double ux = U[1] / D, uy = U[2] / D, uz = U[3] / D;
   const double musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
+#if SRHD_REF_SCHEME == 0
   const double L = std::fma(x, x + 2.0, -musq);
+#else
+  const double L = std::fma(x, x, -musq) - 1.0;
+#endif
   return L > kEps;
 }
 
@@ -169,7 +243,11 @@ void phys_flux(int d, const double W[5], const double U[5], double F[5]) {
   F[2] = U[2] * v;
   F[3] = U[3] * v;
   F[1 + d] += W[4];
-  F[4] = (U[4] + W[4]) * v;
+#if SRHD_REF_SCHEME == 0
+  F[4] = (U[4] + W[4]) * v;                                   // Eq. 7
+#else
+  F[4] = U[1 + d];                                            // original scheme: E is evolved by the flux M (Eq. 4c)
+#endif
 }
 
 // One side of a Riemann problem in the rotated frame (n = normal, t1, t2 = tangential).
@@ -236,7 +314,11 @@ void side_setup(int d, const double W[5], const double U[5], Side& s) {
   s.F[1] = s.U[1] * s.vn + p;
   s.F[2] = s.U[2] * s.vn;
   s.F[3] = s.U[3] * s.vn;
+#if SRHD_REF_SCHEME == 0
   s.F[4] = (s.U[4] + p) * s.vn;
+#else
+  s.F[4] = s.U[1];                                            // M_n = (E + p) v_n: the HLL averages still split it as E v_n + p v_n
+#endif
 }
 
 // The two-wave (HLL) averages of Mignone & Bodo 2005 with the S6 speeds,
@@ -283,8 +365,13 @@ void hllc_rot(const Side& L, const Side& R, double F[5]) {
     Uh[c] = (AR * R.U[c] + BL * L.U[c] + (L.pt[c] - R.pt[c])) / den;
     Fh[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;
   }
+#if SRHD_REF_SCHEME == 0
   const double Eh = Uh[4] + Uh[0];                            // E = Etilde + D   (sums only)
   const double FEh = Fh[4] + Fh[0];
+#else
+  const double Eh = Uh[4];                                    // original scheme: the fifth variable IS E
+  const double FEh = Fh[4];
+#endif
   const double a = FEh, b = Eh + Fh[1], m = Uh[1];
   // contact speed: root of a lam^2 - b lam + m = 0 in (-1,1), rationalised (safe for a -> 0)
   const double lam = 2.0 * m / (b + std::sqrt(b * b - 4.0 * a * m));
