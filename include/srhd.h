@@ -270,6 +270,13 @@ const char* srhd_error_string(int code);
  * (libsrhd_b200_exact.so, used by the bit-parity tests), 0 for the production build. */
 int srhd_build_is_exact(void);
 
+/* Which compile-time variant this library is (one library per variant, like the EoS
+ * choice of the paper's code): "eos=taub-mathews|gamma-5/3|gamma-4/3 energy=reduced|total arithmetic=production|
+ * generic|exact".  eos: Eq. 10 or the polytropic P:107 Eq. 11; energy=total is the paper's "original scheme"
+ * (the fifth conserved variable is E, evolved by the flux M) kept for its A/B runs; arithmetic=generic means
+ * the paper's formulas as written with IEEE division and square root, exact the same without FMA contraction. */
+const char* srhd_build_variant(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -46,7 +46,7 @@ class Stats(C.Structure):
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
            "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_flux_correction", "srhd_ghost_interp", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed", "srhd_grid_step_cfl",
-           "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact"]
+           "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact", "srhd_build_variant"]
 
 _LIBS = {}
 
@@ -56,7 +56,8 @@ class SrhdError(RuntimeError):
 
 
 def load_library(exact=False):
-    """dlopen libsrhd_b200[_exact].so (built in-tree by paper_2012_11130_b200.build)."""
+    """dlopen libsrhd_b200[_exact].so (built in-tree by paper_2012_11130_b200.build); `exact` may also name one of
+    the variant libraries of build.VARIANTS ("gamma53", "gamma53_exact", "gamma43_exact", "orig_exact")."""
     if exact in _LIBS:
         return _LIBS[exact]
     path = _build.lib_path(exact)
@@ -110,6 +111,8 @@ def load_library(exact=False):
     L.srhd_error_string.argtypes = [C.c_int]
     L.srhd_build_is_exact.restype = C.c_int
     L.srhd_build_is_exact.argtypes = []
+    L.srhd_build_variant.restype = C.c_char_p
+    L.srhd_build_variant.argtypes = []
     _LIBS[exact] = L
     return L
 

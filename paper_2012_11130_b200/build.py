@@ -16,13 +16,30 @@ SOURCES = ["srhd_convert.cu", "srhd_fluid.cu", "srhd_grid.cu", "srhd_refine.cu",
 HEADERS = ["srhd_math.cuh", "srhd_common.cuh", "srhd_uniform.cuh", os.path.join("..", "..", "include", "srhd.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared"]
+_EXACT = ["-fmad=false", "-DSRHD_EXACT=1"]
+_G53 = ["-DSRHD_EOS=1", "-DSRHD_GAMMA_NUM=5", "-DSRHD_GAMMA_DEN=3"]
+_G43 = ["-DSRHD_EOS=1", "-DSRHD_GAMMA_NUM=4", "-DSRHD_GAMMA_DEN=3"]
 VARIANTS = {
     "libsrhd_b200.so": [],
-    "libsrhd_b200_exact.so": ["-fmad=false", "-DSRHD_EXACT=1"],
+    "libsrhd_b200_exact.so": _EXACT,
+    # SURVEY.md 8f row 4 (csrc/srhd_math.cuh header): the polytropic EoS of P:107 Eq. 11 and the paper's "original
+    # scheme" (evolve E; for the A/B runs of Fig. 3 / Fig. 16).  The *_exact libraries reproduce the oracle's variants
+    # bit for bit; libsrhd_b200_gamma53.so is the same polytropic path with FMA contraction (for timing).
+    "libsrhd_b200_gamma53.so": _G53,
+    "libsrhd_b200_gamma53_exact.so": _EXACT + _G53,
+    "libsrhd_b200_gamma43_exact.so": _EXACT + _G43,
+    "libsrhd_b200_orig_exact.so": _EXACT + ["-DSRHD_SCHEME=1"],
 }
 
 
 def lib_path(exact=False):
+    """False: the production library; True: the exact build; a string: that variant ("gamma53", "gamma53_exact",
+    "gamma43_exact", "orig_exact")."""
+    if isinstance(exact, str):
+        name = f"libsrhd_b200_{exact}.so"
+        if name not in VARIANTS:
+            raise ValueError(f"unknown library variant {exact!r}")
+        return os.path.join(HERE, name)
     return os.path.join(HERE, "libsrhd_b200_exact.so" if exact else "libsrhd_b200.so")
 
 
@@ -59,4 +76,4 @@ def build(force=False, verbose=False, extra=()):
 
 if __name__ == "__main__":
     build(force="--force" in sys.argv, verbose="-v" in sys.argv)
-    print("\n".join(lib_path(e) for e in (False, True)))
+    print("\n".join(os.path.join(HERE, n) for n in VARIANTS))

@@ -515,6 +515,32 @@ extern "C" const char* srhd_error_string(int code) {
 
 extern "C" int srhd_build_is_exact(void) { return SRHD_EXACT; }
 
+#define SRHD_STR2(x) #x
+#define SRHD_STR(x) SRHD_STR2(x)
+extern "C" const char* srhd_build_variant(void) {
+  return "eos="
+#if SRHD_EOS == 0
+         "taub-mathews"
+#else
+         "gamma-" SRHD_STR(SRHD_GAMMA_NUM) "/" SRHD_STR(SRHD_GAMMA_DEN)
+#endif
+         " energy="
+#if SRHD_SCHEME == 0
+         "reduced"
+#else
+         "total"
+#endif
+         " arithmetic="
+#if SRHD_EXACT
+         "exact"
+#elif SRHD_GENERIC
+         "generic"
+#else
+         "production"
+#endif
+      ;
+}
+
 // ---- fp64 ALU roof: register-only DFMA loop, 8 independent chains per thread, 8 CTAs x 256 threads
 // per SM (full occupancy).  Used by bench.py for the MEASURED denominator of the "alu" roofline.
 namespace srhd {

@@ -19,7 +19,7 @@ constexpr int kVlThreads = 256;
 // by-products of a conversion that the production-build solver wants, recomputed from primitives
 SRHD_DEV Aux aux_of_prim(const double W[5]) {
   Aux a;
-#if SRHD_EXACT
+#if SRHD_GENERIC
   a.ht = a.T = a.rg = 0.0;
 #else
   a.T = W[4] * rcp_f(W[0]);
