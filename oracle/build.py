@@ -19,7 +19,9 @@ HDR = [os.path.join(HERE, "srhd_ref.hpp")]
 VARIANTS = {"": ["-ffp-contract=off"], "fma": ["-ffp-contract=fast", "-mfma"],
             "gamma53": ["-ffp-contract=off", "-DSRHD_REF_EOS=1", "-DSRHD_REF_GAMMA_NUM=5", "-DSRHD_REF_GAMMA_DEN=3"],
             "gamma43": ["-ffp-contract=off", "-DSRHD_REF_EOS=1", "-DSRHD_REF_GAMMA_NUM=4", "-DSRHD_REF_GAMMA_DEN=3"],
-            "orig": ["-ffp-contract=off", "-DSRHD_REF_SCHEME=1"]}
+            "orig": ["-ffp-contract=off", "-DSRHD_REF_SCHEME=1"],
+            # "f32": every array and every operation in single precision (the precision of the paper's performance runs)
+            "f32": ["-ffp-contract=off", "-DSRHD_REF_F32"]}
 
 
 def lib_path(variant=""):

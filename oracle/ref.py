@@ -11,8 +11,22 @@ import numpy as np
 from . import build as _build
 
 _LIB = None
-_D = C.c_double
 _DP = C.POINTER(C.c_double)
+
+
+def _is_f32():
+    return _VARIANT == "f32"
+
+
+def rdtype():
+    """numpy dtype of the oracle's `real` in the current variant (float32 for "f32", else float64)."""
+    return np.float32 if _is_f32() else np.float64
+
+
+def _D(x=None):
+    """ctypes type of `real` (called without an argument) or a `real` scalar argument."""
+    t = C.c_float if _is_f32() else C.c_double
+    return t if x is None else t(x)
 
 
 class Params(C.Structure):
@@ -68,13 +82,13 @@ def lib():
         _LIBS[_VARIANT] = L
         for name in ("htilde_of_T", "T_of_htilde", "dT_dhtilde", "cs2_of_T", "smax_of_umax"):
             f = getattr(L, "srhd_ref_" + name)
-            f.restype, f.argtypes = _D, [_D]
+            f.restype, f.argtypes = _D(), [_D()]
         for name in ("f_eq15", "df_eqA1", "htilde_guess"):
             f = getattr(L, "srhd_ref_" + name)
-            f.restype, f.argtypes = _D, [_D, _D]
-        L.srhd_ref_limited_slope.restype = _D
-        L.srhd_ref_limited_slope.argtypes = [_D, _D, _D]
-        L.srhd_ref_umax_of_prim.restype = _D
+            f.restype, f.argtypes = _D(), [_D(), _D()]
+        L.srhd_ref_limited_slope.restype = _D()
+        L.srhd_ref_limited_slope.argtypes = [_D(), _D(), _D()]
+        L.srhd_ref_umax_of_prim.restype = _D()
         L.srhd_ref_umax_of_prim.argtypes = [_DP]
         L.srhd_ref_step_box.restype = C.c_int
         _LIB = L
@@ -86,14 +100,14 @@ def _p(a):
 
 
 def _f64(a):
-    a = np.ascontiguousarray(a, dtype=np.float64)
+    a = np.ascontiguousarray(a, dtype=rdtype())
     return a
 
 
 # ---- scalar EoS helpers (vectorised over numpy inputs by a Python loop; test-sized only) ----
 def _vec1(name, x):
     f = getattr(lib(), "srhd_ref_" + name)
-    x = np.asarray(x, dtype=np.float64)
+    x = np.asarray(x, dtype=np.float64)   # scalar hooks take Python floats
     return np.array([f(float(v)) for v in x.ravel()]).reshape(x.shape) if x.ndim else f(float(x))
 
 
@@ -115,7 +129,7 @@ def umax_of_prim(W):
 
 def recon_1d(recon, a, beta, beta0):
     a = _f64(a)
-    am, ap = C.c_double(), C.c_double()
+    am, ap = _D()(), _D()()
     lib().srhd_ref_recon_1d(C.c_int(recon), _p(a), _D(beta), _D(beta0), C.byref(am), C.byref(ap))
     return am.value, ap.value
 
@@ -137,7 +151,7 @@ def cons2prim(cons, par=None, diag=False):
     prim = np.empty_like(cons)
     n = cons.shape[1]
     if diag:
-        ht = np.empty(n)
+        ht = np.empty(n, dtype=rdtype())
         it = np.empty(n, dtype=np.int32)
         bad = np.empty(n, dtype=np.uint8)
         lib().srhd_ref_cons2prim_diag(_p(cons), _p(prim), C.c_size_t(n), C.c_size_t(n), C.byref(par),
@@ -153,14 +167,14 @@ def max_signal_speed(cons, par=None):
     cons = _f64(cons)
     par = par or params()
     n = cons.shape[1]
-    out = C.c_double()
+    out = _D()()
     lib().srhd_ref_max_signal_speed(_p(cons), C.c_size_t(n), C.c_size_t(n), C.byref(par), C.byref(out))
     return out.value
 
 
 def phys_flux(d, W, U):
     W, U = _f64(W), _f64(U)
-    F = np.empty(5)
+    F = np.empty(5, dtype=rdtype())
     lib().srhd_ref_phys_flux(C.c_int(d), _p(W), _p(U), _p(F))
     return F
 
@@ -173,7 +187,7 @@ def wave_speeds(d, W):
 def wave_speed_differences(d, W):
     """[lambda_-, lambda_+, lambda_+ - v_n, v_n - lambda_-, 1 - lambda_+, 1 + lambda_-] (reading S6)."""
     W = _f64(W)
-    out = np.empty(6)
+    out = np.empty(6, dtype=rdtype())
     lib().srhd_ref_wave_speeds(C.c_int(d), _p(W), _p(out))
     return out
 
@@ -181,7 +195,7 @@ def wave_speed_differences(d, W):
 def riemann_flux(riemann, d, WL, UL, WR, UR):
     WL, UL, WR, UR = map(_f64, (WL, UL, WR, UR))
     s = {"hlle": 0, "hllc": 1}[riemann] if isinstance(riemann, str) else int(riemann)
-    F = np.empty(5)
+    F = np.empty(5, dtype=rdtype())
     lib().srhd_ref_riemann_flux(C.c_int(s), C.c_int(d), _p(WL), _p(UL), _p(WR), _p(UR), _p(F))
     return F
 
@@ -193,7 +207,7 @@ def step_box(cons_in, dt, dh, par):
     g = par.ghost
     _, sz, sy, sx = cons_in.shape
     nx, ny, nz = sx - 2 * g, sy - 2 * g, sz - 2 * g
-    out = np.empty((5, nz, ny, nx))
+    out = np.empty((5, nz, ny, nx), dtype=rdtype())
     st = Stats()
     passes = lib().srhd_ref_step_box(_p(cons_in), _p(out), C.c_int(nx), C.c_int(ny), C.c_int(nz),
                                      _D(dt), _D(dh), C.byref(par), C.byref(st))
@@ -206,7 +220,7 @@ def fluid_step(cons_in, dt, dh, par, nthreads=0):
     npg = cons_in.shape[0]
     nxt = 16 + 2 * par.ghost
     assert cons_in.shape == (npg, 5, nxt, nxt, nxt)
-    out = np.empty((npg, 8, 5, 8, 8, 8))
+    out = np.empty((npg, 8, 5, 8, 8, 8), dtype=rdtype())
     st = Stats()
     lib().srhd_ref_fluid_step(_p(cons_in), _p(out), C.c_int(npg), _D(dt), _D(dh), C.byref(par),
                               C.byref(st), C.c_int(nthreads))
@@ -217,8 +231,8 @@ def fluid_step_fluxes(cons_in, dt, dh, par, nthreads=0):
     """As fluid_step, plus the patch-boundary fluxes (npg,8,6,5,8,8) of the accepted pass."""
     cons_in = _f64(cons_in)
     npg = cons_in.shape[0]
-    out = np.empty((npg, 8, 5, 8, 8, 8))
-    flux = np.empty((npg, 8, 6, 5, 8, 8))
+    out = np.empty((npg, 8, 5, 8, 8, 8), dtype=rdtype())
+    flux = np.empty((npg, 8, 6, 5, 8, 8), dtype=rdtype())
     st = Stats()
     lib().srhd_ref_fluid_step_fluxes(_p(cons_in), _p(out), _p(flux), C.c_int(npg), _D(dt), _D(dh),
                                      C.byref(par), C.byref(st), C.c_int(nthreads))
@@ -282,7 +296,7 @@ def _inflow(inflow):
 def grid_pad(grid, g, bc, inflow=None):
     grid = _f64(grid)
     _, nz, ny, nx = grid.shape
-    out = np.empty((5, nz + 2 * g, ny + 2 * g, nx + 2 * g))
+    out = np.empty((5, nz + 2 * g, ny + 2 * g, nx + 2 * g), dtype=rdtype())
     mask, cons = _inflow(inflow)
     lib().srhd_ref_grid_pad(_p(grid), _p(out), C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_int(g), _bc(bc),
                             mask.ctypes.data_as(C.POINTER(C.c_ubyte)) if mask is not None else None,
@@ -296,7 +310,7 @@ def grid_gather(grid, g, bc, inflow=None):
     assert nx % 16 == 0 and ny % 16 == 0 and nz % 16 == 0
     npg = (nx // 16) * (ny // 16) * (nz // 16)
     nxt = 16 + 2 * g
-    out = np.empty((npg, 5, nxt, nxt, nxt))
+    out = np.empty((npg, 5, nxt, nxt, nxt), dtype=rdtype())
     mask, cons = _inflow(inflow)
     lib().srhd_ref_grid_gather(_p(grid), _p(out), C.c_int(nx), C.c_int(ny), C.c_int(nz), C.c_int(g), _bc(bc),
                                mask.ctypes.data_as(C.POINTER(C.c_ubyte)) if mask is not None else None,
@@ -307,7 +321,7 @@ def grid_gather(grid, g, bc, inflow=None):
 def grid_scatter(cons_out, shape):
     cons_out = _f64(cons_out)
     nz, ny, nx = shape
-    grid = np.empty((5, nz, ny, nx))
+    grid = np.empty((5, nz, ny, nx), dtype=rdtype())
     lib().srhd_ref_grid_scatter(_p(cons_out), _p(grid), C.c_int(nx), C.c_int(ny), C.c_int(nz))
     return grid
 

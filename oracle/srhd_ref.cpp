@@ -13,6 +13,7 @@
 #include <cfloat>
 #include <cmath>
 #include <cstring>
+#include <limits>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -29,6 +30,8 @@
 //                      fifth conserved variable is the total energy E (Eq. 5c), evolved by the flux M (Eq. 4c), the
 //                      left-hand side of Eq. 15 formed as (E/D)^2 - (|M|/D)^2 - 1 -- for the A/B runs of Fig. 3 and
 //                      Fig. 16 only
+//   SRHD_REF_F32    the whole computation in single precision (`real` = float): the precision of every performance
+//                   number in the paper; eps_machine of Eq. 30 is then FLT_EPSILON ~ 1e-7
 #ifndef SRHD_REF_EOS
 #define SRHD_REF_EOS 0
 #endif
@@ -42,67 +45,68 @@
 
 namespace {
 
-constexpr double kEps = DBL_EPSILON;  // eps_machine of Eq. 30 for double precision
+constexpr real kEps = std::numeric_limits<real>::epsilon();  // eps_machine of Eq. 30: 2.2e-16 (double), 1.2e-7 (single)
+constexpr real kTiny = std::numeric_limits<real>::min();     // smallest positive normal number (reading S10)
 #if SRHD_REF_EOS == 1
-constexpr double kGnum = SRHD_REF_GAMMA_NUM, kGden = SRHD_REF_GAMMA_DEN;   // Gamma = kGnum / kGden
-constexpr double kG1 = kGnum / (kGnum - kGden);                             // Gamma / (Gamma - 1): 2.5 or 4, exact
+constexpr real kGnum = SRHD_REF_GAMMA_NUM, kGden = SRHD_REF_GAMMA_DEN;   // Gamma = kGnum / kGden
+constexpr real kG1 = kGnum / (kGnum - kGden);                             // Gamma / (Gamma - 1): 2.5 or 4, exact
 #endif
 
 // ---------------------------------------------------------------- O1: Taub-Mathews EoS ---------
 // P:185 Eq. 22: htilde = 2.5 T + 2.25 T^2 / (1 + sqrt(2.25 T^2 + 1))      (subtraction free)
 #if SRHD_REF_EOS == 0
-double htilde_of_T(double T) {
-  const double a = 2.25 * T * T;
-  return 2.5 * T + a / (1.0 + std::sqrt(a + 1.0));
+real htilde_of_T(real T) {
+  const real a = real(2.25) * T * T;
+  return real(2.5) * T + a / (real(1.0) + std::sqrt(a + real(1.0)));
 }
 #else
 // P:107 Eq. 11: h = 1 + Gamma/(Gamma-1) T
-double htilde_of_T(double T) { return kG1 * T; }
+real htilde_of_T(real T) { return kG1 * T; }
 #endif
 // P:148 Eq. 16: T = (2 ht^2 + 4 ht) / (5 ht + 5 + sqrt(9 ht^2 + 18 ht + 25))
 #if SRHD_REF_EOS == 0
-double T_of_htilde(double ht) {
-  return (2.0 * ht * ht + 4.0 * ht) / (5.0 * ht + 5.0 + std::sqrt(9.0 * ht * ht + 18.0 * ht + 25.0));
+real T_of_htilde(real ht) {
+  return (real(2.0) * ht * ht + real(4.0) * ht) / (real(5.0) * ht + real(5.0) + std::sqrt(real(9.0) * ht * ht + real(18.0) * ht + real(25.0)));
 }
 #else
-double T_of_htilde(double ht) { return ht / kG1; }             // Eq. 11 inverted
+real T_of_htilde(real ht) { return ht / kG1; }             // Eq. 11 inverted
 #endif
 // P:591 Eq. A2
 #if SRHD_REF_EOS == 0
-double dT_dhtilde(double ht) {
-  const double s = std::sqrt(9.0 * ht * ht + 18.0 * ht + 25.0);
-  const double den = 5.0 * ht + 5.0 + s;
-  return (4.0 * ht + 4.0) / den - (2.0 * ht * ht + 4.0 * ht) * ((9.0 * ht + 9.0) / s + 5.0) / (den * den);
+real dT_dhtilde(real ht) {
+  const real s = std::sqrt(real(9.0) * ht * ht + real(18.0) * ht + real(25.0));
+  const real den = real(5.0) * ht + real(5.0) + s;
+  return (real(4.0) * ht + real(4.0)) / den - (real(2.0) * ht * ht + real(4.0) * ht) * ((real(9.0) * ht + real(9.0)) / s + real(5.0)) / (den * den);
 }
 #else
-double dT_dhtilde(double) { return 1.0 / kG1; }
+real dT_dhtilde(real) { return real(1.0) / kG1; }
 #endif
 // P:129 Eq. 14 squared, with h = 1 + htilde(T) (Eq. 10 == 1 + Eq. 22)
 #if SRHD_REF_EOS == 0
-double cs2_of_T(double T) {
-  const double h = 1.0 + htilde_of_T(T);
-  return (T / (3.0 * h)) * ((5.0 * h - 8.0 * T) / (h - T));
+real cs2_of_T(real T) {
+  const real h = real(1.0) + htilde_of_T(T);
+  return (T / (real(3.0) * h)) * ((real(5.0) * h - real(8.0) * T) / (h - T));
 }
 #else
 // ideal gas with constant Gamma: c_s^2 = Gamma p / (rho h) = Gamma T / h (the paper prints Eq. 14 for the TM EoS
 // only; reading S19)
-double cs2_of_T(double T) {
-  const double h = 1.0 + htilde_of_T(T);
+real cs2_of_T(real T) {
+  const real h = real(1.0) + htilde_of_T(T);
   return (kGnum * T) / (kGden * h);
 }
 #endif
 // P:140-144 Eq. 15, right-hand side f(htilde) with musq = (|M|/D)^2, T = T(htilde) by Eq. 16
-double f_eq15(double ht, double T, double musq) {
-  const double h = ht + 1.0;
-  return ht * ht + 2.0 * ht - 2.0 * T * h + (T * T) * (h * h) / (h * h + musq);
+real f_eq15(real ht, real T, real musq) {
+  const real h = ht + real(1.0);
+  return ht * ht + real(2.0) * ht - real(2.0) * T * h + (T * T) * (h * h) / (h * h + musq);
 }
 // P:587 Eq. A1
-double df_eqA1(double ht, double T, double dT, double musq) {
-  const double h = ht + 1.0;
-  const double den = h * h + musq;
-  const double h4 = (h * h) * (h * h);
-  return 2.0 * ht + 2.0 - 2.0 * T - 2.0 * h * dT +
-         (2.0 * T * h4 * dT + 2.0 * T * h * musq * (h * dT + T)) / (den * den);
+real df_eqA1(real ht, real T, real dT, real musq) {
+  const real h = ht + real(1.0);
+  const real den = h * h + musq;
+  const real h4 = (h * h) * (h * h);
+  return real(2.0) * ht + real(2.0) - real(2.0) * T - real(2.0) * h * dT +
+         (real(2.0) * T * h4 * dT + real(2.0) * T * h * musq * (h * dT + T)) / (den * den);
 }
 // initial guess.  A7 threshold; A6 hot branch; A4 cold branch in the corrected form
 // (reading G2: the positive root of A3; the printed numerator sqrt(...) is a typo).
@@ -111,41 +115,41 @@ double df_eqA1(double ht, double T, double dT, double musq) {
 //   f = (1 - 2a + a^2 xi) htilde^2 + 2 (1 - a) htilde,   xi = h^2/(h^2 + mu^2) in [1/(1+mu^2), 1],
 // a quadratic in htilde for fixed xi.  Its positive root with the LOWER bound of xi is an upper bound of the true
 // root, from which Newton-Raphson on the increasing, convex f descends monotonically (reading S20).
-double htilde_guess(double L, double musq) {
-  const double a = 1.0 / kG1;
-  const double A = 1.0 - 2.0 * a + a * a / (1.0 + musq);
-  const double B = 1.0 - a;
+real htilde_guess(real L, real musq) {
+  const real a = real(1.0) / kG1;
+  const real A = real(1.0) - real(2.0) * a + a * a / (real(1.0) + musq);
+  const real B = real(1.0) - a;
   return L / (B + std::sqrt(B * B + A * L));
 }
 #else
-double htilde_guess(double L, double musq) {
-  const double s = 1.0 + musq;
-  const double q = 43.0 * musq + 63.0;
-  const double r = 1800.0 * s / (437.0 * musq + 117.0);
-  if (L > r * r) return (4.0 / 3.0) * std::sqrt(L);                                   // A6
-  return 125.0 * s * L / (75.0 * s + std::sqrt(125.0 * s * q * L + 5625.0 * s * s));  // A4 (G2)
+real htilde_guess(real L, real musq) {
+  const real s = real(1.0) + musq;
+  const real q = real(43.0) * musq + real(63.0);
+  const real r = real(1800.0) * s / (real(437.0) * musq + real(117.0));
+  if (L > r * r) return (real(4.0) / real(3.0)) * std::sqrt(L);                                   // A6
+  return real(125.0) * s * L / (real(75.0) * s + std::sqrt(real(125.0) * s * q * L + real(5625.0) * s * s));  // A4 (G2)
 }
 #endif
 
 // ---------------------------------------------------------------- O2: prim -> cons --------------
 // P:641 Fig. 15 (right); Eq. 5a, 5b; Eq. 22, 23; Eq. 15 "with known |M|/D".
-void prim2cons(const double W[5], double U[5]) {
-  const double rho = W[0], Ux = W[1], Uy = W[2], Uz = W[3], p = W[4];
-  const double T = p / rho;                                   // Eq. 18
-  const double ht = htilde_of_T(T);                           // Eq. 22
-  const double Usq = Ux * Ux + Uy * Uy + Uz * Uz;
-  const double gamma = std::sqrt(1.0 + Usq);                  // Eq. 8
-  const double D = rho * gamma;                               // Eq. 5a
-  const double h = 1.0 + ht;
-  const double Dh = D * h;
-  const double musq = (h * h) * Usq;                          // (|M|/D)^2 from Eq. 5b
-  const double f = f_eq15(ht, T, musq);                       // Eq. 15
+void prim2cons(const real W[5], real U[5]) {
+  const real rho = W[0], Ux = W[1], Uy = W[2], Uz = W[3], p = W[4];
+  const real T = p / rho;                                   // Eq. 18
+  const real ht = htilde_of_T(T);                           // Eq. 22
+  const real Usq = Ux * Ux + Uy * Uy + Uz * Uz;
+  const real gamma = std::sqrt(real(1.0) + Usq);                  // Eq. 8
+  const real D = rho * gamma;                               // Eq. 5a
+  const real h = real(1.0) + ht;
+  const real Dh = D * h;
+  const real musq = (h * h) * Usq;                          // (|M|/D)^2 from Eq. 5b
+  const real f = f_eq15(ht, T, musq);                       // Eq. 15
   U[0] = D;
   U[1] = Dh * Ux;                                             // Eq. 5b
   U[2] = Dh * Uy;
   U[3] = Dh * Uz;
 #if SRHD_REF_SCHEME == 0
-  U[4] = D * ((musq + f) / (1.0 + std::sqrt(1.0 + musq + f)));  // Eq. 23
+  U[4] = D * ((musq + f) / (real(1.0) + std::sqrt(real(1.0) + musq + f)));  // Eq. 23
 #else
   (void)f;
   U[4] = Dh * gamma - p;                                        // original scheme: E = D h gamma - p (Eq. 5c)
@@ -158,43 +162,43 @@ void prim2cons(const double W[5], double U[5]) {
 // correctly rounded, so L is reproducible bit for bit by any IEEE implementation.
 // Returns true iff the input passes D>0, Etilde>0, L>eps (Eq. 30).  A failing state is evaluated
 // with L <- eps (reading S10) so the result is deterministic and finite.
-bool cons2prim(const double U[5], double W[5], double rtol, int max_iter, int* iters_out,
-               double* ht_out) {
-  const double D = U[0], Et = U[4];
-  bool phys = (D > 0.0) && (Et > 0.0);
-  // S10: a state without positive D is evaluated as vacuum at rest (D <- DBL_MIN, M <- 0, Etilde <- 0)
-  const bool dpos = D > DBL_MIN;
-  const double Dc = dpos ? D : DBL_MIN;
-  const double Mx = dpos ? U[1] : 0.0, My = dpos ? U[2] : 0.0, Mz = dpos ? U[3] : 0.0;
-  const double x = dpos ? Et / Dc : 0.0;
-  const double ux = Mx / Dc, uy = My / Dc, uz = Mz / Dc;
-  const double musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
+bool cons2prim(const real U[5], real W[5], real rtol, int max_iter, int* iters_out,
+               real* ht_out) {
+  const real D = U[0], Et = U[4];
+  bool phys = (D > real(0.0)) && (Et > real(0.0));
+  // S10: a state without positive D is evaluated as vacuum at rest (D <- kTiny, M <- 0, Etilde <- 0)
+  const bool dpos = D > kTiny;
+  const real Dc = dpos ? D : kTiny;
+  const real Mx = dpos ? U[1] : real(0.0), My = dpos ? U[2] : real(0.0), Mz = dpos ? U[3] : real(0.0);
+  const real x = dpos ? Et / Dc : real(0.0);
+  const real ux = Mx / Dc, uy = My / Dc, uz = Mz / Dc;
+  const real musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
 #if SRHD_REF_SCHEME == 0
-  double L = std::fma(x, x + 2.0, -musq);                     // left-hand side of Eq. 15 / Eq. 30
+  real L = std::fma(x, x + real(2.0), -musq);                     // left-hand side of Eq. 15 / Eq. 30
 #else
-  double L = std::fma(x, x, -musq) - 1.0;                     // original scheme: (E/D)^2 - (|M|/D)^2 - 1
+  real L = std::fma(x, x, -musq) - real(1.0);                     // original scheme: (E/D)^2 - (|M|/D)^2 - 1
 #endif
   if (!(L > kEps)) {
     phys = false;
     L = kEps;
   }
-  double ht = htilde_guess(L, musq);
+  real ht = htilde_guess(L, musq);
   int it = 0;
   while (it < max_iter) {                                     // Newton-Raphson
-    const double T = T_of_htilde(ht);
-    const double dT = dT_dhtilde(ht);
-    const double delta = (f_eq15(ht, T, musq) - L) / df_eqA1(ht, T, dT, musq);
-    const double ht_new = ht - delta;
+    const real T = T_of_htilde(ht);
+    const real dT = dT_dhtilde(ht);
+    const real delta = (f_eq15(ht, T, musq) - L) / df_eqA1(ht, T, dT, musq);
+    const real ht_new = ht - delta;
     ++it;
     const bool done = (ht_new == ht) || (std::fabs(delta) <= rtol * std::fabs(ht_new));  // S2
     ht = ht_new;
     if (done) break;
   }
-  const double h = 1.0 + ht;
-  const double Ux = Mx / (Dc * h), Uy = My / (Dc * h), Uz = Mz / (Dc * h);        // Eq. 17
-  const double gamma = std::sqrt(1.0 + (Ux * Ux + Uy * Uy + Uz * Uz));            // Eq. 8
-  const double rho = Dc / gamma;                                                   // Eq. 5a
-  const double T = T_of_htilde(ht);                                                // Eq. 16
+  const real h = real(1.0) + ht;
+  const real Ux = Mx / (Dc * h), Uy = My / (Dc * h), Uz = Mz / (Dc * h);        // Eq. 17
+  const real gamma = std::sqrt(real(1.0) + (Ux * Ux + Uy * Uy + Uz * Uz));            // Eq. 8
+  const real rho = Dc / gamma;                                                   // Eq. 5a
+  const real T = T_of_htilde(ht);                                                // Eq. 16
   W[0] = rho;
   W[1] = Ux;
   W[2] = Uy;
@@ -206,38 +210,38 @@ bool cons2prim(const double U[5], double W[5], double rtol, int max_iter, int* i
 }
 
 // Eq. 30 check alone, same canonical L (used on updated cells, O9)
-bool is_physical(const double U[5]) {
-  const double D = U[0], Et = U[4];
-  if (!(D > 0.0) || !(Et > 0.0)) return false;
-  const double x = Et / D;
-  const double ux = U[1] / D, uy = U[2] / D, uz = U[3] / D;
-  const double musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
+bool is_physical(const real U[5]) {
+  const real D = U[0], Et = U[4];
+  if (!(D > real(0.0)) || !(Et > real(0.0))) return false;
+  const real x = Et / D;
+  const real ux = U[1] / D, uy = U[2] / D, uz = U[3] / D;
+  const real musq = std::fma(ux, ux, std::fma(uy, uy, uz * uz));
 #if SRHD_REF_SCHEME == 0
-  const double L = std::fma(x, x + 2.0, -musq);
+  const real L = std::fma(x, x + real(2.0), -musq);
 #else
-  const double L = std::fma(x, x, -musq) - 1.0;
+  const real L = std::fma(x, x, -musq) - real(1.0);
 #endif
   return L > kEps;
 }
 
 // ---------------------------------------------------------------- O4: signal speed --------------
 // P:241 Eq. 26 (reading G1: |U^x|+|U^y|+|U^z|), from primitives; T = p/rho (Eq. 18)
-double umax_of_prim(const double W[5]) {
-  const double T = W[4] / W[0];
-  const double cs2 = cs2_of_T(T);
-  const double Us2 = cs2 / (1.0 - cs2);                       // U_s = c_s/sqrt(1-c_s^2)
-  const double Us = std::sqrt(Us2);
-  const double gs = std::sqrt(1.0 + Us2);                     // gamma_s (reading G4)
-  const double gamma = std::sqrt(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
-  return gs * (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + 3.0 * gamma * Us;
+real umax_of_prim(const real W[5]) {
+  const real T = W[4] / W[0];
+  const real cs2 = cs2_of_T(T);
+  const real Us2 = cs2 / (real(1.0) - cs2);                       // U_s = c_s/sqrt(1-c_s^2)
+  const real Us = std::sqrt(Us2);
+  const real gs = std::sqrt(real(1.0) + Us2);                     // gamma_s (reading G4)
+  const real gamma = std::sqrt(real(1.0) + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+  return gs * (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + real(3.0) * gamma * Us;
 }
-double smax_of_umax(double umax) { return umax / std::sqrt(1.0 + umax * umax); }  // P:247 Eq. 27
+real smax_of_umax(real umax) { return umax / std::sqrt(real(1.0) + umax * umax); }  // P:247 Eq. 27
 
 // ---------------------------------------------------------------- fluxes ------------------------
 // P:61-65 Eq. 4a, 4b and P:83 Eq. 7 along direction d; v = U_d/gamma
-void phys_flux(int d, const double W[5], const double U[5], double F[5]) {
-  const double gamma = std::sqrt(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
-  const double v = W[1 + d] / gamma;
+void phys_flux(int d, const real W[5], const real U[5], real F[5]) {
+  const real gamma = std::sqrt(real(1.0) + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+  const real v = W[1 + d] / gamma;
   F[0] = U[0] * v;
   F[1] = U[1] * v;
   F[2] = U[2] * v;
@@ -252,12 +256,12 @@ void phys_flux(int d, const double W[5], const double U[5], double F[5]) {
 
 // One side of a Riemann problem in the rotated frame (n = normal, t1, t2 = tangential).
 struct Side {
-  double U[5];   // D, M_n, M_t1, M_t2, Etilde
-  double F[5];   // physical flux along n = U v_n + pt
-  double pt[5];  // its pressure terms (0, p, 0, 0, p v_n)
-  double p, vn, lam_m, lam_p;
-  double dp, dm; // lam_p - v_n and v_n - lam_m (both >= 0), formed without cancellation (reading S6)
-  double cp, cm; // 1 - lam_p and 1 + lam_m, formed without cancellation (reading S6)
+  real U[5];   // D, M_n, M_t1, M_t2, Etilde
+  real F[5];   // physical flux along n = U v_n + pt
+  real pt[5];  // its pressure terms (0, p, 0, 0, p v_n)
+  real p, vn, lam_m, lam_p;
+  real dp, dm; // lam_p - v_n and v_n - lam_m (both >= 0), formed without cancellation (reading S6)
+  real cp, cm; // 1 - lam_p and 1 + lam_m, formed without cancellation (reading S6)
 };
 // Acoustic eigenvalues in 4-velocity form (reading S6):
 //   lambda_pm = (gamma U_n +- U_s Q) / (gamma^2 + U_s^2),  Q = sqrt(1 + U_t^2 + U_s^2)
@@ -269,34 +273,34 @@ struct Side {
 //                                  1 - |lambda|   = a^2 / ((gamma + u)(Q + U_s)(gamma Q + u U_s));
 //   wave running AGAINST the flow: |lambda - v_n| = U_s (gamma Q + u U_s) / (gamma (gamma^2 + U_s^2)),
 //                                  1 - |lambda| needs no care there (|lambda| stays well below 1).
-void side_setup(int d, const double W[5], const double U[5], Side& s) {
+void side_setup(int d, const real W[5], const real U[5], Side& s) {
   const int n = 1 + d, t1 = 1 + (d + 1) % 3, t2 = 1 + (d + 2) % 3;
-  const double rho = W[0], Un = W[n], Ut1 = W[t1], Ut2 = W[t2], p = W[4];
-  const double T = p / rho;
-  const double cs2 = cs2_of_T(T);                             // Eq. 14 (TM sound speed)
-  const double Us2 = cs2 / (1.0 - cs2);
-  const double Us = std::sqrt(Us2);
-  const double Utsq = Ut1 * Ut1 + Ut2 * Ut2;
-  const double g2 = 1.0 + (Un * Un + Utsq);
-  const double gamma = std::sqrt(g2);
-  const double Q = std::sqrt(1.0 + Utsq + Us2);
+  const real rho = W[0], Un = W[n], Ut1 = W[t1], Ut2 = W[t2], p = W[4];
+  const real T = p / rho;
+  const real cs2 = cs2_of_T(T);                             // Eq. 14 (TM sound speed)
+  const real Us2 = cs2 / (real(1.0) - cs2);
+  const real Us = std::sqrt(Us2);
+  const real Utsq = Ut1 * Ut1 + Ut2 * Ut2;
+  const real g2 = real(1.0) + (Un * Un + Utsq);
+  const real gamma = std::sqrt(g2);
+  const real Q = std::sqrt(real(1.0) + Utsq + Us2);
   s.lam_p = (gamma * Un + Us * Q) / (g2 + Us2);
   s.lam_m = (gamma * Un - Us * Q) / (g2 + Us2);
   s.vn = Un / gamma;
-  const double a = 1.0 + Utsq, u = std::fabs(Un);
-  const double w = gamma * Q + u * Us;
-  const double d_with = Us * a / (gamma * w);
-  const double d_against = Us * w / (gamma * (g2 + Us2));
-  const double c_with = a * a / ((gamma + u) * (Q + Us) * w);
-  if (Un >= 0.0) {
+  const real a = real(1.0) + Utsq, u = std::fabs(Un);
+  const real w = gamma * Q + u * Us;
+  const real d_with = Us * a / (gamma * w);
+  const real d_against = Us * w / (gamma * (g2 + Us2));
+  const real c_with = a * a / ((gamma + u) * (Q + Us) * w);
+  if (Un >= real(0.0)) {
     s.dp = d_with;
     s.dm = d_against;
     s.cp = c_with;
-    s.cm = 1.0 + s.lam_m;
+    s.cm = real(1.0) + s.lam_m;
   } else {
     s.dp = d_against;
     s.dm = d_with;
-    s.cp = 1.0 - s.lam_p;
+    s.cp = real(1.0) - s.lam_p;
     s.cm = c_with;
   }
   s.p = p;
@@ -305,10 +309,10 @@ void side_setup(int d, const double W[5], const double U[5], Side& s) {
   s.U[2] = U[t1];
   s.U[3] = U[t2];
   s.U[4] = U[4];
-  s.pt[0] = 0.0;
+  s.pt[0] = real(0.0);
   s.pt[1] = p;
-  s.pt[2] = 0.0;
-  s.pt[3] = 0.0;
+  s.pt[2] = real(0.0);
+  s.pt[3] = real(0.0);
   s.pt[4] = p * s.vn;
   s.F[0] = s.U[0] * s.vn;
   s.F[1] = s.U[1] * s.vn + p;
@@ -329,7 +333,7 @@ void side_setup(int d, const double W[5], const double U[5], Side& s) {
 //   F^hll = (S_R B_L U_L + S_L A_R U_R + S_R pt_L - S_L pt_R)/(S_R - S_L)
 // S_R may belong to either side, v_R to the right one: A_R = (lam_p - v_n)_R + (S_R - (lam_p)_R).
 struct Hll {
-  double SL, SR, AR, BL;
+  real SL, SR, AR, BL;
 };
 Hll hll_speeds(const Side& L, const Side& R) {
   Hll h;
@@ -338,50 +342,50 @@ Hll hll_speeds(const Side& L, const Side& R) {
   // S_R - lam_p of the RIGHT state (zero unless the left state sets S_R): near the light cone as a
   // difference of the complements 1 - lambda (tiny numbers known to full relative accuracy), elsewhere of
   // the speeds themselves -- whichever pair of operands is the smaller one
-  const double cpS = std::min(L.cp, R.cp), cmS = std::min(L.cm, R.cm);   // 1 - S_R, 1 + S_L
-  h.AR = R.dp + ((h.SR > 0.5) ? (R.cp - cpS) : (h.SR - R.lam_p));
-  h.BL = L.dm + ((h.SL < -0.5) ? (L.cm - cmS) : (L.lam_m - h.SL));
+  const real cpS = std::min(L.cp, R.cp), cmS = std::min(L.cm, R.cm);   // 1 - S_R, 1 + S_L
+  h.AR = R.dp + ((h.SR > real(0.5)) ? (R.cp - cpS) : (h.SR - R.lam_p));
+  h.BL = L.dm + ((h.SL < -real(0.5)) ? (L.cm - cmS) : (L.lam_m - h.SL));
   return h;
 }
 // HLLE (Mignone & Bodo 2005 form with the S6 speeds); rotated frame
-void hlle_rot(const Side& L, const Side& R, double F[5]) {
+void hlle_rot(const Side& L, const Side& R, real F[5]) {
   const Hll h = hll_speeds(L, R);
-  const double SL = h.SL, SR = h.SR, AR = h.AR, BL = h.BL;
-  if (SL >= 0.0) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
-  if (SR <= 0.0) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
-  const double den = SR - SL;
+  const real SL = h.SL, SR = h.SR, AR = h.AR, BL = h.BL;
+  if (SL >= real(0.0)) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
+  if (SR <= real(0.0)) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
+  const real den = SR - SL;
   for (int c = 0; c < 5; ++c)
     F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;
 }
 // HLLC adapted to Etilde ("replacing E with Etilde + D c^2"; reading S7); rotated frame
-void hllc_rot(const Side& L, const Side& R, double F[5]) {
+void hllc_rot(const Side& L, const Side& R, real F[5]) {
   const Hll h = hll_speeds(L, R);
-  const double SL = h.SL, SR = h.SR, AR = h.AR, BL = h.BL;
-  if (SL >= 0.0) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
-  if (SR <= 0.0) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
-  const double den = SR - SL;
-  double Uh[5], Fh[5];                                        // HLL state and flux
+  const real SL = h.SL, SR = h.SR, AR = h.AR, BL = h.BL;
+  if (SL >= real(0.0)) { for (int c = 0; c < 5; ++c) F[c] = L.F[c]; return; }
+  if (SR <= real(0.0)) { for (int c = 0; c < 5; ++c) F[c] = R.F[c]; return; }
+  const real den = SR - SL;
+  real Uh[5], Fh[5];                                        // HLL state and flux
   for (int c = 0; c < 5; ++c) {
     Uh[c] = (AR * R.U[c] + BL * L.U[c] + (L.pt[c] - R.pt[c])) / den;
     Fh[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;
   }
 #if SRHD_REF_SCHEME == 0
-  const double Eh = Uh[4] + Uh[0];                            // E = Etilde + D   (sums only)
-  const double FEh = Fh[4] + Fh[0];
+  const real Eh = Uh[4] + Uh[0];                            // E = Etilde + D   (sums only)
+  const real FEh = Fh[4] + Fh[0];
 #else
-  const double Eh = Uh[4];                                    // original scheme: the fifth variable IS E
-  const double FEh = Fh[4];
+  const real Eh = Uh[4];                                    // original scheme: the fifth variable IS E
+  const real FEh = Fh[4];
 #endif
-  const double a = FEh, b = Eh + Fh[1], m = Uh[1];
+  const real a = FEh, b = Eh + Fh[1], m = Uh[1];
   // contact speed: root of a lam^2 - b lam + m = 0 in (-1,1), rationalised (safe for a -> 0)
-  const double lam = 2.0 * m / (b + std::sqrt(b * b - 4.0 * a * m));
-  const double ps = Fh[1] - lam * FEh;                        // p*
-  const bool left = lam >= 0.0;
+  const real lam = real(2.0) * m / (b + std::sqrt(b * b - real(4.0) * a * m));
+  const real ps = Fh[1] - lam * FEh;                        // p*
+  const bool left = lam >= real(0.0);
   const Side& K = left ? L : R;
-  const double S = left ? SL : SR;
-  const double A = left ? -BL : AR;                           // S - v_n of side K
-  const double dK = S - lam;                                  // S and lam have opposite signs: a sum
-  double Us[5];
+  const real S = left ? SL : SR;
+  const real A = left ? -BL : AR;                           // S - v_n of side K
+  const real dK = S - lam;                                  // S and lam have opposite signs: a sum
+  real Us[5];
   Us[0] = K.U[0] * A / dK;
   Us[1] = (K.U[1] * A + ps - K.p) / dK;
   Us[2] = K.U[2] * A / dK;
@@ -395,12 +399,12 @@ void hllc_rot(const Side& L, const Side& R, double F[5]) {
   F[3] = Us[3] * lam;
   F[4] = (Us[4] + ps) * lam;
 }
-void riemann_flux(int riemann, int d, const double WL[5], const double UL[5], const double WR[5],
-                  const double UR[5], double F[5]) {
+void riemann_flux(int riemann, int d, const real WL[5], const real UL[5], const real WR[5],
+                  const real UR[5], real F[5]) {
   Side L, R;
   side_setup(d, WL, UL, L);
   side_setup(d, WR, UR, R);
-  double Fr[5];
+  real Fr[5];
   if (riemann == 0) hlle_rot(L, R, Fr); else hllc_rot(L, R, Fr);
   const int n = 1 + d, t1 = 1 + (d + 1) % 3, t2 = 1 + (d + 2) % 3;
   F[0] = Fr[0];
@@ -412,39 +416,39 @@ void riemann_flux(int riemann, int d, const double WL[5], const double UL[5], co
 
 // ---------------------------------------------------------------- reconstruction ----------------
 // reading S3: van Leer harmonic mean capped by generalised minmod with coefficient beta
-double limited_slope(double sL, double sR, double beta) {
-  if (sL * sR <= 0.0) return 0.0;
-  const double vl = 2.0 * std::fabs(sL * sR) / std::fabs(sL + sR);
-  const double mm = beta * std::min(std::fabs(sL), std::fabs(sR));
-  const double mag = std::min(vl, mm);
-  return (sL > 0.0) ? mag : -mag;
+real limited_slope(real sL, real sR, real beta) {
+  if (sL * sR <= real(0.0)) return real(0.0);
+  const real vl = real(2.0) * std::fabs(sL * sR) / std::fabs(sL + sR);
+  const real mm = beta * std::min(std::fabs(sL), std::fabs(sR));
+  const real mag = std::min(vl, mm);
+  return (sL > real(0.0)) ? mag : -mag;
 }
 // a[0..4] = a_{i-2..i+2}; returns the left/right edge values of cell i.
 // PLM: a -+ d/2.  PPM (reading S4): Colella & Woodward 1984 on a uniform grid.
-void recon_1d(int recon, const double a[5], double beta, double beta0, double& am, double& ap) {
-  const double ai = a[2];
+void recon_1d(int recon, const real a[5], real beta, real beta0, real& am, real& ap) {
+  const real ai = a[2];
   if (recon == 0) {
-    const double d = limited_slope(ai - a[1], a[3] - ai, beta);
-    am = ai - 0.5 * d;
-    ap = ai + 0.5 * d;
+    const real d = limited_slope(ai - a[1], a[3] - ai, beta);
+    am = ai - real(0.5) * d;
+    ap = ai + real(0.5) * d;
     return;
   }
-  const double dm = limited_slope(a[1] - a[0], a[2] - a[1], beta);   // d_{i-1}
-  const double d0 = limited_slope(a[2] - a[1], a[3] - a[2], beta);   // d_i
-  const double dp = limited_slope(a[3] - a[2], a[4] - a[3], beta);   // d_{i+1}
-  am = 0.5 * (a[1] + a[2]) - (d0 - dm) / 6.0;                         // face i-1/2
-  ap = 0.5 * (a[2] + a[3]) - (dp - d0) / 6.0;                         // face i+1/2
-  if ((ap - ai) * (ai - am) <= 0.0) {                                 // CW84 Eq. 1.10
+  const real dm = limited_slope(a[1] - a[0], a[2] - a[1], beta);   // d_{i-1}
+  const real d0 = limited_slope(a[2] - a[1], a[3] - a[2], beta);   // d_i
+  const real dp = limited_slope(a[3] - a[2], a[4] - a[3], beta);   // d_{i+1}
+  am = real(0.5) * (a[1] + a[2]) - (d0 - dm) / real(6.0);                         // face i-1/2
+  ap = real(0.5) * (a[2] + a[3]) - (dp - d0) / real(6.0);                         // face i+1/2
+  if ((ap - ai) * (ai - am) <= real(0.0)) {                                 // CW84 Eq. 1.10
     am = ai;
     ap = ai;
   } else {
-    const double dd = ap - am;
-    const double c6 = 6.0 * (ai - 0.5 * (am + ap));
-    if (dd * c6 > dd * dd) am = 3.0 * ai - 2.0 * ap;
-    else if (-(dd * dd) > dd * c6) ap = 3.0 * ai - 2.0 * am;
+    const real dd = ap - am;
+    const real c6 = real(6.0) * (ai - real(0.5) * (am + ap));
+    if (dd * c6 > dd * dd) am = real(3.0) * ai - real(2.0) * ap;
+    else if (-(dd * dd) > dd * c6) ap = real(3.0) * ai - real(2.0) * am;
   }
   if (beta != beta0) {                                                // retry blend (reading S4)
-    const double w = beta / beta0;
+    const real w = beta / beta0;
     am = ai + w * (am - ai);
     ap = ai + w * (ap - ai);
   }
@@ -462,8 +466,8 @@ struct Box {
 
 // flux_keep (optional, 3*5*padded cells): receives the Riemann fluxes of the ACCEPTED pass,
 // [dir][comp][cell c] = flux through the face between c and c + 1 along dir
-int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt, double dh,
-             const srhd_ref_params& par, srhd_ref_stats& st, double* flux_keep = nullptr) {
+int step_box(const real* cons_in, real* cons_out, int nx, int ny, int nz, real dt, real dh,
+             const srhd_ref_params& par, srhd_ref_stats& st, real* flux_keep = nullptr) {
   const int g = par.ghost;
   Box b{nx, ny, nz, g, nx + 2 * g, ny + 2 * g, nz + 2 * g, 0};
   b.cstride = (size_t)b.sx * b.sy * b.sz;
@@ -472,13 +476,13 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
   const int stp[3] = {1, b.sx, b.sx * b.sy};
 
   // O5a: W = C2P(U) for every tile cell (incl. ghosts); pass independent
-  std::vector<double> Wc(5 * np);
-  double umax = 0.0;
+  std::vector<real> Wc(5 * np);
+  real umax = real(0.0);
   for (int k = -g; k < nz + g; ++k)
     for (int j = -g; j < ny + g; ++j)
       for (int i = -g; i < nx + g; ++i) {
         const size_t c = b.at(i, j, k);
-        double U[5], W[5];
+        real U[5], W[5];
         for (int q = 0; q < 5; ++q) U[q] = cons_in[q * np + c];
         int it = 0;
         const bool phys = cons2prim(U, W, par.newton_rtol, par.newton_max_iter, &it, nullptr);
@@ -490,18 +494,18 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
           umax = std::max(umax, umax_of_prim(W));             // A2 / O4 on the input interior
         }
       }
-  st.max_speed = std::max(st.max_speed, smax_of_umax(umax));
+  st.max_speed = std::max(st.max_speed, (double)smax_of_umax(umax));
 
   // face states of the cells that are face-adjacent to the interior (at most one index outside)
-  std::vector<double> Um(3 * 5 * np), Up(3 * 5 * np);         // [dir][comp][cell] evolved cons
-  std::vector<double> Fx(5 * np);                             // scratch for one direction's fluxes
-  std::vector<double> Flux(3 * 5 * np);                       // [dir][comp][cell c] = F at c+1/2 n
+  std::vector<real> Um(3 * 5 * np), Up(3 * 5 * np);         // [dir][comp][cell] evolved cons
+  std::vector<real> Fx(5 * np);                             // scratch for one direction's fluxes
+  std::vector<real> Flux(3 * 5 * np);                       // [dir][comp][cell c] = F at c+1/2 n
   const int K = par.max_retry;
-  double beta = par.minmod_coeff;
+  real beta = par.minmod_coeff;
   unsigned long long face_fail = 0, cell_fail = 0, face_iters = 0;
   int pass = 0;
   for (;; ++pass) {
-    if (pass > 0) beta = (pass <= K) ? beta * 0.75 : 0.0;     // P:273, reading S9
+    if (pass > 0) beta = (pass <= K) ? beta * real(0.75) : real(0.0);     // P:273, reading S9
     face_fail = 0;
     cell_fail = 0;
     face_iters = 0;
@@ -512,29 +516,29 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
           const int nout = (i < 0 || i >= nx) + (j < 0 || j >= ny) + (k < 0 || k >= nz);
           if (nout > 1) continue;
           const size_t c = b.at(i, j, k);
-          double Wm[3][5], Wp[3][5];
+          real Wm[3][5], Wp[3][5];
           for (int d = 0; d < 3; ++d)
             for (int q = 0; q < 5; ++q) {
-              double a[5];
+              real a[5];
               for (int m = -2; m <= 2; ++m) {
                 // PLM touches only m = -1..1; guard the read for PLM's narrower ghost zone
-                a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0
+                a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? real(0.0)
                                                                      : Wc[q * np + c + (ptrdiff_t)m * stp[d]];
               }
               recon_1d(par.recon, a, beta, par.minmod_coeff, Wm[d][q], Wp[d][q]);
             }
           // O6: MUSCL-Hancock half step (reading S5), 3-D unsplit
-          double Ucm[3][5], Ucp[3][5], dU[5];
-          double dF[3][5];
+          real Ucm[3][5], Ucp[3][5], dU[5];
+          real dF[3][5];
           for (int d = 0; d < 3; ++d) {
-            double Fm[5], Fp[5];
+            real Fm[5], Fp[5];
             prim2cons(Wm[d], Ucm[d]);
             prim2cons(Wp[d], Ucp[d]);
             phys_flux(d, Wm[d], Ucm[d], Fm);
             phys_flux(d, Wp[d], Ucp[d], Fp);
             for (int q = 0; q < 5; ++q) dF[d][q] = Fp[q] - Fm[q];
           }
-          const double hdt = dt / (2.0 * dh);
+          const real hdt = dt / (real(2.0) * dh);
           for (int q = 0; q < 5; ++q) dU[q] = -hdt * ((dF[0][q] + dF[1][q]) + dF[2][q]);
           for (int d = 0; d < 3; ++d)
             for (int q = 0; q < 5; ++q) {
@@ -550,7 +554,7 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
         for (int j = lo[1]; j <= hi[1]; ++j)
           for (int i = lo[0]; i <= hi[0]; ++i) {
             const size_t c = b.at(i, j, k), cr = c + stp[d];
-            double UL[5], UR[5], WL[5], WR[5], F[5];
+            real UL[5], UR[5], WL[5], WR[5], F[5];
             for (int q = 0; q < 5; ++q) {
               UL[q] = Up[(d * 5 + q) * np + c];
               UR[q] = Um[(d * 5 + q) * np + cr];
@@ -565,24 +569,24 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
           }
     }
     // O8: update (reading S12: ((x)+(y))+(z), each (F+ - F-) first)
-    const double dtdh = dt / dh;
+    const real dtdh = dt / dh;
     const size_t no = (size_t)nx * ny * nz;
     for (int k = 0; k < nz; ++k)
       for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
           const size_t c = b.at(i, j, k);
-          double Un[5];
+          real Un[5];
           for (int q = 0; q < 5; ++q) {
-            const double dfx = Flux[(0 * 5 + q) * np + c] - Flux[(0 * 5 + q) * np + c - stp[0]];
-            const double dfy = Flux[(1 * 5 + q) * np + c] - Flux[(1 * 5 + q) * np + c - stp[1]];
-            const double dfz = Flux[(2 * 5 + q) * np + c] - Flux[(2 * 5 + q) * np + c - stp[2]];
+            const real dfx = Flux[(0 * 5 + q) * np + c] - Flux[(0 * 5 + q) * np + c - stp[0]];
+            const real dfy = Flux[(1 * 5 + q) * np + c] - Flux[(1 * 5 + q) * np + c - stp[1]];
+            const real dfz = Flux[(2 * 5 + q) * np + c] - Flux[(2 * 5 + q) * np + c - stp[2]];
             Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);
             cons_out[q * no + ((size_t)k * ny + j) * nx + i] = Un[q];
           }
           if (!is_physical(Un)) ++cell_fail;                  // O9: Eq. 30 on the updated cell
         }
     (void)ext;
-    if ((face_fail == 0 && cell_fail == 0) || beta == 0.0) break;   // S9, S10
+    if ((face_fail == 0 && cell_fail == 0) || beta == real(0.0)) break;   // S9, S10
   }
   if (flux_keep) std::copy(Flux.begin(), Flux.end(), flux_keep);
   if (pass > 0) ++st.n_retry_pg;
@@ -605,8 +609,8 @@ int step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, do
 //   V5  second-order fluxes F2 = Riemann(edge states) at every face touching an interior cell
 //   V6  Unew = U - dt/dh ((F2x+ - F2x-) + (F2y+ - F2y-)) + (F2z+ - F2z-));  Eq. 30 check, retry (S9, S10)
 // Stages V1-V3 do not depend on the pass.  Ghost width: one more than MUSCL-Hancock (PLM 3, PPM 4).
-int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt, double dh,
-                const srhd_ref_params& par, srhd_ref_stats& st, double* flux_keep = nullptr) {
+int step_box_vl(const real* cons_in, real* cons_out, int nx, int ny, int nz, real dt, real dh,
+                const srhd_ref_params& par, srhd_ref_stats& st, real* flux_keep = nullptr) {
   const int g = par.ghost;
   Box b{nx, ny, nz, g, nx + 2 * g, ny + 2 * g, nz + 2 * g, 0};
   b.cstride = (size_t)b.sx * b.sy * b.sz;
@@ -614,13 +618,13 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
   const int stp[3] = {1, b.sx, b.sx * b.sy};
   const int ext[3] = {nx, ny, nz};
   // V1
-  std::vector<double> Wc(5 * np);
-  double umax = 0.0;
+  std::vector<real> Wc(5 * np);
+  real umax = real(0.0);
   for (int k = -g; k < nz + g; ++k)
     for (int j = -g; j < ny + g; ++j)
       for (int i = -g; i < nx + g; ++i) {
         const size_t c = b.at(i, j, k);
-        double U[5], W[5];
+        real U[5], W[5];
         for (int q = 0; q < 5; ++q) U[q] = cons_in[q * np + c];
         int it = 0;
         const bool phys = cons2prim(U, W, par.newton_rtol, par.newton_max_iter, &it, nullptr);
@@ -632,16 +636,16 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
           umax = std::max(umax, umax_of_prim(W));
         }
       }
-  st.max_speed = std::max(st.max_speed, smax_of_umax(umax));
+  st.max_speed = std::max(st.max_speed, (double)smax_of_umax(umax));
   // V2: first-order fluxes; F1[(d*5+q)*np + c] = flux through the face between c and c + n_d
   const int lo = -(g - 1), hx = nx + g - 2, hy = ny + g - 2, hz = nz + g - 2;   // cells that get a predictor
-  std::vector<double> F1(3 * 5 * np, 0.0);
+  std::vector<real> F1(3 * 5 * np, real(0.0));
   for (int d = 0; d < 3; ++d)
     for (int k = lo - (d == 2); k <= hz; ++k)
       for (int j = lo - (d == 1); j <= hy; ++j)
         for (int i = lo - (d == 0); i <= hx; ++i) {
           const size_t c = b.at(i, j, k), cr = c + stp[d];
-          double UL[5], UR[5], WL[5], WR[5], F[5];
+          real UL[5], UR[5], WL[5], WR[5], F[5];
           for (int q = 0; q < 5; ++q) {
             UL[q] = cons_in[q * np + c];
             UR[q] = cons_in[q * np + cr];
@@ -652,18 +656,18 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
           for (int q = 0; q < 5; ++q) F1[(d * 5 + q) * np + c] = F[q];
         }
   // V3: predictor and its primitives
-  std::vector<double> Wh(5 * np, 0.0);
+  std::vector<real> Wh(5 * np, real(0.0));
   unsigned long long half_fail = 0, half_iters = 0;
-  const double hdt = dt / (2.0 * dh);
+  const real hdt = dt / (real(2.0) * dh);
   for (int k = lo; k <= hz; ++k)
     for (int j = lo; j <= hy; ++j)
       for (int i = lo; i <= hx; ++i) {
         const size_t c = b.at(i, j, k);
-        double Uh[5], W[5];
+        real Uh[5], W[5];
         for (int q = 0; q < 5; ++q) {
-          const double dfx = F1[(0 * 5 + q) * np + c] - F1[(0 * 5 + q) * np + c - stp[0]];
-          const double dfy = F1[(1 * 5 + q) * np + c] - F1[(1 * 5 + q) * np + c - stp[1]];
-          const double dfz = F1[(2 * 5 + q) * np + c] - F1[(2 * 5 + q) * np + c - stp[2]];
+          const real dfx = F1[(0 * 5 + q) * np + c] - F1[(0 * 5 + q) * np + c - stp[0]];
+          const real dfy = F1[(1 * 5 + q) * np + c] - F1[(1 * 5 + q) * np + c - stp[1]];
+          const real dfz = F1[(2 * 5 + q) * np + c] - F1[(2 * 5 + q) * np + c - stp[2]];
           Uh[q] = cons_in[q * np + c] - hdt * ((dfx + dfy) + dfz);
         }
         int it = 0;
@@ -672,14 +676,14 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
         for (int q = 0; q < 5; ++q) Wh[q * np + c] = W[q];
       }
   st.newton_iters += half_iters;
-  std::vector<double> Um(3 * 5 * np), Up(3 * 5 * np), Wm(3 * 5 * np), Wp(3 * 5 * np);
-  std::vector<double> Flux(3 * 5 * np);
+  std::vector<real> Um(3 * 5 * np), Up(3 * 5 * np), Wm(3 * 5 * np), Wp(3 * 5 * np);
+  std::vector<real> Flux(3 * 5 * np);
   const int K = par.max_retry;
-  double beta = par.minmod_coeff;
+  real beta = par.minmod_coeff;
   unsigned long long cell_fail = 0;
   int pass = 0;
   for (;; ++pass) {
-    if (pass > 0) beta = (pass <= K) ? beta * 0.75 : 0.0;     // P:273, reading S9
+    if (pass > 0) beta = (pass <= K) ? beta * real(0.75) : real(0.0);     // P:273, reading S9
     cell_fail = 0;
     // V4: edge states of the cells that are face-adjacent to the interior
     for (int k = -1; k <= nz; ++k)
@@ -689,11 +693,11 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
           if (nout > 1) continue;
           const size_t c = b.at(i, j, k);
           for (int d = 0; d < 3; ++d) {
-            double wm[5], wp[5], um[5], up[5];
+            real wm[5], wp[5], um[5], up[5];
             for (int q = 0; q < 5; ++q) {
-              double a[5];
+              real a[5];
               for (int m = -2; m <= 2; ++m)
-                a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0 : Wh[q * np + c + (ptrdiff_t)m * stp[d]];
+                a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? real(0.0) : Wh[q * np + c + (ptrdiff_t)m * stp[d]];
               recon_1d(par.recon, a, beta, par.minmod_coeff, wm[q], wp[q]);
             }
             prim2cons(wm, um);
@@ -714,7 +718,7 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
         for (int j = l3[1]; j <= h3[1]; ++j)
           for (int i = l3[0]; i <= h3[0]; ++i) {
             const size_t c = b.at(i, j, k), cr = c + stp[d];
-            double UL[5], UR[5], WL[5], WR[5], F[5];
+            real UL[5], UR[5], WL[5], WR[5], F[5];
             for (int q = 0; q < 5; ++q) {
               UL[q] = Up[(d * 5 + q) * np + c];
               WL[q] = Wp[(d * 5 + q) * np + c];
@@ -726,17 +730,17 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
           }
     }
     // V6
-    const double dtdh = dt / dh;
+    const real dtdh = dt / dh;
     const size_t no = (size_t)nx * ny * nz;
     for (int k = 0; k < nz; ++k)
       for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
           const size_t c = b.at(i, j, k);
-          double Un[5];
+          real Un[5];
           for (int q = 0; q < 5; ++q) {
-            const double dfx = Flux[(0 * 5 + q) * np + c] - Flux[(0 * 5 + q) * np + c - stp[0]];
-            const double dfy = Flux[(1 * 5 + q) * np + c] - Flux[(1 * 5 + q) * np + c - stp[1]];
-            const double dfz = Flux[(2 * 5 + q) * np + c] - Flux[(2 * 5 + q) * np + c - stp[2]];
+            const real dfx = Flux[(0 * 5 + q) * np + c] - Flux[(0 * 5 + q) * np + c - stp[0]];
+            const real dfy = Flux[(1 * 5 + q) * np + c] - Flux[(1 * 5 + q) * np + c - stp[1]];
+            const real dfz = Flux[(2 * 5 + q) * np + c] - Flux[(2 * 5 + q) * np + c - stp[2]];
             Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);
             cons_out[q * no + ((size_t)k * ny + j) * nx + i] = Un[q];
           }
@@ -745,7 +749,7 @@ int step_box_vl(const double* cons_in, double* cons_out, int nx, int ny, int nz,
     (void)ext;
     // the predictor does not depend on beta: if IT failed, no rung can cure it -- go straight to the last
     // rung's verdict (accept and count), like a face failure in the beta = 0 pass of MUSCL-Hancock (S15)
-    if (cell_fail == 0 || beta == 0.0) break;
+    if (cell_fail == 0 || beta == real(0.0)) break;
   }
   if (flux_keep) std::copy(Flux.begin(), Flux.end(), flux_keep);
   if (pass > 0) ++st.n_retry_pg;
@@ -767,26 +771,26 @@ inline int map_index(int i, int n, int bc_lo, int bc_hi) {
 // =================================================================== C entry points ============
 extern "C" {
 
-double srhd_ref_htilde_of_T(double T) { return htilde_of_T(T); }
-double srhd_ref_T_of_htilde(double ht) { return T_of_htilde(ht); }
-double srhd_ref_dT_dhtilde(double ht) { return dT_dhtilde(ht); }
-double srhd_ref_cs2_of_T(double T) { return cs2_of_T(T); }
-double srhd_ref_f_eq15(double ht, double musq) { return f_eq15(ht, T_of_htilde(ht), musq); }
-double srhd_ref_df_eqA1(double ht, double musq) {
+real srhd_ref_htilde_of_T(real T) { return htilde_of_T(T); }
+real srhd_ref_T_of_htilde(real ht) { return T_of_htilde(ht); }
+real srhd_ref_dT_dhtilde(real ht) { return dT_dhtilde(ht); }
+real srhd_ref_cs2_of_T(real T) { return cs2_of_T(T); }
+real srhd_ref_f_eq15(real ht, real musq) { return f_eq15(ht, T_of_htilde(ht), musq); }
+real srhd_ref_df_eqA1(real ht, real musq) {
   return df_eqA1(ht, T_of_htilde(ht), dT_dhtilde(ht), musq);
 }
-double srhd_ref_htilde_guess(double L, double musq) { return htilde_guess(L, musq); }
-double srhd_ref_umax_of_prim(const double W[5]) { return umax_of_prim(W); }
-double srhd_ref_smax_of_umax(double umax) { return smax_of_umax(umax); }
-double srhd_ref_limited_slope(double sL, double sR, double beta) { return limited_slope(sL, sR, beta); }
-void srhd_ref_recon_1d(int recon, const double* a, double beta, double beta0, double* am, double* ap) {
+real srhd_ref_htilde_guess(real L, real musq) { return htilde_guess(L, musq); }
+real srhd_ref_umax_of_prim(const real W[5]) { return umax_of_prim(W); }
+real srhd_ref_smax_of_umax(real umax) { return smax_of_umax(umax); }
+real srhd_ref_limited_slope(real sL, real sR, real beta) { return limited_slope(sL, sR, beta); }
+void srhd_ref_recon_1d(int recon, const real* a, real beta, real beta0, real* am, real* ap) {
   recon_1d(recon, a, beta, beta0, *am, *ap);
 }
-void srhd_ref_phys_flux(int dir, const double* W, const double* U, double* F) { phys_flux(dir, W, U, F); }
+void srhd_ref_phys_flux(int dir, const real* W, const real* U, real* F) { phys_flux(dir, W, U, F); }
 // test hook: the acoustic wave speeds of one state along dir (reading S6);
 // out = {lambda_-, lambda_+, lambda_+ - v_n, v_n - lambda_-, 1 - lambda_+, 1 + lambda_-}
-void srhd_ref_wave_speeds(int dir, const double* W, double* out) {
-  double U[5];
+void srhd_ref_wave_speeds(int dir, const real* W, real* out) {
+  real U[5];
   prim2cons(W, U);
   Side s;
   side_setup(dir, W, U, s);
@@ -797,27 +801,27 @@ void srhd_ref_wave_speeds(int dir, const double* W, double* out) {
   out[4] = s.cp;
   out[5] = s.cm;
 }
-void srhd_ref_riemann_flux(int riemann, int dir, const double* WL, const double* UL, const double* WR,
-                           const double* UR, double* F) {
+void srhd_ref_riemann_flux(int riemann, int dir, const real* WL, const real* UL, const real* WR,
+                           const real* UR, real* F) {
   riemann_flux(riemann, dir, WL, UL, WR, UR, F);
 }
 
-void srhd_ref_prim2cons(const double* prim, double* cons, size_t n, size_t stride) {
+void srhd_ref_prim2cons(const real* prim, real* cons, size_t n, size_t stride) {
 #pragma omp parallel for schedule(static)
   for (long long i = 0; i < (long long)n; ++i) {
-    double W[5], U[5];
+    real W[5], U[5];
     for (int q = 0; q < 5; ++q) W[q] = prim[q * stride + i];
     prim2cons(W, U);
     for (int q = 0; q < 5; ++q) cons[q * stride + i] = U[q];
   }
 }
 
-void srhd_ref_cons2prim_diag(const double* cons, double* prim, size_t n, size_t stride,
-                             const srhd_ref_params* par, double* htilde, int* iters,
+void srhd_ref_cons2prim_diag(const real* cons, real* prim, size_t n, size_t stride,
+                             const srhd_ref_params* par, real* htilde, int* iters,
                              unsigned char* unphys) {
 #pragma omp parallel for schedule(static)
   for (long long i = 0; i < (long long)n; ++i) {
-    double W[5], U[5], ht;
+    real W[5], U[5], ht;
     int it;
     for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
     const bool phys = cons2prim(U, W, par->newton_rtol, par->newton_max_iter, &it, &ht);
@@ -828,12 +832,12 @@ void srhd_ref_cons2prim_diag(const double* cons, double* prim, size_t n, size_t 
   }
 }
 
-void srhd_ref_cons2prim(const double* cons, double* prim, size_t n, size_t stride,
+void srhd_ref_cons2prim(const real* cons, real* prim, size_t n, size_t stride,
                         const srhd_ref_params* par, srhd_ref_stats* stats) {
   unsigned long long nfail = 0, niter = 0;
 #pragma omp parallel for schedule(static) reduction(+ : nfail, niter)
   for (long long i = 0; i < (long long)n; ++i) {
-    double W[5], U[5];
+    real W[5], U[5];
     int it;
     for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
     if (!cons2prim(U, W, par->newton_rtol, par->newton_max_iter, &it, nullptr)) ++nfail;
@@ -847,12 +851,12 @@ void srhd_ref_cons2prim(const double* cons, double* prim, size_t n, size_t strid
   }
 }
 
-void srhd_ref_max_signal_speed(const double* cons, size_t n, size_t stride,
-                               const srhd_ref_params* par, double* max_speed) {
-  double umax = 0.0;
+void srhd_ref_max_signal_speed(const real* cons, size_t n, size_t stride,
+                               const srhd_ref_params* par, real* max_speed) {
+  real umax = real(0.0);
 #pragma omp parallel for schedule(static) reduction(max : umax)
   for (long long i = 0; i < (long long)n; ++i) {
-    double W[5], U[5];
+    real W[5], U[5];
     for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
     cons2prim(U, W, par->newton_rtol, par->newton_max_iter, nullptr, nullptr);
     umax = std::max(umax, umax_of_prim(W));
@@ -860,8 +864,8 @@ void srhd_ref_max_signal_speed(const double* cons, size_t n, size_t stride,
   *max_speed = smax_of_umax(umax);                            // monotone: convert once (O4)
 }
 
-int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, int nz, double dt,
-                      double dh, const srhd_ref_params* par, srhd_ref_stats* stats) {
+int srhd_ref_step_box(const real* cons_in, real* cons_out, int nx, int ny, int nz, real dt,
+                      real dh, const srhd_ref_params* par, srhd_ref_stats* stats) {
   srhd_ref_stats st;
   std::memset(&st, 0, sizeof(st));
   const int passes = (par->integrator == 1 ? step_box_vl : step_box)(cons_in, cons_out, nx, ny, nz, dt, dh, *par, st, nullptr);
@@ -873,20 +877,20 @@ int srhd_ref_step_box(const double* cons_in, double* cons_out, int nx, int ny, i
 // the AMR driver's flux-correction step consumes.  flux_out (may be null): [npg][8][6][5][8][8],
 // patch p (S13), face 0 x-lo, 1 x-hi, 2 y-lo, 3 y-hi, 4 z-lo, 5 z-hi, component, then the two in-face
 // cell coordinates, slower one first: (z,y) on x faces, (z,x) on y faces, (y,x) on z faces.
-void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
-                                double dt, double dh, const srhd_ref_params* par,
+void srhd_ref_fluid_step_fluxes(const real* cons_in, real* cons_out, real* flux_out, int npg,
+                                real dt, real dh, const srhd_ref_params* par,
                                 srhd_ref_stats* stats, int nthreads);
-void srhd_ref_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+void srhd_ref_fluid_step(const real* cons_in, real* cons_out, int npg, real dt, real dh,
                          const srhd_ref_params* par, srhd_ref_stats* stats, int nthreads) {
   srhd_ref_fluid_step_fluxes(cons_in, cons_out, nullptr, npg, dt, dh, par, stats, nthreads);
 }
-void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
-                                double dt, double dh, const srhd_ref_params* par,
+void srhd_ref_fluid_step_fluxes(const real* cons_in, real* cons_out, real* flux_out, int npg,
+                                real dt, real dh, const srhd_ref_params* par,
                                 srhd_ref_stats* stats, int nthreads) {
   const int nxt = 16 + 2 * par->ghost;
   const size_t in_pg = (size_t)5 * nxt * nxt * nxt, out_pg = (size_t)8 * 5 * 512;
   unsigned long long f1 = 0, f2 = 0, f3 = 0, f4 = 0, f5 = 0;
-  double ms = 0.0;
+  double ms = 0.0;   // srhd_ref_stats.max_speed is a double in every variant
 #ifdef _OPENMP
   if (nthreads <= 0) nthreads = omp_get_max_threads();
 #else
@@ -896,15 +900,15 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
   for (int pg = 0; pg < npg; ++pg) {
     srhd_ref_stats st;
     std::memset(&st, 0, sizeof(st));
-    std::vector<double> box((size_t)5 * 4096);
-    std::vector<double> fl(flux_out ? (size_t)3 * in_pg : 0);
+    std::vector<real> box((size_t)5 * 4096);
+    std::vector<real> fl(flux_out ? (size_t)3 * in_pg : 0);
     (par->integrator == 1 ? step_box_vl : step_box)(cons_in + pg * in_pg, box.data(), 16, 16, 16, dt, dh, *par, st,
                                                     flux_out ? fl.data() : nullptr);
     if (flux_out) {
       const int g = par->ghost;
       const size_t np = (size_t)nxt * nxt * nxt;
       auto at = [&](int i, int j, int k) { return ((size_t)(k + g) * nxt + (j + g)) * nxt + (i + g); };
-      double* fo = flux_out + (size_t)pg * 8 * 6 * 5 * 64;
+      real* fo = flux_out + (size_t)pg * 8 * 6 * 5 * 64;
       for (int p = 0; p < 8; ++p) {
         const int i0 = 8 * (p & 1), j0 = 8 * ((p >> 1) & 1), k0 = 8 * (p >> 2);
         for (int f = 0; f < 6; ++f) {
@@ -921,7 +925,7 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
         }
       }
     }
-    double* out = cons_out + pg * out_pg;
+    real* out = cons_out + pg * out_pg;
     for (int q = 0; q < 5; ++q)
       for (int k = 0; k < 16; ++k)
         for (int j = 0; j < 16; ++j)
@@ -947,8 +951,8 @@ void srhd_ref_fluid_step_fluxes(const double* cons_in, double* cons_out, double*
   }
 }
 
-void srhd_ref_grid_pad(const double* grid, double* padded, int nx, int ny, int nz, int g,
-                       const int* bc, const unsigned char* inflow_mask, const double* inflow_cons) {
+void srhd_ref_grid_pad(const real* grid, real* padded, int nx, int ny, int nz, int g,
+                       const int* bc, const unsigned char* inflow_mask, const real* inflow_cons) {
   const int sx = nx + 2 * g, sy = ny + 2 * g, sz = nz + 2 * g;
   const size_t n = (size_t)nx * ny * nz, np = (size_t)sx * sy * sz;
   for (int k = -g; k < nz + g; ++k)
@@ -964,16 +968,16 @@ void srhd_ref_grid_pad(const double* grid, double* padded, int nx, int ny, int n
       }
 }
 
-void srhd_ref_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int g,
+void srhd_ref_grid_gather(const real* grid, real* cons_in, int nx, int ny, int nz, int g,
                           const int* bc, const unsigned char* inflow_mask,
-                          const double* inflow_cons) {
+                          const real* inflow_cons) {
   const int nxt = 16 + 2 * g;
   const int px = nx / 16, py = ny / 16, pz = nz / 16;
   const size_t n = (size_t)nx * ny * nz, t3 = (size_t)nxt * nxt * nxt;
 #pragma omp parallel for schedule(static)
   for (int pg = 0; pg < px * py * pz; ++pg) {
     const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
-    double* tile = cons_in + (size_t)pg * 5 * t3;
+    real* tile = cons_in + (size_t)pg * 5 * t3;
     for (int k = 0; k < nxt; ++k)
       for (int j = 0; j < nxt; ++j)
         for (int i = 0; i < nxt; ++i) {
@@ -989,13 +993,13 @@ void srhd_ref_grid_gather(const double* grid, double* cons_in, int nx, int ny, i
   }
 }
 
-void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz) {
+void srhd_ref_grid_scatter(const real* cons_out, real* grid, int nx, int ny, int nz) {
   const int px = nx / 16, py = ny / 16, pz = nz / 16;
   const size_t n = (size_t)nx * ny * nz;
 #pragma omp parallel for schedule(static)
   for (int pg = 0; pg < px * py * pz; ++pg) {
     const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
-    const double* src = cons_out + (size_t)pg * 8 * 5 * 512;
+    const real* src = cons_out + (size_t)pg * 8 * 5 * 512;
     for (int p = 0; p < 8; ++p)
       for (int q = 0; q < 5; ++q)
         for (int k = 0; k < 8; ++k)
@@ -1018,15 +1022,15 @@ void srhd_ref_grid_scatter(const double* cons_out, double* grid, int nx, int ny,
 // (all x-lo faces, then x-hi, y-lo, ... ): a cell on a patch edge is corrected through one face after the other.
 //   patches [np][5][8][8][8]; flux_coarse, flux_fine [nf][5][8][8] (in-face layout of flux_out); face_patch,
 //   face_id [nf] (0 x-lo, 1 x-hi, 2 y-lo, 3 y-hi, 4 z-lo, 5 z-hi).  Returns the number of skipped cells.
-unsigned long long srhd_ref_flux_correction(double* patches, const double* flux_coarse, const double* flux_fine,
-                                            const int* face_patch, const int* face_id, int nf, double dt, double dh) {
+unsigned long long srhd_ref_flux_correction(real* patches, const real* flux_coarse, const real* flux_fine,
+                                            const int* face_patch, const int* face_id, int nf, real dt, real dh) {
   unsigned long long skipped = 0;
-  const double dtdh = dt / dh;
+  const real dtdh = dt / dh;
   for (int cls = 0; cls < 6; ++cls)
     for (int f = 0; f < nf; ++f) {
       if (face_id[f] != cls) continue;
       const int d = cls >> 1, hi = cls & 1;
-      double* P = patches + (size_t)face_patch[f] * 5 * 512;
+      real* P = patches + (size_t)face_patch[f] * 5 * 512;
       for (int a = 0; a < 8; ++a)
         for (int bb = 0; bb < 8; ++bb) {
           int i, j, k;
@@ -1034,9 +1038,9 @@ unsigned long long srhd_ref_flux_correction(double* patches, const double* flux_
           else if (d == 1) { i = bb; j = hi ? 7 : 0; k = a; }
           else { i = bb; j = a; k = hi ? 7 : 0; }
           const size_t c = (size_t)k * 64 + j * 8 + i;
-          double Un[5];
+          real Un[5];
           for (int q = 0; q < 5; ++q) {
-            const double dF = flux_fine[((size_t)f * 5 + q) * 64 + a * 8 + bb] - flux_coarse[((size_t)f * 5 + q) * 64 + a * 8 + bb];
+            const real dF = flux_fine[((size_t)f * 5 + q) * 64 + a * 8 + bb] - flux_coarse[((size_t)f * 5 + q) * 64 + a * 8 + bb];
             Un[q] = hi ? P[q * 512 + c] - dtdh * dF : P[q * 512 + c] + dtdh * dF;
           }
           if (is_physical(Un)) { for (int q = 0; q < 5; ++q) P[q * 512 + c] = Un[q]; }
@@ -1052,7 +1056,7 @@ unsigned long long srhd_ref_flux_correction(double* patches, const double* flux_
 // the parent).  If any child fails Eq. 30, the same interpolation is done on the PRIMITIVE variables of the
 // seven cells and the children are converted back (always physical; "ghost zones do not affect conservation").
 //   coarse [5][nz][ny][nx];  fine [5][2(nz-2)][2(ny-2)][2(nx-2)];  fallback (may be null) [nz-2][ny-2][nx-2] bytes.
-unsigned long long srhd_ref_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine, double beta,
+unsigned long long srhd_ref_ghost_interp(const real* coarse, int nx, int ny, int nz, real* fine, real beta,
                                          const srhd_ref_params* par, unsigned char* fallback) {
   const size_t n = (size_t)nx * ny * nz;
   const int fx = 2 * (nx - 2), fy = 2 * (ny - 2), fz = 2 * (nz - 2);
@@ -1063,7 +1067,7 @@ unsigned long long srhd_ref_ghost_interp(const double* coarse, int nx, int ny, i
     for (int j = 1; j < ny - 1; ++j)
       for (int i = 1; i < nx - 1; ++i) {
         const size_t c = ((size_t)k * ny + j) * nx + i;
-        double Q[7][5];                                       // cell, x-, x+, y-, y+, z-, z+
+        real Q[7][5];                                       // cell, x-, x+, y-, y+, z-, z+
         for (int q = 0; q < 5; ++q) {
           Q[0][q] = coarse[q * n + c];
           for (int d = 0; d < 3; ++d) {
@@ -1071,23 +1075,23 @@ unsigned long long srhd_ref_ghost_interp(const double* coarse, int nx, int ny, i
             Q[2 + 2 * d][q] = coarse[q * n + c + stp[d]];
           }
         }
-        double child[8][5];
+        real child[8][5];
         bool ok = true, fell_back = false;
         for (int pass = 0; pass < 2; ++pass) {                // 0: conserved variables, 1: primitive variables
-          double V[7][5];
+          real V[7][5];
           for (int m = 0; m < 7; ++m) {
             if (pass == 0) for (int q = 0; q < 5; ++q) V[m][q] = Q[m][q];
             else cons2prim(Q[m], V[m], par->newton_rtol, par->newton_max_iter, nullptr, nullptr);
           }
-          double sl[3][5];
+          real sl[3][5];
           for (int d = 0; d < 3; ++d)
             for (int q = 0; q < 5; ++q)
-              sl[d][q] = 0.25 * limited_slope(V[0][q] - V[1 + 2 * d][q], V[2 + 2 * d][q] - V[0][q], beta);
+              sl[d][q] = real(0.25) * limited_slope(V[0][q] - V[1 + 2 * d][q], V[2 + 2 * d][q] - V[0][q], beta);
           ok = true;
           for (int ch = 0; ch < 8; ++ch) {
-            double v[5];
+            real v[5];
             for (int q = 0; q < 5; ++q) {
-              const double ax = (ch & 1) ? sl[0][q] : -sl[0][q], ay = (ch & 2) ? sl[1][q] : -sl[1][q],
+              const real ax = (ch & 1) ? sl[0][q] : -sl[0][q], ay = (ch & 2) ? sl[1][q] : -sl[1][q],
                            az = (ch & 4) ? sl[2][q] : -sl[2][q];
               v[q] = ((V[0][q] + ax) + ay) + az;
             }
@@ -1108,22 +1112,22 @@ unsigned long long srhd_ref_ghost_interp(const double* coarse, int nx, int ny, i
 
 // ---- refinement criteria (section 3.1; Eq. 33; reading S17: centred differences) --
 // quantity: 0 none, 1 D, 2 Etilde, 3 rho, 4 Lorentz factor.  flags[pg*8 + p], patch p as in S13.
-void srhd_ref_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
+void srhd_ref_refine_flags(const real* cons_in, int npg, int quantity, real c_q, real mom_over_d,
                            const srhd_ref_params* par, unsigned char* flags) {
   const int g = par->ghost, nxt = 16 + 2 * g;
   const size_t np = (size_t)nxt * nxt * nxt;
   for (int pg = 0; pg < npg; ++pg) {
-    const double* t = cons_in + (size_t)pg * 5 * np;
-    std::vector<double> Q(np, 0.0);
+    const real* t = cons_in + (size_t)pg * 5 * np;
+    std::vector<real> Q(np, real(0.0));
     if (quantity != 0)
       for (size_t c = 0; c < np; ++c) {
         if (quantity == 1) Q[c] = t[c];
         else if (quantity == 2) Q[c] = t[4 * np + c];
         else {
-          double U[5], W[5];
+          real U[5], W[5];
           for (int q = 0; q < 5; ++q) U[q] = t[q * np + c];
           cons2prim(U, W, par->newton_rtol, par->newton_max_iter, nullptr, nullptr);
-          Q[c] = (quantity == 3) ? W[0] : std::sqrt(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+          Q[c] = (quantity == 3) ? W[0] : std::sqrt(real(1.0) + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
         }
       }
     unsigned char* f = flags + (size_t)pg * 8;
@@ -1134,13 +1138,13 @@ void srhd_ref_refine_flags(const double* cons_in, int npg, int quantity, double 
           const size_t c = ((size_t)(k + g) * nxt + (j + g)) * nxt + (i + g);
           bool hit = false;
           if (quantity != 0) {
-            const double gx = std::fabs(Q[c + 1] - Q[c - 1]);
-            const double gy = std::fabs(Q[c + nxt] - Q[c - nxt]);
-            const double gz = std::fabs(Q[c + (size_t)nxt * nxt] - Q[c - (size_t)nxt * nxt]);
-            hit = ((gx + gy) + gz) / (2.0 * std::fabs(Q[c])) > c_q;              // Eq. 33
+            const real gx = std::fabs(Q[c + 1] - Q[c - 1]);
+            const real gy = std::fabs(Q[c + nxt] - Q[c - nxt]);
+            const real gz = std::fabs(Q[c + (size_t)nxt * nxt] - Q[c - (size_t)nxt * nxt]);
+            hit = ((gx + gy) + gz) / (real(2.0) * std::fabs(Q[c])) > c_q;              // Eq. 33
           }
-          if (mom_over_d > 0.0) {
-            const double mx = t[np + c], my = t[2 * np + c], mz = t[3 * np + c];
+          if (mom_over_d > real(0.0)) {
+            const real mx = t[np + c], my = t[2 * np + c], mz = t[3 * np + c];
             hit = hit || (std::sqrt((mx * mx + my * my) + mz * mz) / t[c] > mom_over_d);
           }
           if (hit) f[(i >> 3) + 2 * (j >> 3) + 4 * (k >> 3)] = 1;

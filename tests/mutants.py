@@ -15,32 +15,32 @@ import tempfile
 from concurrent.futures import ThreadPoolExecutor
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_vl.py"]
+PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_vl.py", "tests/test_oracle_variants.py"]
 
 # (name, cited passage, old text, new text, pytest node ids / -k expression that must fail)
 MUTANTS = [
     ("umax: gamma_s dropped", "P:241 Eq. 26",
-     "return gs * (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + 3.0 * gamma * Us;",
-     "return (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + 3.0 * gamma * Us;",
+     "return gs * (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + real(3.0) * gamma * Us;",
+     "return (std::fabs(W[1]) + std::fabs(W[2]) + std::fabs(W[3])) + real(3.0) * gamma * Us;",
      "test_umax"),
     ("umax: gamma dropped from 3 gamma U_s", "P:241 Eq. 26",
-     "+ 3.0 * gamma * Us;", "+ 3.0 * Us;", "test_umax"),
+     "+ real(3.0) * gamma * Us;", "+ real(3.0) * Us;", "test_umax"),
     ("wave speeds: U_s^2 dropped from the denominator", "reading S6",
      "s.lam_p = (gamma * Un + Us * Q) / (g2 + Us2);\n  s.lam_m = (gamma * Un - Us * Q) / (g2 + Us2);",
      "s.lam_p = (gamma * Un + Us * Q) / (g2);\n  s.lam_m = (gamma * Un - Us * Q) / (g2);",
      "test_wave_speed_values or test_riemann_flux_values or test_hlle_satisfies"),
     ("wave-speed differences: U_t^2 dropped from lambda - v_n", "reading S6",
-     "const double d_with = Us * a / (gamma * w);", "const double d_with = Us / (gamma * w);",
+     "const real d_with = Us * a / (gamma * w);", "const real d_with = Us / (gamma * w);",
      "test_wave_speed_differences or test_riemann_flux"),
     ("wave-speed differences: 1 - lambda with a single factor a", "reading S6",
-     "const double c_with = a * a / ((gamma + u) * (Q + Us) * w);", "const double c_with = a / ((gamma + u) * (Q + Us) * w);",
+     "const real c_with = a * a / ((gamma + u) * (Q + Us) * w);", "const real c_with = a / ((gamma + u) * (Q + Us) * w);",
      "test_wave_speed_differences or test_riemann_flux_at_lorentz"),
     ("HLL: S_R - v_R without the other side's wave", "reading S6",
-     "h.AR = R.dp + ((h.SR > 0.5) ? (R.cp - cpS) : (h.SR - R.lam_p));", "h.AR = R.dp;",
+     "h.AR = R.dp + ((h.SR > real(0.5)) ? (R.cp - cpS) : (h.SR - R.lam_p));", "h.AR = R.dp;",
      "test_riemann_flux_values or test_hlle_satisfies"),
     ("HLLE: the right state's term halved", "P:225 (Mignone & Bodo 2005)",
      "    F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
-     "    F[c] = (SR * BL * L.U[c] + 0.5 * SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
+     "    F[c] = (SR * BL * L.U[c] + real(0.5) * SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
      "test_hlle_satisfies or test_riemann_flux_values"),
     ("HLLE: wave speeds swapped on the pressure terms", "P:225 (Mignone & Bodo 2005)",
      "    F[c] = (SR * BL * L.U[c] + SL * AR * R.U[c] + SR * L.pt[c] - SL * R.pt[c]) / den;",
@@ -61,23 +61,35 @@ MUTANTS = [
      "Um[(d * 5 + q) * np + c] = Ucm[d][q] - hdt * dF[d][q];\n              Up[(d * 5 + q) * np + c] = Ucp[d][q] - hdt * dF[d][q];",
      "test_one_step_matches_40_digit or test_retry_ladder_equals"),
     ("retry ladder: factor 0.75 -> 0.5", "P:273",
-     "beta = (pass <= K) ? beta * 0.75 : 0.0;", "beta = (pass <= K) ? beta * 0.5 : 0.0;",
+     "beta = (pass <= K) ? beta * real(0.75) : real(0.0);", "beta = (pass <= K) ? beta * real(0.5) : real(0.0);",
      "test_retry_ladder_equals"),
     ("retry ladder: failing face states ignored", "reading S15",
-     "if ((face_fail == 0 && cell_fail == 0) || beta == 0.0) break;",
-     "if ((cell_fail == 0) || beta == 0.0) break;",
+     "if ((face_fail == 0 && cell_fail == 0) || beta == real(0.0)) break;",
+     "if ((cell_fail == 0) || beta == real(0.0)) break;",
      "test_retry_ladder_equals"),
     ("VL: predictor advanced by a full step", "P:225, reading S18",
-     "Uh[q] = cons_in[q * np + c] - hdt * ((dfx + dfy) + dfz);", "Uh[q] = cons_in[q * np + c] - 2.0 * hdt * ((dfx + dfy) + dfz);",
+     "Uh[q] = cons_in[q * np + c] - hdt * ((dfx + dfy) + dfz);", "Uh[q] = cons_in[q * np + c] - real(2.0) * hdt * ((dfx + dfy) + dfz);",
      "test_vl_second_order or test_vl_equals"),
     ("VL: corrector reconstructs the OLD primitives (predictor ignored)", "P:225, reading S18",
-     "a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0 : Wh[q * np + c + (ptrdiff_t)m * stp[d]];",
-     "a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? 0.0 : Wc[q * np + c + (ptrdiff_t)m * stp[d]];",
+     "a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? real(0.0) : Wh[q * np + c + (ptrdiff_t)m * stp[d]];",
+     "a[m + 2] = (par.recon == 0 && (m == -2 || m == 2)) ? real(0.0) : Wc[q * np + c + (ptrdiff_t)m * stp[d]];",
      "test_vl_second_order"),
     ("update: flux difference with the wrong sign in z", "Eq. 4a, reading S12",
      "Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) + dfz);",
      "Un[q] = cons_in[q * np + c] - dtdh * ((dfx + dfy) - dfz);",
      "test_one_step_matches_40_digit"),
+    ("polytropic EoS: Gamma dropped from the sound speed", "P:107 Eq. 11, reading S19",
+     "return (kGnum * T) / (kGden * h);", "return T / h;",
+     "test_gamma_law_eos_is_eq11 or test_gamma_law_sound_wave"),
+    ("polytropic EoS: Gamma/(Gamma-1) inverted", "P:107 Eq. 11",
+     "constexpr real kG1 = kGnum / (kGnum - kGden);", "constexpr real kG1 = (kGnum - kGden) / kGnum;",
+     "test_gamma_law"),
+    ("original scheme: the rest mass not subtracted in L", "P:198, P:626",
+     "real L = std::fma(x, x, -musq) - real(1.0);", "real L = std::fma(x, x, -musq);",
+     "test_fig16 or test_original"),
+    ("original scheme: HLLC contact speed with D added to E", "reading S7, P:289",
+     "const real Eh = Uh[4];  ", "const real Eh = Uh[4] + Uh[0];",
+     "test_original_and_new"),
 ]
 
 

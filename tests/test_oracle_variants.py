@@ -282,3 +282,63 @@ def test_original_and_new_scheme_are_the_same_method_in_exact_arithmetic(ref):
         assert np.array_equal(out, cu)
     assert np.abs(orig[:4] - new[:4]).max() <= 1e-13 * np.abs(new[:4]).max()
     assert np.abs(orig[4] - (new[4] + new[0])).max() <= 1e-13 * np.abs(orig[4]).max()
+
+
+# ------------------------------------------------------------------ single precision (eps_machine = 1e-7)
+EPS32 = float(np.finfo(np.float32).eps)
+
+
+def test_f32_conversions_follow_eq20_with_single_precision_epsilon(ref):
+    """The single-precision variant against the double-precision oracle: both are the same algorithm, so they may
+    differ by the paper's error model with eps_machine = FLT_EPSILON (Eq. 20), and no more."""
+    W = workloads.conversion_states(n=4000, log_rho=(-3, 3), log_theta=(-6, 3), log_gamma=(0, 1.5))
+    U64 = ref.prim2cons(W)
+    _, ht64, _, bad64 = ref.cons2prim(U64, diag=True)
+    cs2 = ref.cs2_of_T(W[4] / W[0])
+    cond = (1 + (W[1:4] ** 2).sum(0) * (1 - cs2) / cs2) * EPS32
+    with ref.variant("f32"):
+        par = ref.params(newton_rtol=1e-6)
+        U32 = ref.prim2cons(W)
+        assert U32.dtype == np.float32
+        W32, ht32, it, bad32 = ref.cons2prim(U32, par, diag=True)
+    assert (np.abs(U32 / U64 - 1)[:, np.isfinite(U64).all(0)] <= 8 * EPS32).all()       # prim -> cons has no cancellation
+    ok = (cond < 1e-2) & (bad32 == 0)
+    assert ok.sum() > 1500
+    assert (np.abs(1 - ht32[ok] / ht64[ok]) <= 16 * cond[ok]).all()
+    assert (np.abs(W32[0] / W[0] - 1)[ok] <= 64 * cond[ok]).all()
+    assert it.max() <= 8
+    # Eq. 30 with the single-precision eps_machine (P:269): L between the two epsilons passes in double only
+    L = 3e-9
+    x = L / 2                                          # at rest: L = x^2 + 2x
+    U = np.array([[1.0], [0.0], [0.0], [0.0], [x]])
+    assert ref.cons2prim(U, diag=True)[3][0] == 0
+    with ref.variant("f32"):
+        assert ref.cons2prim(U, diag=True)[3][0] == 1
+
+
+def test_f32_step_tracks_the_double_precision_step(ref):
+    rng = np.random.default_rng(4)
+    x = (np.arange(32) + 0.5) / 32
+    prim = np.empty((5, 16, 16, 32))
+    prim[0] = 1 + 0.3 * np.sin(2 * np.pi * x)[None, None, :]
+    prim[1] = 0.8 * np.cos(2 * np.pi * x)[None, None, :]
+    prim[2], prim[3] = 0.3, -0.2 + 0.05 * rng.standard_normal((16, 16, 1))
+    prim[4] = 0.5 * prim[0] ** (4 / 3)
+    par64 = ref.params("plm", "hllc")
+    c64 = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    dt = ref.cfl_dt(c64, 0.4, 1 / 32, par64)
+    n64, _ = ref.grid_step_tiled(c64, dt, 1 / 32, par64, ["periodic"] * 6)
+    with ref.variant("f32"):
+        par = ref.params("plm", "hllc", newton_rtol=1e-6)
+        c32 = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+        whole, st, _ = ref.grid_step_whole(c32, dt, 1 / 32, par, ["periodic"] * 6)
+        tiled, _ = ref.grid_step_tiled(c32, dt, 1 / 32, par, ["periodic"] * 6)
+        assert tiled.dtype == np.float32 and np.array_equal(whole, tiled) and st.n_retry_pg == 0
+        for q in range(5):                              # conservation to single-precision round-off
+            assert abs(float(tiled[q].astype(np.float64).sum() - c32[q].astype(np.float64).sum())) <= \
+                64 * EPS32 * float(np.abs(c32[q]).sum()) / np.sqrt(c32[q].size)
+        Wu = np.array([0.7, 3.0, -1.0, 0.5, 1e-3])
+        cu = ref.prim2cons(np.repeat(Wu[:, None], 16 ** 3, 1)).reshape(5, 16, 16, 16)
+        assert np.array_equal(ref.grid_step_whole(cu, 1e-3, 1e-2, par, ["periodic"] * 6)[0], cu)
+    scale = np.abs(n64).reshape(5, -1).max(1)[:, None, None, None]
+    assert (np.abs(tiled - n64) / scale).max() <= 64 * EPS32
