@@ -28,6 +28,16 @@
 
 #include <stddef.h>
 
+/* Every state array (and the max-speed scalar) is an array of srhd_real: double, or float in the library built
+ * with -DSRHD_F32 (libsrhd_b200_f32*.so: the precision of every performance number in the paper; Eq. 30
+ * then uses eps_machine = FLT_EPSILON).  Scalar arguments (dt, dh, cfl, thresholds), srhd_params and
+ * srhd_stats have the same types in every build. */
+#ifdef SRHD_F32
+typedef float srhd_real;
+#else
+typedef double srhd_real;
+#endif
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -63,7 +73,7 @@ typedef struct {
   int    riemann;          /* SRHD_RIEMANN_HLLE or SRHD_RIEMANN_HLLC                          */
   double minmod_coeff;     /* beta0 in [1,2], "original minmod coefficient"; default 1.5 (S3) */
   int    max_retry;        /* K reductions of beta by 0.75, then beta = 0; default 8 (S9)     */
-  double newton_rtol;      /* Newton-Raphson stop: |delta| <= rtol*|htilde|; default 1e-15 (S2)       */
+  double newton_rtol;      /* Newton-Raphson stop: |delta| <= rtol*|htilde|; default 1e-15, 1e-6 in the f32 build (S2) */
   int    newton_max_iter;  /* iteration cap; default 20 (S2)                                          */
   int    ghost;            /* ghost width of cons_in: MUSCL-Hancock 2 (PLM) / 3 (PPM); VL one more    */
   int    integrator;       /* SRHD_INTEGRATOR_MHM (default) or SRHD_INTEGRATOR_VL             */
@@ -97,20 +107,20 @@ void srhd_default_params(srhd_params* p, int recon, int riemann);
 
 /* prim -> cons for n independent states (Fig. 15 right; Eq. 5a-b; Eq. 22-23).
  * prim, cons: device, SoA with `stride`; the two arrays must not overlap. */
-int srhd_prim2cons(const double* prim, double* cons, size_t n, size_t stride, void* stream);
+int srhd_prim2cons(const srhd_real* prim, srhd_real* cons, size_t n, size_t stride, void* stream);
 
 /* cons -> prim for n independent states (Fig. 15 left; Eq. 15-18; App. A):
  * Newton-Raphson on htilde = h - 1 from the two-branch guess A4/A6, canonical left-hand side
  * L = fma(x, x+2, -mu^2).  A state that fails Eq. 30 is counted in
  * stats->n_c2p_fail and evaluated with L <- eps_machine (S10).  stats may be NULL. */
-int srhd_cons2prim(const double* cons, double* prim, size_t n, size_t stride,
+int srhd_cons2prim(const srhd_real* cons, srhd_real* prim, size_t n, size_t stride,
                    const srhd_params* params, srhd_stats* stats, void* stream);
 
 /* CFL signal speed (Eq. 24-28; G1): *d_max_speed = S_max(max_i U_max,i) with
  * U_max = gamma_s (|U^x|+|U^y|+|U^z|) + 3 gamma U_s from cons2prim of each state.  The time step is
  * dt = C_CFL * dh / *d_max_speed (Eq. 28), formed by the caller.  n == 0 gives 0. */
-int srhd_max_signal_speed(const double* cons, size_t n, size_t stride,
-                          const srhd_params* params, double* d_max_speed, void* stream);
+int srhd_max_signal_speed(const srhd_real* cons, size_t n, size_t stride,
+                          const srhd_params* params, srhd_real* d_max_speed, void* stream);
 
 /* One MUSCL-Hancock step (readings S3-S7, S9-S15) of npg patch groups.
  *   cons_in : [npg][5][nxt][nxt][nxt] doubles, nxt = 16 + 2*ghost, x fastest: the 16^3 interior
@@ -124,7 +134,7 @@ int srhd_max_signal_speed(const double* cons, size_t n, size_t stride,
  * -> Eq. 30 check; if any interior cell or face state of the group fails, the whole group is redone
  * with beta <- 0.75 beta, after max_retry reductions with beta = 0, whose result is accepted.
  * cons_in and cons_out must not overlap.  stats may be NULL. */
-int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+int srhd_fluid_step(const srhd_real* cons_in, srhd_real* cons_out, int npg, double dt, double dh,
                     const srhd_params* params, srhd_stats* stats, void* stream);
 
 /* The same step, additionally returning the fluxes through the six boundary faces of every 8^3 patch
@@ -136,7 +146,7 @@ int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt,
  *             Values are the HLLE/HLLC fluxes of the ACCEPTED pass, positive along +axis; the face shared
  *             by two patches of the group is written to both.  NULL = srhd_fluid_step.
  * Must not overlap cons_in / cons_out.  Same errors and asynchrony as srhd_fluid_step. */
-int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+int srhd_fluid_step_fluxes(const srhd_real* cons_in, srhd_real* cons_out, srhd_real* flux_out, int npg,
                            double dt, double dh, const srhd_params* params, srhd_stats* stats,
                            void* stream);
 
@@ -146,8 +156,8 @@ int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux
  * synchronisation.  d_max_speed: device, one double, read by every CTA at kernel start; min_speed >= 0
  * bounds the speed from below (e.g. the signal speed of a fixed-inflow state that is not in the
  * grid yet); the caller guarantees max(*d_max_speed, min_speed) > 0.  flux_out may be NULL. */
-int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_out, int npg, double cfl,
-                        double dh, const double* d_max_speed, double min_speed,
+int srhd_fluid_step_cfl(const srhd_real* cons_in, srhd_real* cons_out, srhd_real* flux_out, int npg, double cfl,
+                        double dh, const srhd_real* d_max_speed, double min_speed,
                         const srhd_params* params, srhd_stats* stats, void* stream);
 
 /* Refinement criteria of the SRHD module (section 3.1; Eq. 33), one flag per 8^3 patch,
@@ -158,7 +168,7 @@ int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_ou
  *     or  |M| / D > mom_over_d
  *                                                                 -- skipped if mom_over_d == 0
  *   else 0.  flags: device, npg*8 bytes.  Thresholds per level are the caller's business. */
-int srhd_refine_flags(const double* cons_in, int npg, int quantity, double c_q, double mom_over_d,
+int srhd_refine_flags(const srhd_real* cons_in, int npg, int quantity, double c_q, double mom_over_d,
                       const srhd_params* params, unsigned char* flags, void* stream);
 
 /* Flux correction at coarse-fine interfaces with the paper's guard (section 3.3(4)): the coarse cells
@@ -173,7 +183,7 @@ int srhd_refine_flags(const double* cons_in, int npg, int quantity, double c_q, 
  *   d_n_skipped : device, one unsigned long long (zeroed by the call): cells whose correction was ignored
  * Faces are processed class by class (x-lo, x-hi, y-lo, ...), so a cell on a patch edge is corrected through
  * one face after the other, in that order; within a class a (patch, face) pair may appear once. */
-int srhd_flux_correction(double* patches, const double* flux_coarse, const double* flux_fine,
+int srhd_flux_correction(srhd_real* patches, const srhd_real* flux_coarse, const srhd_real* flux_fine,
                          const int* face_patch, const int* face_id, int nf, double dt, double dh,
                          unsigned long long* d_n_skipped, void* stream);
 
@@ -185,7 +195,7 @@ int srhd_flux_correction(double* patches, const double* flux_coarse, const doubl
  *   coarse: device, [5][nz][ny][nx];  fine: device, [5][2(nz-2)][2(ny-2)][2(nx-2)]
  *   fallback: device, (nz-2)(ny-2)(nx-2) bytes, 1 where the fallback was used (may be NULL)
  *   d_n_fallback: device, one unsigned long long (zeroed by the call) */
-int srhd_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine, double minmod_coeff,
+int srhd_ghost_interp(const srhd_real* coarse, int nx, int ny, int nz, srhd_real* fine, double minmod_coeff,
                       const srhd_params* params, unsigned char* fallback, unsigned long long* d_n_fallback,
                       void* stream);
 
@@ -201,16 +211,16 @@ size_t srhd_workspace_bytes(int npg, const srhd_params* params);
  * or SRHD_BC_OUTFLOW (copy the nearest interior cell).  inflow_mask (device, [ny][nx] bytes, may be
  * NULL): ghost cells below z = 0 whose column is marked hold inflow_cons[5] (HOST pointer) instead.
  * Patch group pg = gx + (nx/16)*(gy + (ny/16)*gz). */
-int srhd_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int ghost,
+int srhd_grid_gather(const srhd_real* grid, srhd_real* cons_in, int nx, int ny, int nz, int ghost,
                      const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
                      void* stream);
-int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz, void* stream);
+int srhd_grid_scatter(const srhd_real* cons_out, srhd_real* grid, int nx, int ny, int nz, void* stream);
 
 /* srhd_grid_scatter fused with srhd_max_signal_speed of the state it writes: *d_max_speed (device)
  * receives S_max (Eq. 26-27) of the scattered grid, ready for the next step's dt (Eq. 28).  The copy is
  * memory bound and the conversion ALU bound, so the fused kernel costs about as much as the slower one. */
-int srhd_grid_scatter_speed(const double* cons_out, double* grid, int nx, int ny, int nz,
-                            const srhd_params* params, double* d_max_speed, void* stream);
+int srhd_grid_scatter_speed(const srhd_real* cons_out, srhd_real* grid, int nx, int ny, int nz,
+                            const srhd_params* params, srhd_real* d_max_speed, void* stream);
 
 /* Ghost-zone fill straight from the PATCH layout srhd_fluid_step wrote (cons_out of the previous
  * step of the same uniform grid: patch group pg = gx + (nx/16)*(gy + (ny/16)*gz)), fused with
@@ -218,9 +228,9 @@ int srhd_grid_scatter_speed(const double* cons_out, double* grid, int nx, int ny
  * from the scattered grid, bit for bit) and *d_max_speed = S_max.  With it a uniform-grid step is two
  * kernels (this one and srhd_fluid_step_cfl) and the grid is only materialised on demand.  The ghost
  * width is params->ghost.  Boundary arguments as srhd_grid_gather. */
-int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int ny, int nz, const int* bc,
+int srhd_patch_gather_speed(const srhd_real* patches, srhd_real* cons_in, int nx, int ny, int nz, const int* bc,
                             const unsigned char* inflow_mask, const double* inflow_cons,
-                            const srhd_params* params, double* d_max_speed, void* stream);
+                            const srhd_params* params, srhd_real* d_max_speed, void* stream);
 
 /* One whole step of a uniform grid kept in the patch layout: srhd_patch_gather_speed + srhd_fluid_step_cfl behind
  * one call, with the uniform-tile test done on the way (same results, bit for bit, as the two calls).
@@ -235,10 +245,10 @@ int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int 
  * finished by the first kernel: its new patches are its old ones (srhd_stats.n_uniform_pg counts them), so its
  * state crosses HBM once in and once out and no tile is materialised for it; every other group goes through
  * fluid_step_kernel as in srhd_fluid_step_cfl.  Boundary arguments as srhd_grid_gather; errors as the two calls. */
-int srhd_grid_step_cfl(const double* patches_in, double* patches_out, double* cons_in, double* flux_out,
+int srhd_grid_step_cfl(const srhd_real* patches_in, srhd_real* patches_out, srhd_real* cons_in, srhd_real* flux_out,
                        int nx, int ny, int nz, const int* bc, const unsigned char* inflow_mask,
                        const double* inflow_cons, double cfl, double dh, double min_speed,
-                       const srhd_params* params, srhd_stats* stats, double* d_max_speed, void* stream);
+                       const srhd_params* params, srhd_stats* stats, srhd_real* d_max_speed, void* stream);
 
 /* Measurement helper (not part of the solver): launches a register-only DFMA loop that fills every
  * fp64 lane of the GPU (148 x 8 CTAs x 256 threads, 32*iters dependent-chain DFMA per thread in 8
@@ -271,8 +281,8 @@ const char* srhd_error_string(int code);
 int srhd_build_is_exact(void);
 
 /* Which compile-time variant this library is (one library per variant, like the EoS
- * choice of the paper's code): "eos=taub-mathews|gamma-5/3|gamma-4/3 energy=reduced|total arithmetic=production|
- * generic|exact".  eos: Eq. 10 or the polytropic P:107 Eq. 11; energy=total is the paper's "original scheme"
+ * choice of the paper's code): "eos=taub-mathews|gamma-5/3|gamma-4/3 energy=reduced|total precision=f64|f32
+ * arithmetic=production|generic|exact".  eos: Eq. 10 or the polytropic P:107 Eq. 11; energy=total is the paper's "original scheme"
  * (the fifth conserved variable is E, evolved by the flux M) kept for its A/B runs; arithmetic=generic means
  * the paper's formulas as written with IEEE division and square root, exact the same without FMA contraction. */
 const char* srhd_build_variant(void);

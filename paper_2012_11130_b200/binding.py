@@ -49,6 +49,7 @@ SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_
            "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact", "srhd_build_variant"]
 
 _LIBS = {}
+_CUR_REAL = torch.float64   # srhd_real of the library selected by the latest load_library() call
 
 
 class SrhdError(RuntimeError):
@@ -58,7 +59,9 @@ class SrhdError(RuntimeError):
 def load_library(exact=False):
     """dlopen libsrhd_b200[_exact].so (built in-tree by paper_2012_11130_b200.build); `exact` may also name one of
     the variant libraries of build.VARIANTS ("gamma53", "gamma53_exact", "gamma43_exact", "orig_exact")."""
+    global _CUR_REAL
     if exact in _LIBS:
+        _CUR_REAL = _LIBS[exact]._real_dtype
         return _LIBS[exact]
     path = _build.lib_path(exact)
     if not os.path.exists(path):
@@ -113,6 +116,8 @@ def load_library(exact=False):
     L.srhd_build_is_exact.argtypes = []
     L.srhd_build_variant.restype = C.c_char_p
     L.srhd_build_variant.argtypes = []
+    L._real_dtype = torch.float32 if b"precision=f32" in L.srhd_build_variant() else torch.float64
+    _CUR_REAL = L._real_dtype
     _LIBS[exact] = L
     return L
 
@@ -144,8 +149,10 @@ def _check(code, L):
 
 
 def _dev(t, name):
-    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
-        raise SrhdError(f"{name} must be a contiguous float64 CUDA tensor (no CPU fallback)")
+    """A state array handed to the library most recently selected by load_library(): contiguous, on the GPU, of
+    that library's srhd_real (float64; float32 for the f32 builds)."""
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == _CUR_REAL and t.is_contiguous()):
+        raise SrhdError(f"{name} must be a contiguous {_CUR_REAL} CUDA tensor (no CPU fallback)")
     return t
 
 
@@ -193,7 +200,7 @@ def max_signal_speed(cons, par=None, out=None, exact=False):
     cons = _dev(cons, "cons")
     par = par or params(exact=exact)
     n = cons.shape[1]
-    out = torch.empty(1, dtype=torch.float64, device=cons.device) if out is None else out
+    out = torch.empty(1, dtype=cons.dtype, device=cons.device) if out is None else out
     _check(L.srhd_max_signal_speed(cons.data_ptr(), n, cons.stride(0) if n else 0, C.byref(par),
                                    out.data_ptr(), _stream()), L)
     return out
@@ -208,7 +215,7 @@ def fluid_step(cons_in, dt, dh, par, cons_out=None, stats=None, exact=False):
     if tuple(cons_in.shape) != (npg, 5, nxt, nxt, nxt):
         raise SrhdError(f"cons_in must have shape (npg,5,{nxt},{nxt},{nxt})")
     if cons_out is None:
-        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=torch.float64, device=cons_in.device)
+        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     stats = new_stats(cons_in.device) if stats is None else stats
     _check(L.srhd_fluid_step(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(), npg, float(dt),
                              float(dh), C.byref(par), stats.data_ptr(), _stream()), L)
@@ -221,9 +228,9 @@ def fluid_step_fluxes(cons_in, dt, dh, par, cons_out=None, flux_out=None, stats=
     cons_in = _dev(cons_in, "cons_in")
     npg = cons_in.shape[0]
     if cons_out is None:
-        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=torch.float64, device=cons_in.device)
+        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     if flux_out is None:
-        flux_out = torch.empty((npg, 8, 6, 5, 8, 8), dtype=torch.float64, device=cons_in.device)
+        flux_out = torch.empty((npg, 8, 6, 5, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     stats = new_stats(cons_in.device) if stats is None else stats
     _check(L.srhd_fluid_step_fluxes(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(),
                                     _dev(flux_out, "flux_out").data_ptr(), npg, float(dt), float(dh),
@@ -238,7 +245,7 @@ def fluid_step_cfl(cons_in, cfl, dh, max_speed, par, min_speed=0.0, cons_out=Non
     cons_in = _dev(cons_in, "cons_in")
     npg = cons_in.shape[0]
     if cons_out is None:
-        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=torch.float64, device=cons_in.device)
+        cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     stats = new_stats(cons_in.device) if stats is None else stats
     _check(L.srhd_fluid_step_cfl(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(),
                                  0 if flux_out is None else _dev(flux_out, "flux_out").data_ptr(), npg,
@@ -287,7 +294,7 @@ def ghost_interp(coarse, minmod_coeff, par=None, exact=False):
     coarse = _dev(coarse, "coarse")
     par = par or params(exact=exact)
     _, nz, ny, nx = coarse.shape
-    fine = torch.empty((5, 2 * (nz - 2), 2 * (ny - 2), 2 * (nx - 2)), dtype=torch.float64, device=coarse.device)
+    fine = torch.empty((5, 2 * (nz - 2), 2 * (ny - 2), 2 * (nx - 2)), dtype=coarse.dtype, device=coarse.device)
     fb = torch.zeros((nz - 2, ny - 2, nx - 2), dtype=torch.uint8, device=coarse.device)
     cnt = torch.zeros(1, dtype=torch.int64, device=coarse.device)
     _check(L.srhd_ghost_interp(coarse.data_ptr(), nx, ny, nz, fine.data_ptr(), float(minmod_coeff), C.byref(par),
@@ -308,7 +315,7 @@ def grid_gather(grid, ghost, bc, inflow=None, cons_in=None, exact=False):
     npg = (nx // 16) * (ny // 16) * (nz // 16)
     nxt = 16 + 2 * ghost
     if cons_in is None:
-        cons_in = torch.empty((npg, 5, nxt, nxt, nxt), dtype=torch.float64, device=grid.device)
+        cons_in = torch.empty((npg, 5, nxt, nxt, nxt), dtype=grid.dtype, device=grid.device)
     mask_ptr, icons = None, None
     if inflow is not None:
         mask, vals = inflow
@@ -327,7 +334,7 @@ def grid_scatter(cons_out, shape, grid=None, exact=False):
     cons_out = _dev(cons_out, "cons_out")
     nz, ny, nx = shape
     if grid is None:
-        grid = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=cons_out.device)
+        grid = torch.empty((5, nz, ny, nx), dtype=cons_out.dtype, device=cons_out.device)
     _check(L.srhd_grid_scatter(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, _stream()), L)
     return grid
 
@@ -338,8 +345,8 @@ def grid_scatter_speed(cons_out, shape, par, grid=None, out=None, exact=False):
     cons_out = _dev(cons_out, "cons_out")
     nz, ny, nx = shape
     if grid is None:
-        grid = torch.empty((5, nz, ny, nx), dtype=torch.float64, device=cons_out.device)
-    out = torch.empty(1, dtype=torch.float64, device=cons_out.device) if out is None else out
+        grid = torch.empty((5, nz, ny, nx), dtype=cons_out.dtype, device=cons_out.device)
+    out = torch.empty(1, dtype=cons_out.dtype, device=cons_out.device) if out is None else out
     _check(L.srhd_grid_scatter_speed(cons_out.data_ptr(), grid.data_ptr(), nx, ny, nz, C.byref(par),
                                      out.data_ptr(), _stream()), L)
     return grid, out
@@ -352,8 +359,8 @@ def patch_gather_speed(patches, shape, par, bc, inflow=None, cons_in=None, out=N
     nz, ny, nx = shape
     nxt = 16 + 2 * par.ghost
     if cons_in is None:
-        cons_in = torch.empty((patches.shape[0], 5, nxt, nxt, nxt), dtype=torch.float64, device=patches.device)
-    out = torch.empty(1, dtype=torch.float64, device=patches.device) if out is None else out
+        cons_in = torch.empty((patches.shape[0], 5, nxt, nxt, nxt), dtype=patches.dtype, device=patches.device)
+    out = torch.empty(1, dtype=patches.dtype, device=patches.device) if out is None else out
     mask_ptr, icons = None, None
     if inflow is not None:
         mask, vals = inflow
@@ -379,7 +386,7 @@ def grid_step_cfl(patches_in, patches_out, cons_in, shape, cfl, dh, par, bc, inf
         raise SrhdError(f"cons_in must have shape ({npg}, 5, {nxt}, {nxt}, {nxt})")
     if flux_out is not None and tuple(_dev(flux_out, "flux_out").shape) != (npg, 8, 6, 5, 8, 8):
         raise SrhdError(f"flux_out must have shape ({npg}, 8, 6, 5, 8, 8)")
-    out = torch.empty(1, dtype=torch.float64, device=patches_in.device) if out is None else out
+    out = torch.empty(1, dtype=patches_in.dtype, device=patches_in.device) if out is None else out
     stats = new_stats(patches_in.device) if stats is None else stats
     mask_ptr, icons = None, None
     if inflow is not None:

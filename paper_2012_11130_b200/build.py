@@ -29,12 +29,15 @@ VARIANTS = {
     "libsrhd_b200_gamma53_exact.so": _EXACT + _G53,
     "libsrhd_b200_gamma43_exact.so": _EXACT + _G43,
     "libsrhd_b200_orig_exact.so": _EXACT + ["-DSRHD_SCHEME=1"],
+    # single precision throughout (srhd_real = float): the precision of every performance number in the paper
+    "libsrhd_b200_f32.so": ["-DSRHD_F32"],
+    "libsrhd_b200_f32_exact.so": _EXACT + ["-DSRHD_F32"],
 }
 
 
 def lib_path(exact=False):
     """False: the production library; True: the exact build; a string: that variant ("gamma53", "gamma53_exact",
-    "gamma43_exact", "orig_exact")."""
+    "gamma43_exact", "orig_exact", "f32", "f32_exact")."""
     if isinstance(exact, str):
         name = f"libsrhd_b200_{exact}.so"
         if name not in VARIANTS:

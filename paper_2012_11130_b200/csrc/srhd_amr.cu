@@ -9,11 +9,11 @@
 
 namespace srhd {
 
-__global__ void __launch_bounds__(64) flux_correction_kernel(double* __restrict__ patches,
-                                                             const double* __restrict__ flux_coarse,
-                                                             const double* __restrict__ flux_fine,
+__global__ void __launch_bounds__(64) flux_correction_kernel(real* __restrict__ patches,
+                                                             const real* __restrict__ flux_coarse,
+                                                             const real* __restrict__ flux_fine,
                                                              const int* __restrict__ face_patch,
-                                                             const int* __restrict__ face_id, int cls, double dtdh,
+                                                             const int* __restrict__ face_id, int cls, real dtdh,
                                                              unsigned long long* __restrict__ n_skipped) {
   const int f = blockIdx.x;
   if (face_id[f] != cls) return;                             // faces are processed class by class (see the ABI)
@@ -23,12 +23,12 @@ __global__ void __launch_bounds__(64) flux_correction_kernel(double* __restrict_
   if (d == 0) { i = hi ? 7 : 0; j = bb; k = a; }
   else if (d == 1) { i = bb; j = hi ? 7 : 0; k = a; }
   else { i = bb; j = a; k = hi ? 7 : 0; }
-  double* P = patches + (size_t)face_patch[f] * 5 * 512 + k * 64 + j * 8 + i;
-  double Un[5];
+  real* P = patches + (size_t)face_patch[f] * 5 * 512 + k * 64 + j * 8 + i;
+  real Un[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
     const size_t o = ((size_t)f * 5 + q) * 64 + threadIdx.x;
-    const double dF = flux_fine[o] - flux_coarse[o];
+    const real dF = flux_fine[o] - flux_coarse[o];
     Un[q] = hi ? P[q * 512] - dtdh * dF : P[q * 512] + dtdh * dF;
   }
   const bool ok = is_physical(Un);                           // Eq. 30 on the corrected cell
@@ -41,24 +41,24 @@ __global__ void __launch_bounds__(64) flux_correction_kernel(double* __restrict_
 }
 
 // limited slopes of the five components of V[0] from its six neighbours, times 1/4 (children sit a quarter cell off)
-SRHD_DEV void quarter_slopes(const double V[7][5], double beta, double sl[3][5]) {
+SRHD_DEV void quarter_slopes(const real V[7][5], real beta, real sl[3][5]) {
 #pragma unroll
   for (int d = 0; d < 3; ++d)
 #pragma unroll
     for (int q = 0; q < 5; ++q)
-      sl[d][q] = 0.25 * limited_slope(V[0][q] - V[1 + 2 * d][q], V[2 + 2 * d][q] - V[0][q], beta);
+      sl[d][q] = real(0.25) * limited_slope(V[0][q] - V[1 + 2 * d][q], V[2 + 2 * d][q] - V[0][q], beta);
 }
-SRHD_DEV void child_of(const double V0[5], const double sl[3][5], int ch, double v[5]) {
+SRHD_DEV void child_of(const real V0[5], const real sl[3][5], int ch, real v[5]) {
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
-    const double ax = (ch & 1) ? sl[0][q] : -sl[0][q], ay = (ch & 2) ? sl[1][q] : -sl[1][q],
+    const real ax = (ch & 1) ? sl[0][q] : -sl[0][q], ay = (ch & 2) ? sl[1][q] : -sl[1][q],
                  az = (ch & 4) ? sl[2][q] : -sl[2][q];
     v[q] = ((V0[q] + ax) + ay) + az;
   }
 }
 
-__global__ void __launch_bounds__(128) ghost_interp_kernel(const double* __restrict__ coarse, int nx, int ny, int nz,
-                                                           double* __restrict__ fine, double beta, double rtol,
+__global__ void __launch_bounds__(128) ghost_interp_kernel(const real* __restrict__ coarse, int nx, int ny, int nz,
+                                                           real* __restrict__ fine, real beta, real rtol,
                                                            int max_iter, unsigned char* __restrict__ fallback,
                                                            unsigned long long* __restrict__ n_fallback) {
   const int mx = nx - 2, my = ny - 2, mz = nz - 2;
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const double* __restr
     const int i = (int)(e % mx) + 1, j = (int)((e / mx) % my) + 1, k = (int)(e / ((long long)mx * my)) + 1;
     const size_t c = ((size_t)k * ny + j) * nx + i;
     const ptrdiff_t stp[3] = {1, nx, (ptrdiff_t)nx * ny};
-    double Q[7][5];
+    real Q[7][5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       Q[0][q] = __ldg(coarse + q * n + c);
@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const double* __restr
         Q[2 + 2 * d][q] = __ldg(coarse + q * n + c + stp[d]);
       }
     }
-    double sl[3][5], child[8][5];
+    real sl[3][5], child[8][5];
     quarter_slopes(Q, beta, sl);
     bool ok = true;
 #pragma unroll
@@ -96,10 +96,10 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const double* __restr
     // the fallback converts seven states per cell: a warp-wide loop (cons2prim's Newton iteration votes), entered
     // by every lane as soon as one lane needs it; lanes that do not need it discard the result
     if (__any_sync(0xffffffffu, !ok)) {
-      double W[7][5];
+      real W[7][5];
 #pragma unroll
       for (int m = 0; m < 7; ++m) {
-        double U1[1][5], W1[1][5];
+        real U1[1][5], W1[1][5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) U1[0][q] = Q[m][q];
         bool phys[1];
@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const double* __restr
         quarter_slopes(W, beta, sl);
 #pragma unroll
         for (int ch = 0; ch < 8; ++ch) {
-          double v[5];
+          real v[5];
           child_of(W[0], sl, ch, v);
           prim2cons(v, child[ch]);
         }
@@ -138,13 +138,13 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const double* __restr
 
 using namespace srhd;
 
-extern "C" int srhd_flux_correction(double* patches, const double* flux_coarse, const double* flux_fine,
+extern "C" int srhd_flux_correction(real* patches, const real* flux_coarse, const real* flux_fine,
                                     const int* face_patch, const int* face_id, int nf, double dt, double dh,
                                     unsigned long long* d_n_skipped, void* stream) {
   if (nf < 0) return SRHD_ERR_BAD_SIZE;
   if (!d_n_skipped || (nf > 0 && (!patches || !flux_coarse || !flux_fine || !face_patch || !face_id)))
     return SRHD_ERR_NULL_POINTER;
-  if (!(dt > 0.0) || !(dh > 0.0) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
+  if (!(dt > real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   cudaError_t e = cudaMemsetAsync(d_n_skipped, 0, sizeof(unsigned long long), st);
   if (e != cudaSuccess) return (int)e;
@@ -155,14 +155,14 @@ extern "C" int srhd_flux_correction(double* patches, const double* flux_coarse, 
   return (int)cudaGetLastError();
 }
 
-extern "C" int srhd_ghost_interp(const double* coarse, int nx, int ny, int nz, double* fine, double minmod_coeff,
+extern "C" int srhd_ghost_interp(const real* coarse, int nx, int ny, int nz, real* fine, double minmod_coeff,
                                  const srhd_params* params, unsigned char* fallback,
                                  unsigned long long* d_n_fallback, void* stream) {
   if (!coarse || !fine || !d_n_fallback) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
   if (nx < 3 || ny < 3 || nz < 3) return SRHD_ERR_BAD_SIZE;
-  if (!(minmod_coeff >= 0.0) || !(minmod_coeff <= 2.0)) return SRHD_ERR_BAD_PARAMS;
+  if (!(minmod_coeff >= real(0.0)) || !(minmod_coeff <= real(2.0))) return SRHD_ERR_BAD_PARAMS;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   cudaError_t e = cudaMemsetAsync(d_n_fallback, 0, sizeof(unsigned long long), st);
   if (e != cudaSuccess) return (int)e;

@@ -87,33 +87,34 @@ struct Plan {
   static constexpr int oFY = oFX + 5 * NFXY;
   static constexpr int oFZ = oFY + 5 * NFXY;          // z flux through the lower face of each column's cell
   static constexpr int oCtl = oFZ + 5 * ZS;           // control block (struct Ctl)
-  static constexpr int nDoubles = oCtl + 10;
-  static constexpr size_t bytes = (size_t)nDoubles * sizeof(double);
+  static_assert(oCtl % 2 == 0, "the control block needs 8-byte alignment in every precision");
+  static constexpr size_t bytes = (size_t)oCtl * sizeof(real) + 96;   // + struct Ctl
 };
 
 struct Ctl {                       // lives in shared memory
   uint64_t mbar;
   unsigned long long newton;
-  unsigned long long umax_bits;
+  rbits umax_bits;
   unsigned int face_fail, cell_fail, in_fail;
   int queue;                       // next chunk of interval X
   unsigned int abort;              // a failure was seen in this (non-final) pass: abandon it at the plane's end
   unsigned int exec_c2p, exec_riemann, exec_hancock;
   unsigned long long exec_newton;
 };
+static_assert(sizeof(Ctl) <= 96, "Plan<G>::bytes reserves 96 bytes for the control block");
 
 // Hancock stage of one (cell, direction) lane: PLM/PPM edge values of the five primitives along d
 // (stencil offsets o[] into the primitive ring, component stride PL), prim2cons and physical flux
 // of both edge states; returns the un-evolved conserved edge states and dF = F(W+) - F(W-).
 template <int G>
-SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 * G - 1], double beta,
-                           double beta0, double um[5], double up[5], double dF[5]) {
+SRHD_DEV bool hancock_lane(const real* __restrict__ Wr, int d, const int o[2 * G - 1], real beta,
+                           real beta0, real um[5], real up[5], real dF[5]) {
   using P = Plan<G>;
-  double wm[5], wp[5];
+  real wm[5], wp[5];
   bool allflat = true;
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
-    double a[2 * G - 1];
+    real a[2 * G - 1];
 #pragma unroll
     for (int m = 0; m < 2 * G - 1; ++m) a[m] = Wr[o[m] + q * P::PL];
     // A constant stencil (ambient gas ahead of a blast wave or a jet) has zero slopes and edge values
@@ -131,7 +132,7 @@ SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
       recon_ppm(a, beta, beta0, wm[q], wp[q]);
     }
   }
-  double Fm[5], Fp[5];
+  real Fm[5], Fp[5];
   Aux am, ap;
   if (__all_sync(0xffffffffu, allflat)) {
     // every lane's two edge states are the same state: one conversion, and F(W+) - F(W-) = +0 exactly
@@ -139,7 +140,7 @@ SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       up[q] = um[q];
-      dF[q] = 0.0;
+      dF[q] = real(0.0);
     }
     return true;
   }
@@ -162,28 +163,28 @@ SRHD_DEV bool hancock_lane(const double* __restrict__ Wr, int d, const int o[2 *
 constexpr int kScanThreads = 256;
 template <int G, int RS>
 __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
-    const double* __restrict__ cons_in, double* __restrict__ cons_out, double* __restrict__ flux_out, double dt,
-    double dh, double rtol, int max_iter, srhd_stats* __restrict__ stats, const double* __restrict__ d_smax,
-    double cfl, double min_speed, unsigned char* __restrict__ handled) {
+    const real* __restrict__ cons_in, real* __restrict__ cons_out, real* __restrict__ flux_out, real dt,
+    real dh, real rtol, int max_iter, srhd_stats* __restrict__ stats, const real* __restrict__ d_smax,
+    real cfl, real min_speed, unsigned char* __restrict__ handled) {
   using P = Plan<G>;
   constexpr int NT = kScanThreads, T3 = P::T3;
   constexpr int H = T3 / 2;                                  // 16-byte words per component
   static_assert(T3 % 2 == 0, "tile components must be whole 16-byte words");
   const int tid = threadIdx.x;
-  const double* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
+  const real* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
   if (tid == 0) handled[blockIdx.x] = 0;
-  const double2* __restrict__ t2 = reinterpret_cast<const double2*>(tile);
-  unsigned long long ref[5];
+  const real2* __restrict__ t2 = reinterpret_cast<const real2*>(tile);
+  rbits ref[5];
 #pragma unroll
-  for (int q = 0; q < 5; ++q) ref[q] = (unsigned long long)__double_as_longlong(__ldg(tile + (size_t)q * T3));
-  auto differs = [&](int w, double2 v) {
+  for (int q = 0; q < 5; ++q) ref[q] = real_bits(__ldg(tile + (size_t)q * T3));
+  auto differs = [&](int w, real2 v) {
     const int q = w / H;
-    const unsigned long long r = (q == 0) ? ref[0] : (q == 1) ? ref[1] : (q == 2) ? ref[2] : (q == 3) ? ref[3] : ref[4];
-    return ((unsigned long long)__double_as_longlong(v.x) != r) || ((unsigned long long)__double_as_longlong(v.y) != r);
+    const rbits r = (q == 0) ? ref[0] : (q == 1) ? ref[1] : (q == 2) ? ref[2] : (q == 3) ? ref[3] : ref[4];
+    return (real_bits(v.x) != r) || (real_bits(v.y) != r);
   };
   if (__syncthreads_or(differs(tid, __ldg(t2 + tid)) ? 1 : 0)) return;      // the first 4 KB settle most tiles
   for (int base = NT; base < 5 * H; base += 8 * NT) {
-    double2 v[8];
+    real2 v[8];
     int w[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
@@ -196,10 +197,10 @@ __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
     if (__syncthreads_or(diff ? 1 : 0)) return;
   }
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);      // as the main kernel (srhd_fluid_step_cfl)
-  if (!(fabs(dt / dh) <= DBL_MAX)) return;                   // U0 - (dt/dh) 0 = U0 needs a finite dt/dh
-  double U0[5];
+  if (!(fabs(dt / dh) <= kRealMax)) return;                   // U0 - (dt/dh) 0 = U0 needs a finite dt/dh
+  real U0[5];
 #pragma unroll
-  for (int q = 0; q < 5; ++q) U0[q] = __longlong_as_double((long long)ref[q]);
+  for (int q = 0; q < 5; ++q) U0[q] = bits_real((rbits)ref[q]);
   UniformResult r;
   if (!uniform_eval<RS>(U0, rtol, max_iter, r)) return;      // every thread computed the same verdict
   uniform_write(cons_out + (size_t)blockIdx.x * 8 * 5 * 512,
@@ -212,10 +213,10 @@ __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
 
 template <int G, int RS>
 __global__ void __launch_bounds__(kFluidThreads, 1)
-fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_out,
-                  double* __restrict__ flux_out, double dt, double dh, double beta0, int max_retry, double rtol,
-                  int max_iter, srhd_stats* __restrict__ stats, const double* __restrict__ d_smax, double cfl,
-                  double min_speed, const unsigned char* __restrict__ handled) {
+fluid_step_kernel(const real* __restrict__ cons_in, real* __restrict__ cons_out,
+                  real* __restrict__ flux_out, real dt, real dh, real beta0, int max_retry, real rtol,
+                  int max_iter, srhd_stats* __restrict__ stats, const real* __restrict__ d_smax, real cfl,
+                  real min_speed, const unsigned char* __restrict__ handled) {
   using P = Plan<G>;
   constexpr int NT = kFluidThreads, NW = NT / 32;
   if (handled[blockIdx.x]) return;              // a uniform tile: uniform_tiles_kernel wrote its result
@@ -224,26 +225,26 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   constexpr int NXY = 2 * P::NFXY / 32;         // x and y face chunks per plane (544 faces = 17 x 32)
   static_assert(2 * P::NFXY % 32 == 0 && NW >= 8, "face list must be whole warps; z faces need 8 warps");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  double* sm = reinterpret_cast<double*>(smem_raw);
-  double* Wr = sm + P::oW;
-  double* Stg = sm + P::oStg;
-  double* XSm = sm + P::oXSm;
-  double* XSp = sm + P::oXSp;
-  double* YSm = sm + P::oYSm;
-  double* YSp = sm + P::oYSp;
-  double* ZSm = sm + P::oZSm;
-  double* ZSp = sm + P::oZSp;
-  double* FX = sm + P::oFX;
-  double* FY = sm + P::oFY;
-  double* FZ = sm + P::oFZ;     // written and read by the thread that owns the column: no barrier needed
+  real* sm = reinterpret_cast<real*>(smem_raw);
+  real* Wr = sm + P::oW;
+  real* Stg = sm + P::oStg;
+  real* XSm = sm + P::oXSm;
+  real* XSp = sm + P::oXSp;
+  real* YSm = sm + P::oYSm;
+  real* YSp = sm + P::oYSp;
+  real* ZSm = sm + P::oZSm;
+  real* ZSp = sm + P::oZSp;
+  real* FX = sm + P::oFX;
+  real* FY = sm + P::oFY;
+  real* FZ = sm + P::oFZ;     // written and read by the thread that owns the column: no barrier needed
   Ctl* ctl = reinterpret_cast<Ctl*>(sm + P::oCtl);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const double* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
-  double* __restrict__ out = cons_out + (size_t)blockIdx.x * 8 * 5 * 512;
-  double* __restrict__ fout = flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr;
+  const real* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
+  real* __restrict__ out = cons_out + (size_t)blockIdx.x * 8 * 5 * 512;
+  real* __restrict__ fout = flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr;
   // flux through a patch-boundary face -> flux_out[patch][face][comp][a][b] (include/srhd.h)
-  auto put_flux = [&](int p, int f, int a, int b, const double F[5]) {
+  auto put_flux = [&](int p, int f, int a, int b, const real F[5]) {
 #pragma unroll
     for (int q = 0; q < 5; ++q) fout[(((size_t)p * 6 + f) * 5 + q) * 64 + a * 8 + b] = F[q];
   };
@@ -251,7 +252,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   if (tid == 0) {
     mbar_init(&ctl->mbar, 1);
     ctl->newton = 0ull;
-    ctl->umax_bits = 0ull;
+    ctl->umax_bits = 0;
     ctl->face_fail = ctl->cell_fail = ctl->in_fail = 0u;
     ctl->queue = 0;
     ctl->abort = 0u;
@@ -269,8 +270,8 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   // of the 32): decode them once.  info = in-plane tile index | store offset << 9 | has-edge-array
   // << 18 | interior-column << 19
   static_assert(NW == 16, "the Hancock stage maps 32 chunks of 10 cells onto exactly two rounds of 16 warps");
-  double* const hpm = (hd == 0) ? XSm : ((hd == 1) ? YSm : ZSm);
-  double* const hpp = (hd == 0) ? XSp : ((hd == 1) ? YSp : ZSp);
+  real* const hpm = (hd == 0) ? XSm : ((hd == 1) ? YSm : ZSm);
+  real* const hpp = (hd == 0) ? XSp : ((hd == 1) ? YSp : ZSp);
   const int hqs = (hd == 0) ? P::XS : ((hd == 1) ? P::YS : P::ZS);
   int hinfo[2];
 #pragma unroll
@@ -293,8 +294,8 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   }
 
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);   // Eq. 28 formed on the device (srhd_fluid_step_cfl)
-  const double hdt = dt / (2.0 * dh);
-  const double dtdh = dt / dh;
+  const real hdt = dt / (real(2.0) * dh);
+  const real dtdh = dt / dh;
 
   unsigned long long my_iters = 0;     // iterations of the algorithm's conversions (centre cells + accepted pass)
   unsigned long long ex_newton = 0;    // executed work (every pass, shortcuts taken into account)
@@ -302,28 +303,28 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   int phase_base = 0;                  // TMA phases completed before the current pass (mbarrier parity)
   int planes_counted = 0;              // tile planes whose cells already fed newton_iters / S_max / Eq. 30 counters
   unsigned my_in_fail = 0;
-  double my_umax = 0.0;
-  double beta = beta0;
+  real my_umax = real(0.0);
+  real beta = beta0;
   int pass = 0;
   unsigned n_face_fail = 0, n_cell_fail = 0;
 
   // TMA: conserved tile plane pl -> staging buffer (thread 0 only)
   auto issue_plane = [&](int pl) {
     fence_proxy_async();
-    mbar_expect_tx(&ctl->mbar, 5u * PL * 8u);
+    mbar_expect_tx(&ctl->mbar, 5u * PL * (uint32_t)sizeof(real));
 #pragma unroll
     for (int q = 0; q < 5; ++q)
-      bulk_g2s(Stg + q * PL, tile + (size_t)q * T3 + (size_t)pl * PL, PL * 8u, &ctl->mbar);
+      bulk_g2s(Stg + q * PL, tile + (size_t)q * T3 + (size_t)pl * PL, PL * (uint32_t)sizeof(real), &ctl->mbar);
   };
   // cons2prim of 32 cells of the staged plane pl into its ring slot (Eq. 15-18); pass 0 also feeds
   // the CFL reduction (Eq. 26) and the Eq. 30 counter from the input-interior cells
   auto convert_chunk = [&](int pl, int chunk) {
     mbar_wait(&ctl->mbar, (uint32_t)((phase_base + pl) & 1));   // one phase per staged plane, in order
-    double* Ws = Wr + (pl % R) * 5 * PL;
+    real* Ws = Wr + (pl % R) * 5 * PL;
     const int item = chunk * 32 + lane;
     const bool valid = item < PL;
     const int c = valid ? item : PL - 1;
-    double U[1][5], W[1][5];
+    real U[1][5], W[1][5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) U[0][q] = Stg[q * PL + c];
     bool phys[1];
@@ -349,7 +350,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
   };
 
   for (;; ++pass) {
-    if (pass > 0) beta = (pass <= max_retry) ? beta * 0.75 : 0.0;
+    if (pass > 0) beta = (pass <= max_retry) ? beta * real(0.75) : real(0.0);
     if (tid == 0) {
       ctl->face_fail = 0u;
       ctl->cell_fail = 0u;
@@ -360,7 +361,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     unsigned long long pass_iters = 0;            // Newton iterations of this pass's face conversions
     bool flagged = false, aborted = false;
     int planes_staged = NXT;
-    double part[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // (Fx+ - Fx-) + (Fy+ - Fy-) of this thread's column cell
+    real part[5] = {real(0.0), real(0.0), real(0.0), real(0.0), real(0.0)};   // (Fx+ - Fx-) + (Fy+ - Fy-) of this thread's column cell
 
     // ---- prologue: tile plane 0 -> primitives; stage plane 1
     for (int chunk = warp; chunk < NP1; chunk += NW) convert_chunk(0, chunk);
@@ -375,8 +376,8 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
         const int i = tid & 15, j = tid >> 4;
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          const double dfx = FX[q * P::NFXY + j * 17 + i + 1] - FX[q * P::NFXY + j * 17 + i];
-          const double dfy = FY[q * P::NFXY + (j + 1) * 16 + i] - FY[q * P::NFXY + j * 16 + i];
+          const real dfx = FX[q * P::NFXY + j * 17 + i + 1] - FX[q * P::NFXY + j * 17 + i];
+          const real dfy = FY[q * P::NFXY + (j + 1) * 16 + i] - FY[q * P::NFXY + j * 16 + i];
           part[q] = dfx + dfy;
         }
       }
@@ -397,11 +398,11 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           for (int m = -(G - 1); m <= G - 1; ++m)
             o[m + G - 1] = (hd == 2) ? (((tk + m) % R) * 5 * PL + cidx)
                                      : ((tk % R) * 5 * PL + cidx + m * ((hd == 0) ? 1 : NXT));
-          double um[5], up[5], dF[5];
+          real um[5], up[5], dF[5];
           const bool warp_flat = hancock_lane<G>(Wr, hd, o, beta, beta0, um, up, dF);
           ex_hancock += (valid && !warp_flat) ? 1u : 0u;
-          double* pm = hpm + soff;
-          double* pp = hpp + soff + ((hd == 2) ? zb * 5 * P::ZS : 0);
+          real* pm = hpm + soff;
+          real* pp = hpp + soff + ((hd == 2) ? zb * 5 * P::ZS : 0);
           const int qs = hqs;
           bool has = ((info >> 18) & 1) && (hd == 2 || inplane);
           has = has && valid;
@@ -424,10 +425,10 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           __syncwarp();
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            const double fx = __shfl_sync(0xffffffffu, dF[q], hbase);
-            const double fy = __shfl_sync(0xffffffffu, dF[q], hbase + 1);
-            const double fz = __shfl_sync(0xffffffffu, dF[q], hbase + 2);
-            const double dU = -hdt * ((fx + fy) + fz);
+            const real fx = __shfl_sync(0xffffffffu, dF[q], hbase);
+            const real fy = __shfl_sync(0xffffffffu, dF[q], hbase + 1);
+            const real fz = __shfl_sync(0xffffffffu, dF[q], hbase + 2);
+            const real dU = -hdt * ((fx + fy) + fz);
             if (has) {
               pm[q * qs] = um[q] + dU;
               pp[q * qs] = up[q] + dU;
@@ -461,7 +462,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
             idx = 256 + c * 32 + lane;
           }
           int d, qs;
-          const double *pL, *pR;
+          const real *pL, *pR;
           if (idx < 256) {
             d = 2;
             qs = P::ZS;
@@ -480,7 +481,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
             pL = YSp + f;
             pR = YSm + f + 16;
           }
-          double U[2][5], W[2][5], F[5];
+          real U[2][5], W[2][5], F[5];
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
             U[0][q] = pL[q * qs];
@@ -538,13 +539,13 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
           if (idx < 256) {
             if (kh >= 1) {                          // update cell (i, j, kh-1): Eq. 4a, 4b, 7; S12
               const int ku = kh - 1, i = idx & 15, j = idx >> 4;
-              const double* uin = tile + ((size_t)(ku + G) * NXT + (j + G)) * NXT + (i + G);
+              const real* uin = tile + ((size_t)(ku + G) * NXT + (j + G)) * NXT + (i + G);
               const int p = (i >> 3) + 2 * (j >> 3) + 4 * (ku >> 3);   // S13
-              double* o = out + (size_t)p * 5 * 512 + (ku & 7) * 64 + (j & 7) * 8 + (i & 7);
-              double Un[5];
+              real* o = out + (size_t)p * 5 * 512 + (ku & 7) * 64 + (j & 7) * 8 + (i & 7);
+              real Un[5];
 #pragma unroll
               for (int q = 0; q < 5; ++q) {
-                const double dfz = F[q] - FZ[q * P::ZS + idx];
+                const real dfz = F[q] - FZ[q * P::ZS + idx];
                 Un[q] = __ldg(uin + (size_t)q * T3) - dtdh * (part[q] + dfz);
                 o[q * 512] = Un[q];
               }
@@ -568,13 +569,13 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
         }
         // A failure anywhere fails the whole pass (S9, S15), so a pass that is not the last rung of the
         // ladder can be abandoned as soon as one is seen: same verdict, same accepted pass, less work.
-        if (!flagged && beta != 0.0 && (my_face_fail | my_cell_fail) != 0u) {
+        if (!flagged && beta != real(0.0) && (my_face_fail | my_cell_fail) != 0u) {
           *reinterpret_cast<volatile unsigned int*>(&ctl->abort) = 1u;
           flagged = true;
         }
       }
       __syncthreads();
-      if (beta != 0.0 && s + 1 < NXT && *reinterpret_cast<volatile unsigned int*>(&ctl->abort) != 0u) {
+      if (beta != real(0.0) && s + 1 < NXT && *reinterpret_cast<volatile unsigned int*>(&ctl->abort) != 0u) {
         aborted = true;                           // block uniform; planes 0 .. s+1 were staged and consumed
         planes_staged = s + 2;
         break;
@@ -601,7 +602,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     n_face_fail = ctl->face_fail;
     n_cell_fail = ctl->cell_fail;
     __syncthreads();
-    if ((n_face_fail == 0 && n_cell_fail == 0) || beta == 0.0) {
+    if ((n_face_fail == 0 && n_cell_fail == 0) || beta == real(0.0)) {
       my_iters += pass_iters;                     // the accepted pass's face conversions count, no other pass's
       break;
     }
@@ -622,7 +623,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     atomicAdd(&ctl->exec_hancock, ex_hancock);
     atomicAdd(&ctl->newton, my_iters);
     if (my_in_fail) atomicAdd(&ctl->in_fail, my_in_fail);
-    atomicMax(&ctl->umax_bits, (unsigned long long)__double_as_longlong(my_umax));
+    atomicMax(&ctl->umax_bits, real_bits(my_umax));
   }
   __syncthreads();
   if (tid == 0 && stats) {
@@ -636,7 +637,7 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
     atomicAdd(&stats->exec_c2p, (unsigned long long)ctl->exec_c2p);
     atomicAdd(&stats->exec_riemann, (unsigned long long)ctl->exec_riemann);
     atomicAdd(&stats->exec_hancock, (unsigned long long)ctl->exec_hancock);
-    const double umax = __longlong_as_double((long long)ctl->umax_bits);
+    const real umax = bits_real((rbits)ctl->umax_bits);
     atomic_max_nonneg(&stats->max_speed, smax_of_umax(umax));      // Eq. 27 per group, then max
   }
 }
@@ -644,14 +645,14 @@ fluid_step_kernel(const double* __restrict__ cons_in, double* __restrict__ cons_
 // handled == nullptr: run the uniform-tile pre-pass first (flags in a stream-ordered scratch allocation);
 // else the caller has run a pre-pass of its own and only the march is launched
 template <int G, int RS>
-int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-                 const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-                 double min_speed, const unsigned char* handled) {
+int launch_fluid(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt, real dh,
+                 const srhd_params* p, srhd_stats* stats, cudaStream_t st, const real* d_smax, real cfl,
+                 real min_speed, const unsigned char* handled) {
   auto kern = fluid_step_kernel<G, RS>;
   const size_t smem = Plan<G>::bytes;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
-  const double rtol = newton_stop_rtol(p->newton_rtol);
+  const real rtol = newton_stop_rtol(p->newton_rtol);
   unsigned char* scratch = nullptr;
   if (!handled) {
     e = cudaMallocAsync(reinterpret_cast<void**>(&scratch), (size_t)npg, st);
@@ -667,9 +668,9 @@ int launch_fluid(const double* cons_in, double* cons_out, double* flux_out, int 
   return (int)(e != cudaSuccess ? e : e2);
 }
 
-int fluid_march(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-                const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-                double min_speed, const unsigned char* handled) {
+int fluid_march(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt, real dh,
+                const srhd_params* p, srhd_stats* stats, cudaStream_t st, const real* d_smax, real cfl,
+                real min_speed, const unsigned char* handled) {
   if (p->recon == SRHD_RECON_PLM) {
     return p->riemann == SRHD_RIEMANN_HLLE
                ? launch_fluid<2, 0>(cons_in, cons_out, flux_out, npg, dt, dh, p, stats, st, d_smax, cfl, min_speed, handled)
@@ -683,9 +684,9 @@ int fluid_march(const double* cons_in, double* cons_out, double* flux_out, int n
 }  // namespace srhd
 
 namespace srhd {   // srhd_vl.cu
-int vl_step(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-            const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-            double min_speed);
+int vl_step(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt, real dh,
+            const srhd_params* p, srhd_stats* stats, cudaStream_t st, const real* d_smax, real cfl,
+            real min_speed);
 size_t vl_workspace_bytes(int npg, const srhd_params* p);
 }  // namespace srhd
 
@@ -697,19 +698,19 @@ extern "C" size_t srhd_workspace_bytes(int npg, const srhd_params* params) {
   return vl_workspace_bytes(npg, params);
 }
 
-static int fluid_step_impl(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt,
-                           double dh, const srhd_params* params, srhd_stats* stats, void* stream,
-                           const double* d_smax, double cfl, double min_speed) {
+static int fluid_step_impl(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt,
+                           real dh, const srhd_params* params, srhd_stats* stats, void* stream,
+                           const real* d_smax, real cfl, real min_speed) {
   if (npg > 0 && (!cons_in || !cons_out)) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
   if (npg < 0) return SRHD_ERR_BAD_SIZE;
-  if (!(dt > 0.0) || !(dh > 0.0) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
+  if (!(dt > real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
   if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & 7u))
     return SRHD_ERR_BAD_ALIGN;
   const int nxt = 16 + 2 * params->ghost;
-  const size_t in_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(double);
-  const size_t out_bytes = (size_t)npg * 8 * 5 * 512 * sizeof(double);
+  const size_t in_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(real);
+  const size_t out_bytes = (size_t)npg * 8 * 5 * 512 * sizeof(real);
   const uintptr_t a = reinterpret_cast<uintptr_t>(cons_in), b = reinterpret_cast<uintptr_t>(cons_out);
   if (a < b + out_bytes && b < a + in_bytes) return SRHD_ERR_ALIAS;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -723,23 +724,23 @@ static int fluid_step_impl(const double* cons_in, double* cons_out, double* flux
   return fluid_march(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, st, d_smax, cfl, min_speed, nullptr);
 }
 
-extern "C" int srhd_fluid_step_fluxes(const double* cons_in, double* cons_out, double* flux_out, int npg,
+extern "C" int srhd_fluid_step_fluxes(const real* cons_in, real* cons_out, real* flux_out, int npg,
                                       double dt, double dh, const srhd_params* params, srhd_stats* stats,
                                       void* stream) {
-  return fluid_step_impl(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, stream, nullptr, 0.0, 0.0);
+  return fluid_step_impl(cons_in, cons_out, flux_out, npg, dt, dh, params, stats, stream, nullptr, real(0.0), real(0.0));
 }
 
-extern "C" int srhd_fluid_step(const double* cons_in, double* cons_out, int npg, double dt, double dh,
+extern "C" int srhd_fluid_step(const real* cons_in, real* cons_out, int npg, double dt, double dh,
                                const srhd_params* params, srhd_stats* stats, void* stream) {
-  return fluid_step_impl(cons_in, cons_out, nullptr, npg, dt, dh, params, stats, stream, nullptr, 0.0, 0.0);
+  return fluid_step_impl(cons_in, cons_out, nullptr, npg, dt, dh, params, stats, stream, nullptr, real(0.0), real(0.0));
 }
 
-extern "C" int srhd_fluid_step_cfl(const double* cons_in, double* cons_out, double* flux_out, int npg, double cfl,
-                                   double dh, const double* d_max_speed, double min_speed,
+extern "C" int srhd_fluid_step_cfl(const real* cons_in, real* cons_out, real* flux_out, int npg, double cfl,
+                                   double dh, const real* d_max_speed, double min_speed,
                                    const srhd_params* params, srhd_stats* stats, void* stream) {
   if (!d_max_speed) return SRHD_ERR_NULL_POINTER;
-  if (!(cfl > 0.0) || !std::isfinite(cfl) || !(min_speed >= 0.0)) return SRHD_ERR_BAD_STEP;
+  if (!(cfl > real(0.0)) || !std::isfinite(cfl) || !(min_speed >= real(0.0))) return SRHD_ERR_BAD_STEP;
   // dt is formed on the device; the host-side check of dt is replaced by the one of cfl (dt = 1 passes it)
-  return fluid_step_impl(cons_in, cons_out, flux_out, npg, 1.0, dh, params, stats, stream, d_max_speed, cfl,
+  return fluid_step_impl(cons_in, cons_out, flux_out, npg, real(1.0), dh, params, stats, stream, d_max_speed, cfl,
                          min_speed);
 }

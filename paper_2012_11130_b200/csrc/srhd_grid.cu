@@ -8,7 +8,7 @@ namespace srhd {
 
 struct GridBC {
   int bc[6];
-  double inflow[5];
+  real inflow[5];
   int has_inflow;
 };
 
@@ -25,8 +25,8 @@ SRHD_DEV int map_index(int i, int n, int bc_lo, int bc_hi) {
 // into shared-memory tables, so an element costs one index split (compile-time extents), three table
 // reads, one load and one store; four elements in flight per thread.
 template <int G>
-__global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restrict__ grid,
-                                                          double* __restrict__ cons_in, int nx, int ny,
+__global__ void __launch_bounds__(256) grid_gather_kernel(const real* __restrict__ grid,
+                                                          real* __restrict__ cons_in, int nx, int ny,
                                                           int nz, GridBC b,
                                                           const unsigned char* __restrict__ mask) {
   constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
@@ -45,11 +45,11 @@ __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restri
     zs[t] = (b.has_inflow && kk < 0) ? -1 - off : off;
   }
   __syncthreads();
-  const double* __restrict__ src = grid + (size_t)q * n;
-  double* __restrict__ dst = cons_in + ((size_t)pg * 5 + q) * t3;
-  const double inflow_q = b.inflow[q];
+  const real* __restrict__ src = grid + (size_t)q * n;
+  real* __restrict__ dst = cons_in + ((size_t)pg * 5 + q) * t3;
+  const real inflow_q = b.inflow[q];
   for (int c0 = threadIdx.x; c0 < t3; c0 += 4 * 256) {
-    double v[4];
+    real v[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int c = c0 + u * 256;
@@ -74,19 +74,19 @@ __global__ void __launch_bounds__(256) grid_gather_kernel(const double* __restri
 }
 
 // one CTA per (patch group, component): 4096 cells, writes coalesced along x in 16-cell rows
-__global__ void __launch_bounds__(256) grid_scatter_kernel(const double* __restrict__ cons_out,
-                                                           double* __restrict__ grid, int nx, int ny,
+__global__ void __launch_bounds__(256) grid_scatter_kernel(const real* __restrict__ cons_out,
+                                                           real* __restrict__ grid, int nx, int ny,
                                                            int nz) {
   const int px = nx / 16, py = ny / 16;
   const int pg = blockIdx.x, q = blockIdx.y;
   const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
   const size_t n = (size_t)nx * ny * nz;
-  const double* __restrict__ src = cons_out + (size_t)pg * 8 * 5 * 512;
-  double* __restrict__ dst = grid + (size_t)q * n;
+  const real* __restrict__ src = cons_out + (size_t)pg * 8 * 5 * 512;
+  real* __restrict__ dst = grid + (size_t)q * n;
   for (int c = threadIdx.x; c < 4096; c += blockDim.x) {
     const int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
     const int p = (i >> 3) + 2 * (j >> 3) + 4 * (k >> 3);
-    const double v = __ldg(src + ((size_t)p * 5 + q) * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7));
+    const real v = __ldg(src + ((size_t)p * 5 + q) * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7));
     dst[((size_t)(gz * 16 + k) * ny + (gy * 16 + j)) * nx + (gx * 16 + i)] = v;
   }
 }
@@ -94,22 +94,22 @@ __global__ void __launch_bounds__(256) grid_scatter_kernel(const double* __restr
 // The scatter fused with the CFL reduction of the state it writes (Eq. 26): one CTA per patch group,
 // each thread moves all five components of its cells, converts them (cons2prim) and keeps the
 // running max of U_max; the copy is memory bound and the conversion ALU bound, so they overlap.
-__global__ void __launch_bounds__(256) grid_scatter_speed_kernel(const double* __restrict__ cons_out,
-                                                                 double* __restrict__ grid, int nx, int ny, int nz,
-                                                                 double rtol, int max_iter,
-                                                                 double* __restrict__ umax_out) {
+__global__ void __launch_bounds__(256) grid_scatter_speed_kernel(const real* __restrict__ cons_out,
+                                                                 real* __restrict__ grid, int nx, int ny, int nz,
+                                                                 real rtol, int max_iter,
+                                                                 real* __restrict__ umax_out) {
   const int px = nx / 16, py = ny / 16;
   const int pg = blockIdx.x;
   const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
   const size_t n = (size_t)nx * ny * nz;
-  const double* __restrict__ src = cons_out + (size_t)pg * 8 * 5 * 512;
-  double umax = 0.0;
+  const real* __restrict__ src = cons_out + (size_t)pg * 8 * 5 * 512;
+  real umax = real(0.0);
   for (int c = threadIdx.x; c < 4096; c += 256) {          // 4096 = 16 x 256: every lane of every warp works
     const int i = c & 15, j = (c >> 4) & 15, k = c >> 8;
     const int p = (i >> 3) + 2 * (j >> 3) + 4 * (k >> 3);
     const size_t so = (size_t)p * 5 * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7);
     const size_t go = ((size_t)(gz * 16 + k) * ny + (gy * 16 + j)) * nx + (gx * 16 + i);
-    double U[1][5], W[1][5];
+    real U[1][5], W[1][5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       U[0][q] = __ldg(src + so + (size_t)q * 512);
@@ -130,12 +130,12 @@ __global__ void __launch_bounds__(256) grid_scatter_speed_kernel(const double* _
 // tile axes in shared-memory tables, as in grid_gather_kernel); loop B converts the group's own 16^3
 // cells (cons2prim) and keeps the running max of U_max (Eq. 26).
 template <int G>
-__global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* __restrict__ patches,
-                                                                 double* __restrict__ cons_in, int nx, int ny,
+__global__ void __launch_bounds__(256) patch_gather_speed_kernel(const real* __restrict__ patches,
+                                                                 real* __restrict__ cons_in, int nx, int ny,
                                                                  int nz, GridBC b,
                                                                  const unsigned char* __restrict__ mask,
-                                                                 double rtol, int max_iter,
-                                                                 double* __restrict__ umax_out) {
+                                                                 real rtol, int max_iter,
+                                                                 real* __restrict__ umax_out) {
   constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
   __shared__ int ax[nxt], ay[nxt], mx[nxt], my[nxt];
   __shared__ long long az[nxt];               // -1 - offset for a plane below z = 0 of an inflow boundary
@@ -156,9 +156,9 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* _
     az[t] = (b.has_inflow && kk < 0) ? -1 - off : off;
   }
   __syncthreads();
-  double* __restrict__ dst = cons_in + (size_t)pg * 5 * t3;
+  real* __restrict__ dst = cons_in + (size_t)pg * 5 * t3;
   for (int c0 = threadIdx.x; c0 < t3; c0 += 2 * 256) {     // loop A: two cells (ten loads) in flight
-    double v[2][5];
+    real v[2][5];
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
       const int c = c0 + u * 256;
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* _
           z = -1 - z;
           inflow = mask[my[j] + mx[i]] != 0;
         }
-        const double* __restrict__ sp = patches + z + ay[j] + ax[i];
+        const real* __restrict__ sp = patches + z + ay[j] + ax[i];
 #pragma unroll
         for (int q = 0; q < 5; ++q) v[u][q] = inflow ? b.inflow[q] : __ldg(sp + q * 512);
       }
@@ -185,11 +185,11 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* _
     }
   }
   // loop B: S_max of the group's own cells (every lane of every warp works: 4096 = 16 x 256)
-  const double* __restrict__ own = patches + (size_t)pg * 8 * 5 * 512;
-  double umax = 0.0;
+  const real* __restrict__ own = patches + (size_t)pg * 8 * 5 * 512;
+  real umax = real(0.0);
   for (int c = threadIdx.x; c < 4096; c += 256) {
     const size_t so = (size_t)(c >> 9) * 5 * 512 + (c & 511);
-    double U[1][5], W[1][5];
+    real U[1][5], W[1][5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) U[0][q] = __ldg(own + so + (size_t)q * 512);
     bool phys[1];
@@ -211,12 +211,12 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const double* _
 // and no tile is ever materialised.  Any other group gets its tile and the U_max of its 4096 cells exactly as
 // patch_gather_speed_kernel does it, and handled[pg] = 0 leaves it to fluid_step_kernel.
 template <int G, int RS>
-__global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __restrict__ patches,
-                                                            double* __restrict__ patches_out,
-                                                            double* __restrict__ cons_in,
-                                                            double* __restrict__ flux_out, int nx, int ny, int nz,
+__global__ void __launch_bounds__(256) patch_prepass_kernel(const real* __restrict__ patches,
+                                                            real* __restrict__ patches_out,
+                                                            real* __restrict__ cons_in,
+                                                            real* __restrict__ flux_out, int nx, int ny, int nz,
                                                             GridBC b, const unsigned char* __restrict__ mask,
-                                                            double rtol, int max_iter, double* __restrict__ umax_out,
+                                                            real rtol, int max_iter, real* __restrict__ umax_out,
                                                             srhd_stats* __restrict__ stats,
                                                             unsigned char* __restrict__ handled) {
   constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
@@ -240,9 +240,9 @@ __global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __rest
   }
   if (tid == 0) handled[pg] = 0;
   __syncthreads();
-  const double* __restrict__ own = patches + (size_t)pg * 8 * 5 * 512;
+  const real* __restrict__ own = patches + (size_t)pg * 8 * 5 * 512;
   // the five doubles of tile cell c as the gather would write them
-  auto tile_cell = [&](int c, double v[5]) {
+  auto tile_cell = [&](int c, real v[5]) {
     const int k = c / nrow, r = c - k * nrow, j = r / nxt, i = r - j * nxt;
     long long z = az[k];
     bool inflow = false;
@@ -250,24 +250,24 @@ __global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __rest
       z = -1 - z;
       inflow = mask[my[j] + mx[i]] != 0;
     }
-    const double* __restrict__ sp = patches + z + ay[j] + ax[i];
+    const real* __restrict__ sp = patches + z + ay[j] + ax[i];
 #pragma unroll
     for (int q = 0; q < 5; ++q) v[q] = inflow ? b.inflow[q] : __ldg(sp + q * 512);
   };
   // ---- phase 1: is the tile one state?
-  double U0[5];
+  real U0[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) U0[q] = __ldg(own + q * 512);
   bool uniform = true;
   for (int c0 = tid; c0 < t3; c0 += 2 * 256) {
-    double v[2][5];
+    real v[2][5];
     bool diff = false;
 #pragma unroll
     for (int u = 0; u < 2; ++u) tile_cell(min(c0 + u * 256, t3 - 1), v[u]);
 #pragma unroll
     for (int u = 0; u < 2; ++u)
 #pragma unroll
-      for (int q = 0; q < 5; ++q) diff = diff || (__double_as_longlong(v[u][q]) != __double_as_longlong(U0[q]));
+      for (int q = 0; q < 5; ++q) diff = diff || (real_bits(v[u][q]) != real_bits(U0[q]));
     if (__syncthreads_or(diff ? 1 : 0)) {
       uniform = false;
       break;
@@ -287,9 +287,9 @@ __global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __rest
     }
   }
   // ---- phase 2 (any other group): the tile and U_max of the group's own cells, as patch_gather_speed_kernel
-  double* __restrict__ dst = cons_in + (size_t)pg * 5 * t3;
+  real* __restrict__ dst = cons_in + (size_t)pg * 5 * t3;
   for (int c0 = tid; c0 < t3; c0 += 2 * 256) {
-    double v[2][5];
+    real v[2][5];
 #pragma unroll
     for (int u = 0; u < 2; ++u)
       if (c0 + u * 256 < t3) tile_cell(c0 + u * 256, v[u]);
@@ -302,10 +302,10 @@ __global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __rest
       }
     }
   }
-  double umax = 0.0;
+  real umax = real(0.0);
   for (int c = tid; c < 4096; c += 256) {
     const size_t so = (size_t)(c >> 9) * 5 * 512 + (c & 511);
-    double U[1][5], W[1][5];
+    real U[1][5], W[1][5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) U[0][q] = __ldg(own + so + (size_t)q * 512);
     bool phys[1];
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(256) patch_prepass_kernel(const double* __rest
   if ((tid & 31) == 0) atomic_max_nonneg(umax_out, umax);
 }
 
-__global__ void smax_finish_kernel2(double* v) { *v = smax_of_umax(*v); }   // Eq. 27 once, after the max
+__global__ void smax_finish_kernel2(real* v) { *v = smax_of_umax(*v); }   // Eq. 27 once, after the max
 
 }  // namespace srhd
 
@@ -329,7 +329,7 @@ static int check_extents(int nx, int ny, int nz) {
   return SRHD_OK;
 }
 
-extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int ny, int nz, int ghost,
+extern "C" int srhd_grid_gather(const real* grid, real* cons_in, int nx, int ny, int nz, int ghost,
                                 const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
                                 void* stream) {
   if (!grid || !cons_in || !bc) return SRHD_ERR_NULL_POINTER;
@@ -343,7 +343,7 @@ extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int
   }
   b.has_inflow = (inflow_mask != nullptr);
   if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
-  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
+  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : real(0.0);
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   if (ghost == 2)
     grid_gather_kernel<2><<<dim3(npg, 5), 256, 0, static_cast<cudaStream_t>(stream)>>>(grid, cons_in, nx, ny, nz,
@@ -357,7 +357,7 @@ extern "C" int srhd_grid_gather(const double* grid, double* cons_in, int nx, int
   return (int)cudaGetLastError();
 }
 
-extern "C" int srhd_grid_scatter(const double* cons_out, double* grid, int nx, int ny, int nz, void* stream) {
+extern "C" int srhd_grid_scatter(const real* cons_out, real* grid, int nx, int ny, int nz, void* stream) {
   if (!cons_out || !grid) return SRHD_ERR_NULL_POINTER;
   const int ce = check_extents(nx, ny, nz);
   if (ce) return ce;
@@ -366,15 +366,15 @@ extern "C" int srhd_grid_scatter(const double* cons_out, double* grid, int nx, i
   return (int)cudaGetLastError();
 }
 
-extern "C" int srhd_grid_scatter_speed(const double* cons_out, double* grid, int nx, int ny, int nz,
-                                       const srhd_params* params, double* d_max_speed, void* stream) {
+extern "C" int srhd_grid_scatter_speed(const real* cons_out, real* grid, int nx, int ny, int nz,
+                                       const srhd_params* params, real* d_max_speed, void* stream) {
   if (!cons_out || !grid || !d_max_speed) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
   const int ce = check_extents(nx, ny, nz);
   if (ce) return ce;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(double), st);
+  const cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(real), st);
   if (e != cudaSuccess) return (int)e;
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   grid_scatter_speed_kernel<<<npg, 256, 0, st>>>(cons_out, grid, nx, ny, nz, newton_stop_rtol(params->newton_rtol),
@@ -383,9 +383,9 @@ extern "C" int srhd_grid_scatter_speed(const double* cons_out, double* grid, int
   return (int)cudaGetLastError();
 }
 
-extern "C" int srhd_patch_gather_speed(const double* patches, double* cons_in, int nx, int ny, int nz,
+extern "C" int srhd_patch_gather_speed(const real* patches, real* cons_in, int nx, int ny, int nz,
                                        const int* bc, const unsigned char* inflow_mask, const double* inflow_cons,
-                                       const srhd_params* params, double* d_max_speed, void* stream) {
+                                       const srhd_params* params, real* d_max_speed, void* stream) {
   if (!patches || !cons_in || !bc || !d_max_speed) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
@@ -398,12 +398,12 @@ extern "C" int srhd_patch_gather_speed(const double* patches, double* cons_in, i
   }
   b.has_inflow = (inflow_mask != nullptr);
   if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
-  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
+  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : real(0.0);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(double), st);
+  const cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(real), st);
   if (e != cudaSuccess) return (int)e;
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
-  const double rtol = newton_stop_rtol(params->newton_rtol);
+  const real rtol = newton_stop_rtol(params->newton_rtol);
   if (params->ghost == 2)
     patch_gather_speed_kernel<2><<<npg, 256, 0, st>>>(patches, cons_in, nx, ny, nz, b, inflow_mask, rtol,
                                                       params->newton_max_iter, d_max_speed);
@@ -418,24 +418,24 @@ extern "C" int srhd_patch_gather_speed(const double* patches, double* cons_in, i
 }
 
 template <int G, int RS>
-static void launch_prepass(const double* patches, double* patches_out, double* cons_in, double* flux_out, int nx,
-                           int ny, int nz, const GridBC& b, const unsigned char* mask, double rtol, int max_iter,
-                           double* umax_out, srhd_stats* stats, unsigned char* handled, cudaStream_t st) {
+static void launch_prepass(const real* patches, real* patches_out, real* cons_in, real* flux_out, int nx,
+                           int ny, int nz, const GridBC& b, const unsigned char* mask, real rtol, int max_iter,
+                           real* umax_out, srhd_stats* stats, unsigned char* handled, cudaStream_t st) {
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
   patch_prepass_kernel<G, RS><<<npg, 256, 0, st>>>(patches, patches_out, cons_in, flux_out, nx, ny, nz, b, mask, rtol,
                                                    max_iter, umax_out, stats, handled);
 }
 
-extern "C" int srhd_grid_step_cfl(const double* patches_in, double* patches_out, double* cons_in, double* flux_out,
+extern "C" int srhd_grid_step_cfl(const real* patches_in, real* patches_out, real* cons_in, real* flux_out,
                                   int nx, int ny, int nz, const int* bc, const unsigned char* inflow_mask,
                                   const double* inflow_cons, double cfl, double dh, double min_speed,
-                                  const srhd_params* params, srhd_stats* stats, double* d_max_speed, void* stream) {
+                                  const srhd_params* params, srhd_stats* stats, real* d_max_speed, void* stream) {
   if (!patches_in || !patches_out || !cons_in || !bc || !d_max_speed) return SRHD_ERR_NULL_POINTER;
   const int pc = check_params(params);
   if (pc) return pc;
   const int ce = check_extents(nx, ny, nz);
   if (ce) return ce;
-  if (!(cfl > 0.0) || !std::isfinite(cfl) || !(min_speed >= 0.0) || !(dh > 0.0) || !std::isfinite(dh))
+  if (!(cfl > real(0.0)) || !std::isfinite(cfl) || !(min_speed >= real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dh))
     return SRHD_ERR_BAD_STEP;
   if (patches_in == patches_out) return SRHD_ERR_ALIAS;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -454,8 +454,8 @@ extern "C" int srhd_grid_step_cfl(const double* patches_in, double* patches_out,
   }
   b.has_inflow = (inflow_mask != nullptr);
   if (b.has_inflow && !inflow_cons) return SRHD_ERR_NULL_POINTER;
-  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : 0.0;
-  cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(double), st);
+  for (int q = 0; q < 5; ++q) b.inflow[q] = b.has_inflow ? inflow_cons[q] : real(0.0);
+  cudaError_t e = cudaMemsetAsync(d_max_speed, 0, sizeof(real), st);
   if (e != cudaSuccess) return (int)e;
   if (stats) {
     e = cudaMemsetAsync(stats, 0, sizeof(srhd_stats), st);
@@ -464,7 +464,7 @@ extern "C" int srhd_grid_step_cfl(const double* patches_in, double* patches_out,
   unsigned char* handled = nullptr;
   e = cudaMallocAsync(reinterpret_cast<void**>(&handled), (size_t)npg, st);
   if (e != cudaSuccess) return (int)e;
-  const double rtol = newton_stop_rtol(params->newton_rtol);
+  const real rtol = newton_stop_rtol(params->newton_rtol);
   const int mi = params->newton_max_iter;
   if (params->recon == SRHD_RECON_PLM) {
     if (params->riemann == SRHD_RIEMANN_HLLE)
@@ -481,7 +481,7 @@ extern "C" int srhd_grid_step_cfl(const double* patches_in, double* patches_out,
   e = cudaGetLastError();
   int rc = (int)e;
   if (e == cudaSuccess)
-    rc = fluid_march(cons_in, patches_out, flux_out, npg, 1.0, dh, params, stats, st, d_max_speed, cfl, min_speed, handled);
+    rc = fluid_march(cons_in, patches_out, flux_out, npg, real(1.0), dh, params, stats, st, d_max_speed, cfl, min_speed, handled);
   const cudaError_t e2 = cudaFreeAsync(handled, st);
   return rc ? rc : (int)e2;
 }
@@ -490,9 +490,9 @@ extern "C" void srhd_default_params(srhd_params* p, int recon, int riemann) {
   if (!p) return;
   p->recon = recon;
   p->riemann = riemann;
-  p->minmod_coeff = 1.5;
+  p->minmod_coeff = real(1.5);
   p->max_retry = 8;
-  p->newton_rtol = 1e-15;
+  p->newton_rtol = SRHD_IS_F32 ? 1e-6 : 1e-15;   // a few eps_machine of the build's precision
   p->newton_max_iter = 20;
   p->ghost = (recon == SRHD_RECON_PLM) ? 2 : 3;
   p->integrator = SRHD_INTEGRATOR_MHM;
@@ -530,6 +530,12 @@ extern "C" const char* srhd_build_variant(void) {
 #else
          "total"
 #endif
+         " precision="
+#if SRHD_IS_F32
+         "f32"
+#else
+         "f64"
+#endif
          " arithmetic="
 #if SRHD_EXACT
          "exact"
@@ -541,6 +547,7 @@ extern "C" const char* srhd_build_variant(void) {
       ;
 }
 
+// SRHD_F64_ONLY_BEGIN (measurement helpers: double precision in every build)
 // ---- fp64 ALU roof: register-only DFMA loop, 8 independent chains per thread, 8 CTAs x 256 threads
 // per SM (full occupancy).  Used by bench.py for the MEASURED denominator of the "alu" roofline.
 namespace srhd {
@@ -620,3 +627,5 @@ extern "C" int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long lon
   if (flops) *flops = 2ull * 32ull * (unsigned long long)iters * (unsigned long long)grid * block;
   return (int)cudaGetLastError();
 }
+
+// SRHD_F64_ONLY_END

@@ -14,14 +14,14 @@ namespace srhd {
 
 struct UniformResult {
   int it0, it1;       // Newton-Raphson iterations of C2P(U0) and C2P(U1)
-  double umax;        // Eq. 26 of W0
-  double F[3][5];     // the Riemann flux of (U1, U1) along x, y, z
+  real umax;        // Eq. 26 of W0
+  real F[3][5];     // the Riemann flux of (U1, U1) along x, y, z
 };
 
 // every thread of the CTA calls this with the same U0 (the warp votes inside cons2prim_multi need whole warps)
 template <int RS>
-SRHD_DEV bool uniform_eval(const double U0in[5], double rtol, int max_iter, UniformResult& r) {
-  double U0[1][5], W0[1][5], U1[1][5], W1[1][5];
+SRHD_DEV bool uniform_eval(const real U0in[5], real rtol, int max_iter, UniformResult& r) {
+  real U0[1][5], W0[1][5], U1[1][5], W1[1][5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) U0[0][q] = U0in[q];
   bool ph0[1], ph1[1];
@@ -35,7 +35,7 @@ SRHD_DEV bool uniform_eval(const double U0in[5], double rtol, int max_iter, Unif
   for (int d = 0; d < 3; ++d) {
     riemann_flux<RS>(d, W1[0], U1[0], a1[0], W1[0], U1[0], a1[0], r.F[d], true);
 #pragma unroll
-    for (int q = 0; q < 5; ++q) ok = ok && (fabs(r.F[d][q]) <= DBL_MAX);
+    for (int q = 0; q < 5; ++q) ok = ok && (fabs(r.F[d][q]) <= kRealMax);
   }
   r.it0 = it0[0];
   r.it1 = it1[0];
@@ -45,18 +45,18 @@ SRHD_DEV bool uniform_eval(const double U0in[5], double rtol, int max_iter, Unif
 
 // the 8 patches of the group (out[patch][component][512]) and, if asked for, the patch-boundary fluxes
 // (fout[patch][face][component][64]); NT threads, thread tid
-SRHD_DEV void uniform_write(double* __restrict__ out, double* __restrict__ fout, const double U0[5],
+SRHD_DEV void uniform_write(real* __restrict__ out, real* __restrict__ fout, const real U0[5],
                             const UniformResult& r, int tid, int NT) {
-  double2* __restrict__ o2 = reinterpret_cast<double2*>(out);
+  real2* __restrict__ o2 = reinterpret_cast<real2*>(out);
   for (int w = tid; w < 8 * 5 * 256; w += NT) {
     const int q = (w >> 8) % 5;
-    const double u = (q == 0) ? U0[0] : (q == 1) ? U0[1] : (q == 2) ? U0[2] : (q == 3) ? U0[3] : U0[4];
-    o2[w] = make_double2(u, u);
+    const real u = (q == 0) ? U0[0] : (q == 1) ? U0[1] : (q == 2) ? U0[2] : (q == 3) ? U0[3] : U0[4];
+    o2[w] = make_real2(u, u);
   }
   if (fout) {
     for (int w = tid; w < 8 * 6 * 5 * 64; w += NT) {
       const int q = (w >> 6) % 5, d = ((w / 320) % 6) >> 1;
-      double f = 0.0;
+      real f = real(0.0);
 #pragma unroll
       for (int dd = 0; dd < 3; ++dd)
 #pragma unroll
@@ -80,8 +80,8 @@ SRHD_DEV void uniform_count(srhd_stats* __restrict__ stats, int tile_cells, cons
 }
 
 // srhd_fluid.cu: the march alone, for patch groups whose handled[] byte is 0 (the caller ran a pre-pass)
-int fluid_march(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-                const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-                double min_speed, const unsigned char* handled);
+int fluid_march(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt, real dh,
+                const srhd_params* p, srhd_stats* stats, cudaStream_t st, const real* d_smax, real cfl,
+                real min_speed, const unsigned char* handled);
 
 }  // namespace srhd

@@ -17,41 +17,41 @@ namespace srhd {
 constexpr int kVlThreads = 256;
 
 // by-products of a conversion that the production-build solver wants, recomputed from primitives
-SRHD_DEV Aux aux_of_prim(const double W[5]) {
+SRHD_DEV Aux aux_of_prim(const real W[5]) {
   Aux a;
 #if SRHD_GENERIC
-  a.ht = a.T = a.rg = 0.0;
+  a.ht = a.T = a.rg = real(0.0);
 #else
   a.T = W[4] * rcp_f(W[0]);
-  const double a2 = 2.25 * a.T * a.T, a1 = a2 + 1.0;
-  a.ht = fma(a2, rcp_f(1.0 + a1 * rsqrt_f(a1)), 2.5 * a.T);     // Eq. 22
-  a.rg = rsqrt_f(1.0 + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
+  const real a2 = real(2.25) * a.T * a.T, a1 = a2 + real(1.0);
+  a.ht = fma(a2, rcp_f(real(1.0) + a1 * rsqrt_f(a1)), real(2.5) * a.T);     // Eq. 22
+  a.rg = rsqrt_f(real(1.0) + (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]));
 #endif
   return a;
 }
 
 struct VlScratch {
-  double* Wc;                 // [npg][5][T3] primitives of the tile
-  double* Wh;                 // [npg][5][T3] primitives of the half-step state (predictor cells only)
+  real* Wc;                 // [npg][5][T3] primitives of the tile
+  real* Wh;                 // [npg][5][T3] primitives of the half-step state (predictor cells only)
   unsigned long long* umax;   // bit pattern of max U_max over the interior input cells
 };
 
 template <int G>
-__global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const double* __restrict__ cons_in, VlScratch s,
-                                                               long long ncell, double rtol, int max_iter,
+__global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const real* __restrict__ cons_in, VlScratch s,
+                                                               long long ncell, real rtol, int max_iter,
                                                                srhd_stats* __restrict__ stats) {
   constexpr int NXT = 16 + 2 * G, PL = NXT * NXT, T3 = PL * NXT;
   const unsigned lane = threadIdx.x & 31u;
   const long long step = (long long)gridDim.x * blockDim.x;
   unsigned long long iters = 0, fail = 0;
-  double umax = 0.0;
+  real umax = real(0.0);
   for (long long i0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; i0 - lane < ncell; i0 += step) {
     const bool valid = i0 < ncell;
     const long long i = valid ? i0 : ncell - 1;
     const long long pg = i / T3;
     const int c = (int)(i - pg * T3);
-    const double* t = cons_in + pg * 5 * T3 + c;
-    double U[1][5], W[1][5];
+    const real* t = cons_in + pg * 5 * T3 + c;
+    real U[1][5], W[1][5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) U[0][q] = __ldg(t + (size_t)q * T3);
     bool phys[1];
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const double* __r
     Aux aux[1];
     cons2prim_multi<1>(U, W, aux, rtol, max_iter, phys, it);
     if (valid) {
-      double* w = s.Wc + pg * 5 * T3 + c;
+      real* w = s.Wc + pg * 5 * T3 + c;
 #pragma unroll
       for (int q = 0; q < 5; ++q) w[(size_t)q * T3] = W[0][q];
       iters += (unsigned)it[0];
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const double* __r
   fail = warp_sum(fail);
   umax = warp_max(umax);
   if (lane == 0) {
-    atomicMax(s.umax, (unsigned long long)__double_as_longlong(umax));
+    atomicMax(s.umax, real_bits(umax));
     if (stats) {
       atomicAdd(&stats->newton_iters, iters);
       atomicAdd(&stats->exec_newton, iters);
@@ -86,10 +86,10 @@ __global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const double* __r
 
 // first-order flux through the face between tile cells cl and cl + stride_d (centre states)
 template <int G, int RS>
-SRHD_DEV void flux1(const double* __restrict__ t, const double* __restrict__ w, int d, int cl, double F[5]) {
+SRHD_DEV void flux1(const real* __restrict__ t, const real* __restrict__ w, int d, int cl, real F[5]) {
   constexpr int NXT = 16 + 2 * G, T3 = NXT * NXT * NXT;
   const int cr = cl + ((d == 0) ? 1 : ((d == 1) ? NXT : NXT * NXT));
-  double UL[5], UR[5], WL[5], WR[5];
+  real UL[5], UR[5], WL[5], WR[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
     UL[q] = __ldg(t + (size_t)q * T3 + cl);
@@ -101,14 +101,14 @@ SRHD_DEV void flux1(const double* __restrict__ t, const double* __restrict__ w, 
 }
 
 template <int G, int RS>
-__global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const double* __restrict__ cons_in, VlScratch s,
-                                                                  long long ncell, double dt, double dh, double rtol,
+__global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const real* __restrict__ cons_in, VlScratch s,
+                                                                  long long ncell, real dt, real dh, real rtol,
                                                                   int max_iter, srhd_stats* __restrict__ stats,
-                                                                  const double* __restrict__ d_smax, double cfl,
-                                                                  double min_speed) {
+                                                                  const real* __restrict__ d_smax, real cfl,
+                                                                  real min_speed) {
   constexpr int NXT = 16 + 2 * G, PL = NXT * NXT, T3 = PL * NXT, E = NXT - 2, E3 = E * E * E;
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);        // Eq. 28 on the device
-  const double hdt = dt / (2.0 * dh);
+  const real hdt = dt / (real(2.0) * dh);
   const unsigned lane = threadIdx.x & 31u;
   const long long step = (long long)gridDim.x * blockDim.x;
   unsigned long long iters = 0, fail = 0;
@@ -118,13 +118,13 @@ __global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const double* 
     const long long pg = i / E3;
     const int e = (int)(i - pg * E3);
     const int c = ((e / (E * E)) + 1) * PL + (((e / E) % E) + 1) * NXT + (e % E) + 1;   // one layer in from the rim
-    const double* t = cons_in + pg * 5 * T3;
-    const double* w = s.Wc + pg * 5 * T3;
-    double Uh[1][5], W[1][5], df[3][5];
+    const real* t = cons_in + pg * 5 * T3;
+    const real* w = s.Wc + pg * 5 * T3;
+    real Uh[1][5], W[1][5], df[3][5];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       const int st = (d == 0) ? 1 : ((d == 1) ? NXT : PL);
-      double Fm[5], Fp[5];
+      real Fm[5], Fp[5];
       flux1<G, RS>(t, w, d, c - st, Fm);
       flux1<G, RS>(t, w, d, c, Fp);
 #pragma unroll
@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const double* 
     Aux aux[1];
     cons2prim_multi<1>(Uh, W, aux, rtol, max_iter, phys, it);
     if (valid) {
-      double* wh = s.Wh + pg * 5 * T3 + c;
+      real* wh = s.Wh + pg * 5 * T3 + c;
 #pragma unroll
       for (int q = 0; q < 5; ++q) wh[(size_t)q * T3] = W[0][q];
       iters += (unsigned)it[0];
@@ -159,57 +159,57 @@ __global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const double* 
 
 // edge primitives of tile cell c along d from the half-step primitives, and their conserved form
 template <int G>
-SRHD_DEV void edges_of(const double* __restrict__ wh, int c, int st, double beta, double beta0, double Wm[5],
-                       double Wp[5]) {
+SRHD_DEV void edges_of(const real* __restrict__ wh, int c, int st, real beta, real beta0, real Wm[5],
+                       real Wp[5]) {
   constexpr int NXT = 16 + 2 * G, T3 = NXT * NXT * NXT;
   constexpr bool PPM = (G == 4);
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
-    const double* p = wh + (size_t)q * T3 + c;
+    const real* p = wh + (size_t)q * T3 + c;
     if (PPM) {
-      const double a[5] = {p[-2 * st], p[-st], p[0], p[st], p[2 * st]};
+      const real a[5] = {p[-2 * st], p[-st], p[0], p[st], p[2 * st]};
       recon_ppm(a, beta, beta0, Wm[q], Wp[q]);
     } else {
-      const double a[3] = {p[-st], p[0], p[st]};
+      const real a[3] = {p[-st], p[0], p[st]};
       recon_plm(a, beta, Wm[q], Wp[q]);
     }
   }
 }
 
 template <int G, int RS>
-__global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const double* __restrict__ cons_in,
-                                                                  double* __restrict__ cons_out,
-                                                                  double* __restrict__ flux_out, VlScratch s, double dt,
-                                                                  double dh, double beta0, int max_retry,
+__global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const real* __restrict__ cons_in,
+                                                                  real* __restrict__ cons_out,
+                                                                  real* __restrict__ flux_out, VlScratch s, real dt,
+                                                                  real dh, real beta0, int max_retry,
                                                                   srhd_stats* __restrict__ stats,
-                                                                  const double* __restrict__ d_smax, double cfl,
-                                                                  double min_speed) {
+                                                                  const real* __restrict__ d_smax, real cfl,
+                                                                  real min_speed) {
   constexpr int NXT = 16 + 2 * G, PL = NXT * NXT, T3 = PL * NXT;
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);
-  const double dtdh = dt / dh;
+  const real dtdh = dt / dh;
   const long long pg = blockIdx.x;
-  const double* t = cons_in + pg * 5 * T3;
-  const double* wh = s.Wh + pg * 5 * T3;
-  double* out = cons_out + pg * 8 * 5 * 512;
-  double* fout = flux_out ? flux_out + pg * 8 * 6 * 5 * 64 : nullptr;
-  double beta = beta0;
+  const real* t = cons_in + pg * 5 * T3;
+  const real* wh = s.Wh + pg * 5 * T3;
+  real* out = cons_out + pg * 8 * 5 * 512;
+  real* fout = flux_out ? flux_out + pg * 8 * 6 * 5 * 64 : nullptr;
+  real beta = beta0;
   int pass = 0, nfail = 0;
   unsigned ex_riemann = 0, ex_edges = 0;
   for (;; ++pass) {
-    if (pass > 0) beta = (pass <= max_retry) ? beta * 0.75 : 0.0;
+    if (pass > 0) beta = (pass <= max_retry) ? beta * real(0.75) : real(0.0);
     int my_fail = 0;
     for (int cell = threadIdx.x; cell < 4096; cell += kVlThreads) {
       const int i = cell & 15, j = (cell >> 4) & 15, k = cell >> 8;
       const int c = (k + G) * PL + (j + G) * NXT + (i + G);
-      double dfs[3][5];
+      real dfs[3][5];
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
         const int st = (d == 0) ? 1 : ((d == 1) ? NXT : PL);
-        double Wm0[5], Wp0[5], Wmm[5], Wpm[5], Wmp[5], Wpp[5];
+        real Wm0[5], Wp0[5], Wmm[5], Wpm[5], Wmp[5], Wpp[5];
         edges_of<G>(wh, c, st, beta, beta0, Wm0, Wp0);           // this cell
         edges_of<G>(wh, c - st, st, beta, beta0, Wmm, Wpm);      // lower neighbour: its plus edge is used
         edges_of<G>(wh, c + st, st, beta, beta0, Wmp, Wpp);      // upper neighbour: its minus edge is used
-        double UL[5], UR[5], Flo[5], Fhi[5];
+        real UL[5], UR[5], Flo[5], Fhi[5];
         Aux aL, aR;
         prim2cons_aux(Wpm, UL, aL);
         prim2cons_aux(Wm0, UR, aR);
@@ -236,8 +236,8 @@ __global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const double* 
         }
       }
       const int p = (i >> 3) + 2 * (j >> 3) + 4 * (k >> 3);       // S13
-      double* o = out + (size_t)p * 5 * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7);
-      double Un[5];
+      real* o = out + (size_t)p * 5 * 512 + (k & 7) * 64 + (j & 7) * 8 + (i & 7);
+      real Un[5];
 #pragma unroll
       for (int q = 0; q < 5; ++q) {
         Un[q] = __ldg(t + (size_t)q * T3 + c) - dtdh * ((dfs[0][q] + dfs[1][q]) + dfs[2][q]);   // S12
@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const double* 
     }
     nfail = __syncthreads_count(my_fail != 0) ? 1 : 0;
     // the count of failing CELLS of the accepted pass is needed only when the ladder ends here
-    if (nfail == 0 || beta == 0.0) {
+    if (nfail == 0 || beta == real(0.0)) {
       const unsigned long long tot = warp_sum((unsigned long long)my_fail);
       if ((threadIdx.x & 31) == 0 && tot && stats) atomicAdd(&stats->n_unphys_final, tot);
       break;
@@ -266,26 +266,26 @@ __global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const double* 
 
 __global__ void vl_finish_kernel(VlScratch s, srhd_stats* stats) {
   if (!stats) return;
-  const double umax = __longlong_as_double((long long)*s.umax);
+  const real umax = bits_real((rbits)*s.umax);
   atomic_max_nonneg(&stats->max_speed, smax_of_umax(umax));      // Eq. 27 (monotone: max first, convert once)
 }
 
 template <int G, int RS>
-int launch_vl(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-              const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-              double min_speed) {
+int launch_vl(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt, real dh,
+              const srhd_params* p, srhd_stats* stats, cudaStream_t st, const real* d_smax, real cfl,
+              real min_speed) {
   constexpr int NXT = 16 + 2 * G, T3 = NXT * NXT * NXT, E = NXT - 2;
   const int chunk = npg < 4096 ? npg : 4096;                      // bounds the scratch: 2 x 4096 x 5 x T3 doubles
   const size_t tile = (size_t)5 * T3;
-  double* buf = nullptr;
-  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf), (2 * (size_t)chunk * tile + 2) * sizeof(double), st);
+  real* buf = nullptr;
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf), (2 * (size_t)chunk * tile + 2) * sizeof(real), st);
   if (e != cudaSuccess) return (int)e;
   VlScratch s{buf, buf + (size_t)chunk * tile, reinterpret_cast<unsigned long long*>(buf + 2 * (size_t)chunk * tile)};
   e = cudaMemsetAsync(s.umax, 0, sizeof(unsigned long long), st);
-  const double rtol = newton_stop_rtol(p->newton_rtol);
+  const real rtol = newton_stop_rtol(p->newton_rtol);
   for (int g0 = 0; g0 < npg && e == cudaSuccess; g0 += chunk) {
     const int n = (npg - g0 < chunk) ? npg - g0 : chunk;
-    const double* in = cons_in + (size_t)g0 * tile;
+    const real* in = cons_in + (size_t)g0 * tile;
     const long long nc = (long long)n * T3, ne = (long long)n * E * E * E;
     const int gc = (int)((nc + kVlThreads - 1) / kVlThreads), ge = (int)((ne + kVlThreads - 1) / kVlThreads);
     const int cap = kNumSMs * 8 * 4;
@@ -306,9 +306,9 @@ int launch_vl(const double* cons_in, double* cons_out, double* flux_out, int npg
 }
 
 // called by srhd_fluid.cu's dispatcher (arguments already validated, stats already zeroed)
-int vl_step(const double* cons_in, double* cons_out, double* flux_out, int npg, double dt, double dh,
-            const srhd_params* p, srhd_stats* stats, cudaStream_t st, const double* d_smax, double cfl,
-            double min_speed) {
+int vl_step(const real* cons_in, real* cons_out, real* flux_out, int npg, real dt, real dh,
+            const srhd_params* p, srhd_stats* stats, cudaStream_t st, const real* d_smax, real cfl,
+            real min_speed) {
   if (p->recon == SRHD_RECON_PLM) {
     return p->riemann == SRHD_RIEMANN_HLLE
                ? launch_vl<3, 0>(cons_in, cons_out, flux_out, npg, dt, dh, p, stats, st, d_smax, cfl, min_speed)
@@ -322,7 +322,7 @@ int vl_step(const double* cons_in, double* cons_out, double* flux_out, int npg, 
 size_t vl_workspace_bytes(int npg, const srhd_params* p) {
   const int nxt = 16 + 2 * p->ghost;
   const size_t chunk = npg < 4096 ? (size_t)(npg > 0 ? npg : 0) : 4096;
-  return (2 * chunk * 5 * nxt * nxt * nxt + 2) * sizeof(double);
+  return (2 * chunk * 5 * nxt * nxt * nxt + 2) * sizeof(real);
 }
 
 }  // namespace srhd

@@ -39,7 +39,8 @@ class GridStepper:
         self.npg = (nx // 16) * (ny // 16) * (nz // 16)
         self.ncell = nx * ny * nz
         nxt = 16 + 2 * self.par.ghost
-        f64 = dict(dtype=torch.float64, device=device)
+        B.load_library(exact)
+        f64 = dict(dtype=B._CUR_REAL, device=device)   # srhd_real of the selected library (float32 for the f32 builds)
         self._grid = torch.empty((5, nz, ny, nx), **f64)
         self.tiles = torch.empty((self.npg, 5, nxt, nxt, nxt), **f64)
         self.patches = torch.empty((self.npg, 8, 5, 8, 8, 8), **f64)
@@ -77,7 +78,7 @@ class GridStepper:
     def set_prim(self, prim):
         """Upload a primitive field (5,nz,ny,nx) (numpy or CUDA tensor) and convert with srhd_prim2cons."""
         p = prim if isinstance(prim, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(prim))
-        p = p.to(self._grid.device).reshape(5, -1).contiguous()
+        p = p.to(self._grid.device, dtype=self._grid.dtype).reshape(5, -1).contiguous()
         B.prim2cons(p, cons=self._grid.view(5, -1), exact=self.exact)
         self._in_patches = self._grid_stale = False
         return self

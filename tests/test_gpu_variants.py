@@ -18,12 +18,14 @@ PAIRS = [("gamma53_exact", "gamma53"), ("gamma43_exact", "gamma43"), ("orig_exac
 
 
 def test_variant_strings():
-    want = {False: "eos=taub-mathews energy=reduced arithmetic=production",
-            True: "eos=taub-mathews energy=reduced arithmetic=exact",
-            "gamma53": "eos=gamma-5/3 energy=reduced arithmetic=generic",
-            "gamma53_exact": "eos=gamma-5/3 energy=reduced arithmetic=exact",
-            "gamma43_exact": "eos=gamma-4/3 energy=reduced arithmetic=exact",
-            "orig_exact": "eos=taub-mathews energy=total arithmetic=exact"}
+    want = {False: "eos=taub-mathews energy=reduced precision=f64 arithmetic=production",
+            True: "eos=taub-mathews energy=reduced precision=f64 arithmetic=exact",
+            "gamma53": "eos=gamma-5/3 energy=reduced precision=f64 arithmetic=generic",
+            "gamma53_exact": "eos=gamma-5/3 energy=reduced precision=f64 arithmetic=exact",
+            "gamma43_exact": "eos=gamma-4/3 energy=reduced precision=f64 arithmetic=exact",
+            "orig_exact": "eos=taub-mathews energy=total precision=f64 arithmetic=exact",
+            "f32": "eos=taub-mathews energy=reduced precision=f32 arithmetic=generic",
+            "f32_exact": "eos=taub-mathews energy=reduced precision=f32 arithmetic=exact"}
     for k, v in want.items():
         assert B.load_library(k).srhd_build_variant().decode() == v
 
@@ -154,3 +156,71 @@ def test_fig3_on_the_gpu(ref, T0):
         for e in orig:
             assert 1e-7 < e < 2e-5, orig                                # "roughly equal to a constant of 2e-6"
         assert orig[1] > 0.3 * orig[0] and orig[1] > 100 * new[1]
+
+
+# ------------------------------------------------------------------ single precision
+EPS32 = float(np.finfo(np.float32).eps)
+
+
+def test_f32_exact_build_is_bit_identical_to_the_f32_oracle(ref):
+    lib = "f32_exact"
+    W = wl.conversion_states(n=1 << 15, log_rho=(-3, 3), log_theta=(-6, 3), log_gamma=(0, 1.5))
+    with ref.variant("f32"):
+        po = ref.params("plm", "hllc", newton_rtol=1e-6)
+        U = ref.prim2cons(W)
+        W2, st = ref.cons2prim(U, po)
+        smax = ref.max_signal_speed(U, po)
+        tiles = make_tiles(ref, 4, po.ghost, seed=41)
+        dt = cfl_dt(ref, tiles, 1.0 / 64)
+        want, wflux, stw = ref.fluid_step_fluxes(tiles, dt, 1.0 / 64, po)
+        pq = ref.params("ppm", "hlle", newton_rtol=1e-6, max_retry=3)
+        rough = make_tiles(ref, 3, pq.ghost, seed=5, umax=8.0, rough=3.0, log_theta=(-4.0, 1.0))
+        dt3 = 4.0 * cfl_dt(ref, rough, 1.0 / 64)
+        want3, st3 = ref.fluid_step(rough, dt3, 1.0 / 64, pq)
+    assert tiles.dtype == np.float32 and want.dtype == np.float32
+    par = B.params("plm", "hllc", exact=lib)
+    assert par.newton_rtol == 1e-6
+    dU = B.prim2cons(dev(W.astype(np.float32)), exact=lib)
+    assert dU.dtype == torch.float32 and np.array_equal(dU.cpu().numpy(), U, equal_nan=True)
+    dW, sbuf = B.cons2prim(dev(U), par, exact=lib)
+    assert np.array_equal(dW.cpu().numpy(), W2, equal_nan=True)
+    s = B.stats_to_host(sbuf)
+    assert (s.n_c2p_fail, s.newton_iters) == (st.n_c2p_fail, st.newton_iters)
+    assert float(B.max_signal_speed(dev(U), par, exact=lib).cpu()) == smax
+    got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, 1.0 / 64, par, exact=lib)
+    assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+    assert np.array_equal(gflux.cpu().numpy(), wflux, equal_nan=True)
+    assert B.stats_to_host(sbuf).algorithm_dict() == stw.as_dict()
+    assert st3.n_retry_pg > 0
+    got3, sbuf3 = B.fluid_step(dev(rough), dt3, 1.0 / 64, B.params("ppm", "hlle", max_retry=3, exact=lib), exact=lib)
+    assert np.array_equal(got3.cpu().numpy(), want3, equal_nan=True)
+    assert B.stats_to_host(sbuf3).algorithm_dict() == st3.as_dict()
+    with pytest.raises(B.SrhdError):                     # a float64 tensor is refused by the f32 library
+        B.prim2cons(dev(W), exact=lib)
+
+
+def test_f32_grid_run_bit_identical_and_fma_build_close(ref):
+    """12 steps of a strong shock tube piece with uniform patch groups; dt from the oracle's CFL reduction is handed
+    to both sides (reading S16).  The FMA-contracted f32 build stays within a few single-precision ulps per step."""
+    prim, dh, bc = wl.shock_tube(n_long=64, n_trans=32, left=(1.0, 0.0, 10.0), right=(1.0, 0.0, 1e-2))
+    shape = prim.shape[1:]
+    st = GridStepper(shape, dh, bc, "plm", "hllc", cfl=0.5, exact="f32_exact").set_prim(prim)
+    sf = GridStepper(shape, dh, bc, "plm", "hllc", cfl=0.5, exact="f32").set_prim(prim)
+    with ref.variant("f32"):
+        po = ref.params("plm", "hllc", newton_rtol=1e-6)
+        cons = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+        for _ in range(12):
+            dt = ref.cfl_dt(cons, 0.5, dh, po)
+            cons, _ = ref.grid_step_tiled(cons, dt, dh, po, bc)
+            st.advance(dt)
+            sf.advance(dt)
+    assert st.grid.dtype == torch.float32
+    assert np.array_equal(st.grid.cpu().numpy(), cons)
+    g = sf.grid.cpu().numpy().astype(np.float64)
+    scale = np.abs(cons).reshape(5, -1).max(1).astype(np.float64)
+    scale[1:4] = float((np.sqrt((cons[1:4].astype(np.float64) ** 2).sum(0)) + np.abs(cons[4])).max())   # S14: one scale for M
+    assert (np.abs(g - cons) / scale[:, None, None, None]).max() <= 12 * 64 * EPS32
+    # and the fused no-host-sync step of the f32 library runs (dt formed on the device in single precision)
+    sf.step_async()
+    torch.cuda.synchronize()
+    assert 0 < sf.last_stats().n_uniform_pg < sf.npg and bool(torch.isfinite(sf.grid).all())
