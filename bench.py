@@ -295,7 +295,7 @@ def ncu_traffic(workload):
         return None
 
 
-def time_workload(name, steps, warmup, scale, world, local, rank, from_start=False, e2e_steps=0, fused=True):
+def time_workload(name, steps, warmup, scale, world, local, rank, from_start=False, e2e_steps=0, fused=True, lib=False):
     """Time `steps` steps of one workload after `warmup` untimed ones (from_start: the config's own run from
     its initial condition, warm-up on a second instance).  Returns a dict of measured figures."""
     import torch
@@ -310,9 +310,10 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
     st_inflow = None
     if inflow is not None:
         mask, prim_jet = inflow
-        cj = B.prim2cons(torch.from_numpy(prim_jet.reshape(5, 1).copy()).cuda()).cpu().numpy().ravel()
+        B.load_library(lib)
+        cj = B.prim2cons(torch.from_numpy(prim_jet.reshape(5, 1).copy()).cuda().to(B._CUR_REAL), exact=lib).cpu().numpy().ravel()
         st_inflow = (mask, cj)
-    st = GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=st_inflow, fused=fused)
+    st = GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=st_inflow, fused=fused, exact=lib)
     prim_d = torch.from_numpy(prim).cuda() if from_start else None
     st.set_prim(prim if prim_d is None else prim_d)
     del prim
@@ -371,7 +372,8 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
         "exec_riemann_per_cell": tot["exec_riemann"] / (ncell * steps),
         "state_mb": st.grid.numel() * 8 / 1e6, "tiles_mb": st.tiles.numel() * 8 / 1e6,
         "launches_per_step": st.launches_per_step,
-        "hbm_gbs": ncell * 80.0 / (ms_max / steps * 1e-3) / 1e9,      # algorithmic 80 B per cell update / step time
+        # algorithmic bytes per cell update (5 reals in, 5 out) / step time
+        "hbm_gbs": ncell * 10.0 * st.patches.element_size() / (ms_max / steps * 1e-3) / 1e9,
     }
     if e2e_steps:
         # end to end through the public API: every step copies its input grid from pinned host memory, runs
@@ -380,12 +382,12 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
         # buffers, own CUDA stream) are in flight round-robin so one instance's PCIe copies overlap another's
         # kernels: the figure is aggregate throughput over independent instances, the latency of one step of
         # one instance is about n_pipe times longer.
-        nbytes = st.grid.numel() * 8
+        nbytes = st.grid.numel() * st.grid.element_size()
         n_pipe = 3 if nbytes * 5 < 20e9 else 1
-        inst = [st] + [GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=st_inflow) for _ in range(n_pipe - 1)]
+        inst = [st] + [GridStepper(shape, dh, bc, recon, riemann, cfl=cfl, inflow=st_inflow, exact=lib) for _ in range(n_pipe - 1)]
         streams = [torch.cuda.Stream() for _ in range(n_pipe)]
-        h_in = [torch.empty(st.grid.shape, dtype=torch.float64, pin_memory=True) for _ in range(n_pipe)]
-        h_out = [torch.empty(st.grid.shape, dtype=torch.float64, pin_memory=True) for _ in range(n_pipe)]
+        h_in = [torch.empty(st.grid.shape, dtype=st.grid.dtype, pin_memory=True) for _ in range(n_pipe)]
+        h_out = [torch.empty(st.grid.shape, dtype=st.grid.dtype, pin_memory=True) for _ in range(n_pipe)]
         for h in h_in:
             h.copy_(st.grid)
         n_e2e = max(n_pipe, e2e_steps // n_pipe * n_pipe)
@@ -478,20 +480,21 @@ def run_ours(args):
     B.load_library()
 
     # ---- headline: K steps of the chosen workload after W warm-up steps, then end to end
+    lib = {"production": False, "exact": True}.get(args.lib, args.lib)
     head = time_workload(args.workload, args.steps, args.warmup, args.scale, world, local, rank,
-                         e2e_steps=0 if args.no_e2e else min(args.steps, 6))
+                         e2e_steps=0 if args.no_e2e else min(args.steps, 6), lib=lib)
     # ---- every 3-D config over its OWN step count from its initial condition (seconds of GPU time)
     per = {}
     if args.per_workload and world == 1:
         for name in ("blast256", "random512", "jet"):
             per[name] = time_workload(name, max(1, CONFIG_STEPS[name] // (args.scale if args.scale > 1 else 1)), 3,
-                                      args.scale, world, local, rank, from_start=True)
+                                      args.scale, world, local, rank, from_start=True, lib=lib)
     # the roofline kernel (fluid_step_kernel, general path) timed on its own: the same random512 run through the two
     # separate calls, so that the CUDA events bracket srhd_fluid_step_cfl alone and not the ghost-zone fill with it
     gen = None
     if args.per_workload and world == 1:
         gen = time_workload("random512", max(1, CONFIG_STEPS["random512"] // (args.scale if args.scale > 1 else 1)), 3,
-                            args.scale, world, local, rank, from_start=True, fused=False)
+                            args.scale, world, local, rank, from_start=True, fused=False, lib=lib)
     if world > 1:
         dist.barrier()
     if rank != 0:
@@ -522,8 +525,9 @@ def run_ours(args):
     out = {
         "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "what": head["desc"], "grid": head["shape"], "patch_groups": head["npg"],
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32" if "f32" in str(args.lib) else "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "library": B.load_library(lib).srhd_build_variant().decode(),
+                   "what": head["desc"], "grid": head["shape"], "patch_groups": head["npg"],
                    "scheme": f'{head["recon"]}+{head["riemann"]}', "cfl": head["cfl"],
                    "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": f'inputs larger than L2 ({head["state_mb"]:.0f} MB state, {head["tiles_mb"]:.0f} MB tiles)'
@@ -556,6 +560,9 @@ def main():
     ap.add_argument("--no-per-workload", dest="per_workload", action="store_false",
                     help="skip the runs of blast256 / random512 / jet over their own step counts")
     ap.add_argument("--scale", type=int, default=1, help="divide the grid extents (debugging only; 1 = the config)")
+    ap.add_argument("--lib", default="production",
+                    help="which in-tree library to time: production (default), exact, or a variant of "
+                         "paper_2012_11130_b200/build.py (gamma53, f32, ...); the headline is the production library")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

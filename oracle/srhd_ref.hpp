@@ -13,10 +13,14 @@
 //   conserved U = (D, M^x, M^y, M^z, Etilde) -- REDUCED energy Etilde = E - D (Eq. 6)
 // SoA convention of the C entry points: component c of state i at ptr[c*stride + i].
 //
-// Pin status (see tests/test_oracle_*.py and DESIGN.md "Oracle pins"):
-//   EoS, prim2cons, cons2prim, max speed, HLLE/HLLC, PLM/PPM, fluid step: pinned.
-//   Retry ladder (K, beta0, granularity = patch group; S3/S9) and the PPM/limiter details (S3/S4):
-//   "parity unpinned" against the paper -- the paper is silent; pinned only by textbook properties.
+// Pin status (tests/test_oracle_*.py): EoS, prim2cons, cons2prim, max speed (incl. the
+// relativistic factors of Eq. 26), wave speeds and their differences, HLLE/HLLC values, PLM/PPM properties, the
+// fluid step (3-D diagonal wave of section 4.1, 40-digit one-step evaluation), the retry ladder (Python re-assembly of
+// a pass; beta = 0 == first-order Godunov), the VL integrator, the coarse-fine hooks, the refinement flags and the
+// variants (polytropic EoS, original scheme, single precision): pinned; tests/mutants.py checks that one-line
+// mistakes in any of them fail a pin.  The values K, beta0 and the per-patch-group granularity of the ladder are
+// readings (S3, S9); the PPM / limiter DETAILS (PPM is named by BASELINE.json only; S3, S4) are "parity unpinned"
+// against the paper -- pinned by textbook properties only.
 #pragma once
 #include <cstddef>
 
