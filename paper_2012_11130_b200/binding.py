@@ -160,6 +160,36 @@ def _stream():
     return torch.cuda.current_stream().cuda_stream
 
 
+def _tiles(cons_in, par):
+    """Validate the ghosted tiles handed to a tile-consuming call: (npg,5,nxt,nxt,nxt), nxt = 16 + 2*par.ghost
+    (the C ABI sees only a pointer; a PLM-shaped tile with PPM parameters would be read out of bounds)."""
+    cons_in = _dev(cons_in, "cons_in")
+    nxt = 16 + 2 * par.ghost
+    if cons_in.dim() != 5 or tuple(cons_in.shape[1:]) != (5, nxt, nxt, nxt):
+        raise SrhdError(f"cons_in must have shape (npg,5,{nxt},{nxt},{nxt}) for ghost = {par.ghost}")
+    return cons_in, cons_in.shape[0]
+
+
+def _shaped(t, shape, name):
+    t = _dev(t, name)
+    if tuple(t.shape) != tuple(shape):
+        raise SrhdError(f"{name} must have shape {tuple(shape)}, not {tuple(t.shape)}")
+    return t
+
+
+def _inflow(inflow, ny, nx):
+    """(mask pointer, 5 doubles) of a fixed-inflow boundary, validated: uint8 CUDA mask of shape (ny,nx)."""
+    if inflow is None:
+        return None, None
+    mask, vals = inflow
+    if not (isinstance(mask, torch.Tensor) and mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous()
+            and tuple(mask.shape) == (ny, nx)):
+        raise SrhdError(f"inflow mask must be a contiguous uint8 CUDA tensor of shape ({ny},{nx})")
+    if len(vals) != 5:
+        raise SrhdError("inflow state must have 5 components")
+    return mask.data_ptr(), (C.c_double * 5)(*[float(v) for v in vals])
+
+
 def new_stats(device="cuda"):
     """Device buffer holding one srhd_stats (40 bytes)."""
     return torch.zeros(C.sizeof(Stats), dtype=torch.uint8, device=device)
@@ -209,15 +239,11 @@ def max_signal_speed(cons, par=None, out=None, exact=False):
 def fluid_step(cons_in, dt, dh, par, cons_out=None, stats=None, exact=False):
     """srhd_fluid_step: cons_in (npg,5,nxt,nxt,nxt) -> cons_out (npg,8,5,8,8,8); returns (cons_out, stats)."""
     L = load_library(exact)
-    cons_in = _dev(cons_in, "cons_in")
-    npg = cons_in.shape[0]
-    nxt = 16 + 2 * par.ghost
-    if tuple(cons_in.shape) != (npg, 5, nxt, nxt, nxt):
-        raise SrhdError(f"cons_in must have shape (npg,5,{nxt},{nxt},{nxt})")
+    cons_in, npg = _tiles(cons_in, par)
     if cons_out is None:
         cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     stats = new_stats(cons_in.device) if stats is None else stats
-    _check(L.srhd_fluid_step(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(), npg, float(dt),
+    _check(L.srhd_fluid_step(cons_in.data_ptr(), _shaped(cons_out, (npg, 8, 5, 8, 8, 8), "cons_out").data_ptr(), npg, float(dt),
                              float(dh), C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, stats
 
@@ -225,15 +251,14 @@ def fluid_step(cons_in, dt, dh, par, cons_out=None, stats=None, exact=False):
 def fluid_step_fluxes(cons_in, dt, dh, par, cons_out=None, flux_out=None, stats=None, exact=False):
     """srhd_fluid_step_fluxes: as fluid_step, plus the patch-boundary fluxes (npg,8,6,5,8,8)."""
     L = load_library(exact)
-    cons_in = _dev(cons_in, "cons_in")
-    npg = cons_in.shape[0]
+    cons_in, npg = _tiles(cons_in, par)
     if cons_out is None:
         cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     if flux_out is None:
         flux_out = torch.empty((npg, 8, 6, 5, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     stats = new_stats(cons_in.device) if stats is None else stats
-    _check(L.srhd_fluid_step_fluxes(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(),
-                                    _dev(flux_out, "flux_out").data_ptr(), npg, float(dt), float(dh),
+    _check(L.srhd_fluid_step_fluxes(cons_in.data_ptr(), _shaped(cons_out, (npg, 8, 5, 8, 8, 8), "cons_out").data_ptr(),
+                                    _shaped(flux_out, (npg, 8, 6, 5, 8, 8), "flux_out").data_ptr(), npg, float(dt), float(dh),
                                     C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, flux_out, stats
 
@@ -242,14 +267,13 @@ def fluid_step_cfl(cons_in, cfl, dh, max_speed, par, min_speed=0.0, cons_out=Non
                    exact=False):
     """srhd_fluid_step_cfl: dt = cfl*dh/max(*max_speed, min_speed) formed on the device (no host sync)."""
     L = load_library(exact)
-    cons_in = _dev(cons_in, "cons_in")
-    npg = cons_in.shape[0]
+    cons_in, npg = _tiles(cons_in, par)
     if cons_out is None:
         cons_out = torch.empty((npg, 8, 5, 8, 8, 8), dtype=cons_in.dtype, device=cons_in.device)
     stats = new_stats(cons_in.device) if stats is None else stats
-    _check(L.srhd_fluid_step_cfl(cons_in.data_ptr(), _dev(cons_out, "cons_out").data_ptr(),
-                                 0 if flux_out is None else _dev(flux_out, "flux_out").data_ptr(), npg,
-                                 float(cfl), float(dh), _dev(max_speed, "max_speed").data_ptr(), float(min_speed),
+    _check(L.srhd_fluid_step_cfl(cons_in.data_ptr(), _shaped(cons_out, (npg, 8, 5, 8, 8, 8), "cons_out").data_ptr(),
+                                 0 if flux_out is None else _shaped(flux_out, (npg, 8, 6, 5, 8, 8), "flux_out").data_ptr(), npg,
+                                 float(cfl), float(dh), _shaped(max_speed, (1,), "max_speed").data_ptr(), float(min_speed),
                                  C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, stats
 
@@ -260,10 +284,11 @@ REFINE_Q = {None: 0, "none": 0, "D": 1, "Etilde": 2, "rho": 3, "gamma": 4}
 def refine_flags(cons_in, par, quantity="rho", c_q=0.3, mom_over_d=0.0, flags=None, exact=False):
     """srhd_refine_flags: (npg,5,nxt,nxt,nxt) tiles -> (npg,8) uint8 patch flags."""
     L = load_library(exact)
-    cons_in = _dev(cons_in, "cons_in")
-    npg = cons_in.shape[0]
+    cons_in, npg = _tiles(cons_in, par)
     if flags is None:
         flags = torch.empty((npg, 8), dtype=torch.uint8, device=cons_in.device)
+    if not (flags.is_cuda and flags.dtype == torch.uint8 and flags.is_contiguous() and flags.numel() == npg * 8):
+        raise SrhdError(f"flags must be a contiguous uint8 CUDA tensor of {npg * 8} elements")
     q = REFINE_Q[quantity] if not isinstance(quantity, int) else quantity
     _check(L.srhd_refine_flags(cons_in.data_ptr(), npg, q, float(c_q), float(mom_over_d), C.byref(par),
                                flags.data_ptr(), _stream()), L)
@@ -316,13 +341,7 @@ def grid_gather(grid, ghost, bc, inflow=None, cons_in=None, exact=False):
     nxt = 16 + 2 * ghost
     if cons_in is None:
         cons_in = torch.empty((npg, 5, nxt, nxt, nxt), dtype=grid.dtype, device=grid.device)
-    mask_ptr, icons = None, None
-    if inflow is not None:
-        mask, vals = inflow
-        if not (mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous()):
-            raise SrhdError("inflow mask must be a contiguous uint8 CUDA tensor")
-        mask_ptr = mask.data_ptr()
-        icons = (C.c_double * 5)(*[float(v) for v in vals])
+    mask_ptr, icons = _inflow(inflow, ny, nx)
     _check(L.srhd_grid_gather(grid.data_ptr(), cons_in.data_ptr(), nx, ny, nz, ghost, _bc(bc), mask_ptr,
                               icons, _stream()), L)
     return cons_in
@@ -355,17 +374,16 @@ def grid_scatter_speed(cons_out, shape, par, grid=None, out=None, exact=False):
 def patch_gather_speed(patches, shape, par, bc, inflow=None, cons_in=None, out=None, exact=False):
     """srhd_patch_gather_speed: patches (npg,8,5,8,8,8) -> tiles (npg,5,nxt,nxt,nxt) and S_max (1 element)."""
     L = load_library(exact)
-    patches = _dev(patches, "patches")
     nz, ny, nx = shape
+    npg = (nx // 16) * (ny // 16) * (nz // 16)
+    patches = _shaped(patches, (npg, 8, 5, 8, 8, 8), "patches")
     nxt = 16 + 2 * par.ghost
+    if cons_in is not None:
+        cons_in = _shaped(cons_in, (npg, 5, nxt, nxt, nxt), "cons_in")
     if cons_in is None:
         cons_in = torch.empty((patches.shape[0], 5, nxt, nxt, nxt), dtype=patches.dtype, device=patches.device)
     out = torch.empty(1, dtype=patches.dtype, device=patches.device) if out is None else out
-    mask_ptr, icons = None, None
-    if inflow is not None:
-        mask, vals = inflow
-        mask_ptr = mask.data_ptr()
-        icons = (C.c_double * 5)(*[float(v) for v in vals])
+    mask_ptr, icons = _inflow(inflow, ny, nx)
     _check(L.srhd_patch_gather_speed(patches.data_ptr(), cons_in.data_ptr(), nx, ny, nz, _bc(bc), mask_ptr, icons,
                                      C.byref(par), out.data_ptr(), _stream()), L)
     return cons_in, out
@@ -388,11 +406,7 @@ def grid_step_cfl(patches_in, patches_out, cons_in, shape, cfl, dh, par, bc, inf
         raise SrhdError(f"flux_out must have shape ({npg}, 8, 6, 5, 8, 8)")
     out = torch.empty(1, dtype=patches_in.dtype, device=patches_in.device) if out is None else out
     stats = new_stats(patches_in.device) if stats is None else stats
-    mask_ptr, icons = None, None
-    if inflow is not None:
-        mask, vals = inflow
-        mask_ptr = mask.data_ptr()
-        icons = (C.c_double * 5)(*[float(v) for v in vals])
+    mask_ptr, icons = _inflow(inflow, ny, nx)
     _check(L.srhd_grid_step_cfl(patches_in.data_ptr(), patches_out.data_ptr(), cons_in.data_ptr(),
                                 None if flux_out is None else flux_out.data_ptr(), nx, ny, nz, _bc(bc), mask_ptr,
                                 icons, float(cfl), float(dh), float(min_speed), C.byref(par), stats.data_ptr(),

@@ -167,7 +167,7 @@ extern "C" int srhd_ghost_interp(const real* coarse, int nx, int ny, int nz, rea
   cudaError_t e = cudaMemsetAsync(d_n_fallback, 0, sizeof(unsigned long long), st);
   if (e != cudaSuccess) return (int)e;
   const long long ncell = (long long)(nx - 2) * (ny - 2) * (nz - 2);
-  const long long want = (ncell + 127) / 128, cap = (long long)kNumSMs * 16;
+  const long long want = (ncell + 127) / 128, cap = (long long)num_sms() * 16;
   ghost_interp_kernel<<<(int)(want < cap ? want : cap), 128, 0, st>>>(coarse, nx, ny, nz, fine, minmod_coeff,
                                                                      newton_stop_rtol(params->newton_rtol),
                                                                      params->newton_max_iter, fallback, d_n_fallback);

@@ -10,7 +10,17 @@
 
 namespace srhd {
 
-constexpr int kNumSMs = 148;   // B200: 2 dies x 74 SMs; grids are sized in multiples of this
+// SMs of the current device (B200: 2 dies x 74 = 148); grid-stride kernels size their grids in multiples of it
+inline int num_sms() {
+  static int n = 0;
+  if (n <= 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+      n = 148;
+  }
+  return n;
+}
 
 inline int check_params(const srhd_params* p) {
   if (!p) return SRHD_ERR_NULL_POINTER;

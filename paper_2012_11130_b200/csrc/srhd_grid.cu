@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const real* __r
 // and no tile is ever materialised.  Any other group gets its tile and the U_max of its 4096 cells exactly as
 // patch_gather_speed_kernel does it, and handled[pg] = 0 leaves it to fluid_step_kernel.
 template <int G, int RS>
-__global__ void __launch_bounds__(256) patch_prepass_kernel(const real* __restrict__ patches,
+__global__ void __launch_bounds__(256, 4) patch_prepass_kernel(const real* __restrict__ patches,
                                                             real* __restrict__ patches_out,
                                                             real* __restrict__ cons_in,
                                                             real* __restrict__ flux_out, int nx, int ny, int nz,
@@ -258,20 +258,27 @@ __global__ void __launch_bounds__(256) patch_prepass_kernel(const real* __restri
   real U0[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) U0[q] = __ldg(own + q * 512);
+  // the first 256 cells settle almost every group that is not uniform; then four cells (twenty loads) per thread
+  // in flight between two block-wide votes
   bool uniform = true;
-  for (int c0 = tid; c0 < t3; c0 += 2 * 256) {
-    real v[2][5];
+  {
+    real v[5];
+    tile_cell(tid, v);
     bool diff = false;
 #pragma unroll
-    for (int u = 0; u < 2; ++u) tile_cell(min(c0 + u * 256, t3 - 1), v[u]);
+    for (int q = 0; q < 5; ++q) diff = diff || (real_bits(v[q]) != real_bits(U0[q]));
+    if (__syncthreads_or(diff ? 1 : 0)) uniform = false;
+  }
+  for (int base = 256; uniform && base < t3; base += 4 * 256) {   // block-uniform trip count: every thread votes
+    real v[4][5];
+    bool diff = false;
 #pragma unroll
-    for (int u = 0; u < 2; ++u)
+    for (int u = 0; u < 4; ++u) tile_cell(min(base + u * 256 + tid, t3 - 1), v[u]);
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
 #pragma unroll
       for (int q = 0; q < 5; ++q) diff = diff || (real_bits(v[u][q]) != real_bits(U0[q]));
-    if (__syncthreads_or(diff ? 1 : 0)) {
-      uniform = false;
-      break;
-    }
+    if (__syncthreads_or(diff ? 1 : 0)) uniform = false;
   }
   if (uniform) {
     UniformResult r;
@@ -605,7 +612,7 @@ extern "C" int srhd_issue_probe(double* d_sink, int iters, int ffma_per_8_dfma, 
                                 void* stream) {
   if (!d_sink) return SRHD_ERR_NULL_POINTER;
   if (iters < 1) return SRHD_ERR_BAD_SIZE;
-  const int grid = srhd::kNumSMs * 8, block = 256;
+  const int grid = srhd::num_sms() * 8, block = 256;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   switch (ffma_per_8_dfma) {
     case 0: srhd::issue_probe_kernel<0><<<grid, block, 0, st>>>(d_sink, iters, 0.999999, 1e-6, 0.99999f, 1e-6f); break;
@@ -622,7 +629,7 @@ extern "C" int srhd_issue_probe(double* d_sink, int iters, int ffma_per_8_dfma, 
 extern "C" int srhd_fp64_peak_probe(double* d_sink, int iters, unsigned long long* flops, void* stream) {
   if (!d_sink) return SRHD_ERR_NULL_POINTER;
   if (iters < 1) return SRHD_ERR_BAD_SIZE;
-  const int grid = srhd::kNumSMs * 8, block = 256;
+  const int grid = srhd::num_sms() * 8, block = 256;
   srhd::fp64_peak_kernel<<<grid, block, 0, static_cast<cudaStream_t>(stream)>>>(d_sink, iters, 0.999999, 1e-6);
   if (flops) *flops = 2ull * 32ull * (unsigned long long)iters * (unsigned long long)grid * block;
   return (int)cudaGetLastError();

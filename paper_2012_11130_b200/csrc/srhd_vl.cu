@@ -288,7 +288,7 @@ int launch_vl(const real* cons_in, real* cons_out, real* flux_out, int npg, real
     const real* in = cons_in + (size_t)g0 * tile;
     const long long nc = (long long)n * T3, ne = (long long)n * E * E * E;
     const int gc = (int)((nc + kVlThreads - 1) / kVlThreads), ge = (int)((ne + kVlThreads - 1) / kVlThreads);
-    const int cap = kNumSMs * 8 * 4;
+    const int cap = num_sms() * 8 * 4;
     vl_centre_kernel<G><<<gc < cap ? gc : cap, kVlThreads, 0, st>>>(in, s, nc, rtol, p->newton_max_iter, stats);
     vl_predictor_kernel<G, RS><<<ge < cap ? ge : cap, kVlThreads, 0, st>>>(in, s, ne, dt, dh, rtol, p->newton_max_iter,
                                                                             stats, d_smax, cfl, min_speed);

@@ -134,6 +134,9 @@ class GridStepper:
         else:
             self._fill_tiles(need_speed=True)
             smax = max(float(self.smax.cpu()), self.smax_inflow)   # the one device->host double per step
+            if not (0.0 < smax <= 1.0):   # a NaN / vacuum state somewhere: the max-reduction cannot speak for it
+                raise B.SrhdError(f"signal speed {smax!r} is not in (0, 1]: the state holds non-finite or unphysical cells "
+                                  f"(srhd_stats of the last step: {self.last_stats().algorithm_dict()})")
         dt = self.cfl * self.dh / smax
         if t_end is not None and self.t + dt > t_end:
             dt = t_end - self.t
