@@ -30,7 +30,8 @@ VARIANTS = {
     "libsrhd_b200_gamma43_exact.so": _EXACT + _G43,
     "libsrhd_b200_orig_exact.so": _EXACT + ["-DSRHD_SCHEME=1"],
     # single precision throughout (srhd_real = float): the precision of every performance number in the paper
-    "libsrhd_b200_f32.so": ["-DSRHD_F32"],
+    # (the non-exact one with nvcc's fast single-precision division and square root: <= 2 ulp, no slow path)
+    "libsrhd_b200_f32.so": ["-DSRHD_F32", "-prec-div=false", "-prec-sqrt=false"],
     "libsrhd_b200_f32_exact.so": _EXACT + ["-DSRHD_F32"],
 }
 
