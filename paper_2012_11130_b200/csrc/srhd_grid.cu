@@ -202,6 +202,43 @@ __global__ void __launch_bounds__(256) patch_gather_speed_kernel(const real* __r
   if ((threadIdx.x & 31) == 0) atomic_max_nonneg(umax_out, umax);
 }
 
+// srhd_grid_step_cfl, kernel 0: own_uniform[pg] = 1 if the 8 patches of group pg (20480 contiguous values) hold ONE
+// state bit for bit -- a single coalesced pass over the state with 16-byte loads, dropped at the first 4 KB that
+// show a difference.  The pre-pass below then knows without reading any ghost cell that a tile is uniform
+// whenever the group and its 26 neighbours (after the boundary mapping) all carry this flag with the same state.
+__global__ void __launch_bounds__(256) patch_own_uniform_kernel(const real* __restrict__ patches,
+                                                               unsigned char* __restrict__ own_uniform) {
+  const int pg = blockIdx.x, tid = threadIdx.x;
+  const real* __restrict__ own = patches + (size_t)pg * 20480;
+  const real2* __restrict__ o2 = reinterpret_cast<const real2*>(own);
+  rbits ref[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) ref[q] = real_bits(__ldg(own + q * 512));
+  auto differs = [&](int w, real2 v) {                       // w: index of the pair; component = (w / 256) % 5
+    const int q = (w >> 8) % 5;
+    const rbits r = (q == 0) ? ref[0] : (q == 1) ? ref[1] : (q == 2) ? ref[2] : (q == 3) ? ref[3] : ref[4];
+    return (real_bits(v.x) != r) || (real_bits(v.y) != r);
+  };
+  bool uniform = true;
+  // pairs tid + 256 * (0, 1, 2, 3, 4): one of each component of patch 0
+  {
+    bool diff = false;
+#pragma unroll
+    for (int u = 0; u < 5; ++u) diff = diff || differs(tid + 256 * u, __ldg(o2 + tid + 256 * u));
+    if (__syncthreads_or(diff ? 1 : 0)) uniform = false;
+  }
+  for (int base = 5 * 256; uniform && base < 10240; base += 8 * 256) {   // 10240 pairs in all; block-uniform trip count
+    real2 v[8];
+    bool diff = false;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = __ldg(o2 + min(base + u * 256 + tid, 10239));
+#pragma unroll
+    for (int u = 0; u < 8; ++u) diff = diff || differs(min(base + u * 256 + tid, 10239), v[u]);
+    if (__syncthreads_or(diff ? 1 : 0)) uniform = false;
+  }
+  if (tid == 0) own_uniform[pg] = uniform ? 1 : 0;
+}
+
 // One whole step of a uniform grid kept in the patch layout, first kernel (srhd_grid_step_cfl): patch_gather_speed_kernel
 // with the uniform-tile test of srhd_uniform.cuh in front of it.  Phase 1 reads the (16+2g)^3 tile cells of the
 // group from the source patches WITHOUT writing them and compares them, as bit patterns, with the group's first
@@ -218,11 +255,12 @@ __global__ void __launch_bounds__(256, 4) patch_prepass_kernel(const real* __res
                                                             GridBC b, const unsigned char* __restrict__ mask,
                                                             real rtol, int max_iter, real* __restrict__ umax_out,
                                                             srhd_stats* __restrict__ stats,
-                                                            unsigned char* __restrict__ handled) {
+                                                            unsigned char* __restrict__ handled,
+                                                            const unsigned char* __restrict__ own_uniform) {
   constexpr int nxt = 16 + 2 * G, nrow = nxt * nxt, t3 = nrow * nxt;
   __shared__ int ax[nxt], ay[nxt], mx[nxt], my[nxt];
   __shared__ long long az[nxt];               // -1 - offset for a plane below z = 0 of an inflow boundary
-  const int px = nx / 16, py = ny / 16;
+  const int px = nx / 16, py = ny / 16, pz = nz / 16;
   const int pg = blockIdx.x, tid = threadIdx.x;
   const int gx = pg % px, gy = (pg / px) % py, gz = pg / (px * py);
   if (tid < nxt) {
@@ -258,10 +296,31 @@ __global__ void __launch_bounds__(256, 4) patch_prepass_kernel(const real* __res
   real U0[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) U0[q] = __ldg(own + q * 512);
+  // Shortcut that needs no ghost cell: the group and its 26 neighbours (periodic: wrapped; outflow: the group
+  // itself stands in for the missing neighbour, whose ghost cells copy this group's edge cells) each hold one state
+  // (patch_own_uniform_kernel) and it is the same state everywhere.  Fixed-inflow ghost cells below z = 0 hold
+  // another state, so the bottom layer of groups always takes the full test.
+  bool by_flags = false;
+  {
+    bool bad = false;
+    if (tid < 27) {
+      const int dx = tid % 3 - 1, dy = (tid / 3) % 3 - 1, dz = tid / 9 - 1;
+      int X = gx + dx, Y = gy + dy, Z = gz + dz;
+      X = (X < 0) ? (b.bc[0] == SRHD_BC_PERIODIC ? px - 1 : gx) : (X >= px) ? (b.bc[1] == SRHD_BC_PERIODIC ? 0 : gx) : X;
+      Y = (Y < 0) ? (b.bc[2] == SRHD_BC_PERIODIC ? py - 1 : gy) : (Y >= py) ? (b.bc[3] == SRHD_BC_PERIODIC ? 0 : gy) : Y;
+      Z = (Z < 0) ? (b.bc[4] == SRHD_BC_PERIODIC ? pz - 1 : gz) : (Z >= pz) ? (b.bc[5] == SRHD_BC_PERIODIC ? 0 : gz) : Z;
+      const int ng = X + px * (Y + py * Z);
+      bad = own_uniform[ng] == 0;
+      const real* __restrict__ nb = patches + (size_t)ng * 20480;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) bad = bad || (real_bits(__ldg(nb + q * 512)) != real_bits(U0[q]));
+    }
+    by_flags = !__syncthreads_or(bad ? 1 : 0) && !(b.has_inflow && gz == 0);
+  }
   // the first 256 cells settle almost every group that is not uniform; then four cells (twenty loads) per thread
   // in flight between two block-wide votes
   bool uniform = true;
-  {
+  if (!by_flags) {
     real v[5];
     tile_cell(tid, v);
     bool diff = false;
@@ -269,7 +328,7 @@ __global__ void __launch_bounds__(256, 4) patch_prepass_kernel(const real* __res
     for (int q = 0; q < 5; ++q) diff = diff || (real_bits(v[q]) != real_bits(U0[q]));
     if (__syncthreads_or(diff ? 1 : 0)) uniform = false;
   }
-  for (int base = 256; uniform && base < t3; base += 4 * 256) {   // block-uniform trip count: every thread votes
+  for (int base = 256; !by_flags && uniform && base < t3; base += 4 * 256) {   // block-uniform trip count: every thread votes
     real v[4][5];
     bool diff = false;
 #pragma unroll
@@ -429,8 +488,10 @@ static void launch_prepass(const real* patches, real* patches_out, real* cons_in
                            int ny, int nz, const GridBC& b, const unsigned char* mask, real rtol, int max_iter,
                            real* umax_out, srhd_stats* stats, unsigned char* handled, cudaStream_t st) {
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  unsigned char* own_uniform = handled + npg;                 // second half of the scratch allocation
+  patch_own_uniform_kernel<<<npg, 256, 0, st>>>(patches, own_uniform);
   patch_prepass_kernel<G, RS><<<npg, 256, 0, st>>>(patches, patches_out, cons_in, flux_out, nx, ny, nz, b, mask, rtol,
-                                                   max_iter, umax_out, stats, handled);
+                                                   max_iter, umax_out, stats, handled, own_uniform);
 }
 
 extern "C" int srhd_grid_step_cfl(const real* patches_in, real* patches_out, real* cons_in, real* flux_out,
@@ -469,7 +530,7 @@ extern "C" int srhd_grid_step_cfl(const real* patches_in, real* patches_out, rea
     if (e != cudaSuccess) return (int)e;
   }
   unsigned char* handled = nullptr;
-  e = cudaMallocAsync(reinterpret_cast<void**>(&handled), (size_t)npg, st);
+  e = cudaMallocAsync(reinterpret_cast<void**>(&handled), 2 * (size_t)npg, st);   // handled[npg] + own_uniform[npg]
   if (e != cudaSuccess) return (int)e;
   const real rtol = newton_stop_rtol(params->newton_rtol);
   const int mi = params->newton_max_iter;
