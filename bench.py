@@ -347,7 +347,8 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
     barrier()
     clocks = sampler.result()
     ms = ev0.elapsed_time(ev1)
-    k_ms = sum(a.elapsed_time(b) for a, b in kev) / len(kev)
+    k_each = [a.elapsed_time(b) for a, b in kev]
+    k_ms = sum(k_each) / len(k_each)
     for row in log.cpu():
         s = B.Stats.from_buffer_copy(row.numpy().tobytes())
         for k in tot:
@@ -372,6 +373,7 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
         "exec_riemann_per_cell": tot["exec_riemann"] / (ncell * steps),
         "state_mb": st.grid.numel() * 8 / 1e6, "tiles_mb": st.tiles.numel() * 8 / 1e6,
         "launches_per_step": st.launches_per_step,
+        "call_ms": {"min": min(k_each), "median": float(np.median(k_each)), "max": max(k_each)},
         # algorithmic bytes per cell update (5 reals in, 5 out) / step time
         "hbm_gbs": ncell * 10.0 * st.patches.element_size() / (ms_max / steps * 1e-3) / 1e9,
     }
@@ -450,7 +452,7 @@ def summary_of(r):
             "newton_iters_per_conversion": r["k_mean"], "passes_per_patch_group": r["passes_per_group"],
             "retry_patch_groups_per_step": r["retry_groups_per_step"], "unphysical_cells": r["unphysical_cells"],
             "uniform_patch_group_fraction": r["uniform_fraction"],
-            "step_hbm_gbs_algorithmic": r["hbm_gbs"],
+            "step_hbm_gbs_algorithmic": r["hbm_gbs"], "step_call_ms": r["call_ms"],
             "executed_conversions_per_cell": r["exec_conversions_per_cell"],
             "executed_riemann_solves_per_cell": r["exec_riemann_per_cell"],
             "sm_mhz": r["clocks"]["sm_mhz"], "throttle_reasons": r["clocks"]["reasons"]}
@@ -537,6 +539,7 @@ def run_ours(args):
                    "retry_patch_groups_per_step": head["retry_groups_per_step"],
                    "executed_conversions_per_cell": head["exec_conversions_per_cell"],
                    "uniform_patch_group_fraction": head["uniform_fraction"],
+                   "step_call_ms": head["call_ms"],
                    "per_workload": {k: summary_of(v) for k, v in per.items()}},
         "clocks": head["clocks"],
         "roofline": roof,

@@ -8,7 +8,7 @@ One step (collapsed onto the GPU):
                                                        with the CFL reduction of that state (Eq. 26-27)
     srhd_fluid_step_cfl(tiles) -> patches              the fused MUSCL-Hancock update with
                                                        dt = C dh / S_max formed on the device (Eq. 28)
-step_async() issues both behind ONE call, srhd_grid_step_cfl (3 launches, patches double buffered), whose first
+step_async() issues both behind ONE call, srhd_grid_step_cfl (4 launches, patches double buffered), whose first
 kernel also finishes the patch groups that hold a single state (their new patches are their old ones) without
 ever materialising their tiles; fused=False keeps the two separate calls (same results bit for bit).
 The first step after set_prim / set_cons starts from the grid instead: srhd_max_signal_speed +
@@ -62,9 +62,9 @@ class GridStepper:
         self.nstep = 0
         self._in_patches = False   # True: self.patches holds the current state (self._grid may be stale)
         self._grid_stale = False
-        # fused: pre-pass (ghost-zone fill + speed + uniform tiles), smax finish, march; else gather + speed, smax
-        # finish, uniform-tile scan, march
-        self.launches_per_step = 3 if self.fused else 4
+        # fused: own-uniform flags, pre-pass (ghost-zone fill + speed + uniform tiles), smax finish, march; else
+        # gather + speed, smax finish, uniform-tile scan, march
+        self.launches_per_step = 4
 
     # ---- state in / out -------------------------------------------------------------------------
     @property
