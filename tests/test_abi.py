@@ -13,7 +13,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def libs():
     from paper_2012_11130_b200 import build
     build.build()
-    return [C.CDLL(build.lib_path(False)), C.CDLL(build.lib_path(True))]
+    paths = [build.lib_path(False), build.lib_path(True)]
+    paths += [os.path.join(os.path.dirname(paths[0]), n) for n in build.VARIANTS if os.path.join(os.path.dirname(paths[0]), n) not in paths]
+    return [C.CDLL(p) for p in paths]     # production, exact, then every variant library
 
 
 def declared_symbols():
@@ -86,6 +88,19 @@ def test_argument_errors_without_gpu():
     bc = (C.c_int * 6)(0, 0, 0, 0, 0, 0)
     assert L.srhd_grid_gather(16, 32, 16, 24, 16, 2, bc, None, None, None) == -3
     assert L.srhd_grid_scatter(16, 32, 16, 16, 0, None) == -3
+    # the whole-step call: pointers, extents, Courant number, in == out
+    assert L.srhd_grid_step_cfl(None, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -1
+    assert L.srhd_grid_step_cfl(16, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, None, None) == -1
+    assert L.srhd_grid_step_cfl(16, 1 << 30, 1 << 31, None, 16, 24, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -3
+    assert L.srhd_grid_step_cfl(16, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.0, 1.0, 0.0, C.byref(p), None, 64, None) == -4
+    assert L.srhd_grid_step_cfl(16, 16, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -5
+    assert L.srhd_grid_step_cfl(16, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(bad), None, 64, None) == -2
+    # every variant library answers the same way and says what it is
+    for key in ("gamma53", "gamma53_exact", "gamma43_exact", "orig_exact", "f32", "f32_exact", True):
+        V = b.load_library(key)
+        assert V.srhd_prim2cons(None, None, 4, 4, None) == -1
+        assert b"eos=" in V.srhd_build_variant() and b"precision=" in V.srhd_build_variant()
+    b.load_library()
 
 
 def test_no_cpu_fallback():
