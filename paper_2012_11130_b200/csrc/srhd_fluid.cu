@@ -201,10 +201,10 @@ __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
   real U0[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) U0[q] = bits_real((rbits)ref[q]);
+  uniform_write_state(cons_out + (size_t)blockIdx.x * 8 * 5 * 512, U0, tid, NT);   // (rewritten by the march if the verdict is no)
   UniformResult r;
-  if (!uniform_eval<RS>(U0, rtol, max_iter, r)) return;      // every thread computed the same verdict
-  uniform_write(cons_out + (size_t)blockIdx.x * 8 * 5 * 512,
-                flux_out ? flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64 : nullptr, U0, r, tid, NT);
+  if (!uniform_eval_by_warp0<RS>(U0, rtol, max_iter, r)) return;      // block-uniform verdict
+  if (flux_out) uniform_write_flux(flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64, r, tid, NT);
   if (tid == 0) {
     handled[blockIdx.x] = 1;
     uniform_count(stats, T3, r);

@@ -340,10 +340,11 @@ __global__ void __launch_bounds__(256, 4) patch_prepass_kernel(const real* __res
     if (__syncthreads_or(diff ? 1 : 0)) uniform = false;
   }
   if (uniform) {
+    // the stores go out first (harmless if the group is marched after all), one warp evaluates the state meanwhile
+    uniform_write_state(patches_out + (size_t)pg * 8 * 5 * 512, U0, tid, 256);
     UniformResult r;
-    if (uniform_eval<RS>(U0, rtol, max_iter, r)) {           // every thread computed the same verdict
-      uniform_write(patches_out + (size_t)pg * 8 * 5 * 512,
-                    flux_out ? flux_out + (size_t)pg * 8 * 6 * 5 * 64 : nullptr, U0, r, tid, 256);
+    if (uniform_eval_by_warp0<RS>(U0, rtol, max_iter, r)) {   // block-uniform verdict
+      if (flux_out) uniform_write_flux(flux_out + (size_t)pg * 8 * 6 * 5 * 64, r, tid, 256);
       if (tid == 0) {
         handled[pg] = 1;
         uniform_count(stats, t3, r);

@@ -43,27 +43,45 @@ SRHD_DEV bool uniform_eval(const real U0in[5], real rtol, int max_iter, UniformR
   return ok;
 }
 
-// the 8 patches of the group (out[patch][component][512]) and, if asked for, the patch-boundary fluxes
-// (fout[patch][face][component][64]); NT threads, thread tid
-SRHD_DEV void uniform_write(real* __restrict__ out, real* __restrict__ fout, const real U0[5],
-                            const UniformResult& r, int tid, int NT) {
+// the 8 patches of the group, out[patch][component][512] = U0[component]; NT threads, thread tid.  It may be
+// issued BEFORE the verdict of uniform_eval is known: a group that is marched after all has every cell rewritten.
+SRHD_DEV void uniform_write_state(real* __restrict__ out, const real U0[5], int tid, int NT) {
   real2* __restrict__ o2 = reinterpret_cast<real2*>(out);
   for (int w = tid; w < 8 * 5 * 256; w += NT) {
     const int q = (w >> 8) % 5;
     const real u = (q == 0) ? U0[0] : (q == 1) ? U0[1] : (q == 2) ? U0[2] : (q == 3) ? U0[3] : U0[4];
     o2[w] = make_real2(u, u);
   }
-  if (fout) {
-    for (int w = tid; w < 8 * 6 * 5 * 64; w += NT) {
-      const int q = (w >> 6) % 5, d = ((w / 320) % 6) >> 1;
-      real f = real(0.0);
+}
+// the patch-boundary fluxes, fout[patch][face][component][64] = F[face >> 1][component]
+SRHD_DEV void uniform_write_flux(real* __restrict__ fout, const UniformResult& r, int tid, int NT) {
+  for (int w = tid; w < 8 * 6 * 5 * 64; w += NT) {
+    const int q = (w >> 6) % 5, d = ((w / 320) % 6) >> 1;
+    real f = real(0.0);
 #pragma unroll
-      for (int dd = 0; dd < 3; ++dd)
+    for (int dd = 0; dd < 3; ++dd)
 #pragma unroll
-        for (int qq = 0; qq < 5; ++qq) f = (dd == d && qq == q) ? r.F[dd][qq] : f;
-      fout[w] = f;
+      for (int qq = 0; qq < 5; ++qq) f = (dd == d && qq == q) ? r.F[dd][qq] : f;
+    fout[w] = f;
+  }
+}
+// One warp evaluates the uniform state while the others' stores are in flight; the verdict and the result go through
+// shared memory.  Block-uniform return value; every thread of the CTA must call it.
+template <int RS>
+SRHD_DEV bool uniform_eval_by_warp0(const real U0[5], real rtol, int max_iter, UniformResult& r) {
+  __shared__ UniformResult s_r;
+  __shared__ int s_ok;
+  if (threadIdx.x < 32) {
+    UniformResult t;
+    const bool ok = uniform_eval<RS>(U0, rtol, max_iter, t);
+    if (threadIdx.x == 0) {
+      s_r = t;
+      s_ok = ok ? 1 : 0;
     }
   }
+  __syncthreads();
+  r = s_r;
+  return s_ok != 0;
 }
 
 // what the march would have counted for this group (one thread); tile_cells = (16 + 2 ghost)^3
