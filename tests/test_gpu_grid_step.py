@@ -87,3 +87,32 @@ def test_fused_step_inflow_and_flux_output(ref):
                                         inflow, min_speed=st.smax_inflow, flux_out=flux_a)
     torch.cuda.synchronize()
     assert torch.equal(out_a, out_b) and torch.equal(flux_a, flux_b) and float(smax_a.cpu()) == float(smax.cpu())
+
+
+@pytest.mark.parametrize("name", ["blast256", "jet_half"])
+def test_fused_step_equals_two_calls_at_config_size(name):
+    """The launch configuration bench.py times (GridStepper.step_async -> srhd_grid_step_cfl, production library) against
+    the two separate calls on the blast wave at full size and on the jet at half size (nozzle, outflow): identical
+    patches, S_max and counters after every one of 24 steps, with both kinds of patch group present."""
+    from paper_2012_11130_b200 import workloads as wl
+    inflow = None
+    if name == "blast256":
+        prim, dh, bc = wl.blast_wave(n=256)
+    else:
+        prim, dh, bc, (mask, pj) = wl.jet(nx=256, ny=256, nz=512, radius=0.04)
+        cj = B.prim2cons(torch.from_numpy(pj.reshape(5, 1).copy()).cuda()).cpu().numpy().ravel()
+        inflow = (mask, cj)
+    shape = prim.shape[1:]
+    a = GridStepper(shape, dh, bc, "ppm", "hllc", cfl=0.4, inflow=inflow, fused=True).set_prim(prim)
+    b = GridStepper(shape, dh, bc, "ppm", "hllc", cfl=0.4, inflow=inflow, fused=False).set_prim(prim)
+    del prim
+    for step in range(24):
+        a.step_async()
+        b.step_async()
+        if step % 6 == 5 or step < 2:
+            torch.cuda.synchronize()
+            sa, sb = a.last_stats(), b.last_stats()
+            assert torch.equal(a.patches, b.patches), (name, step)
+            assert float(a.smax.cpu()) == float(b.smax.cpu())
+            assert sa.algorithm_dict() == sb.algorithm_dict() and sa.n_uniform_pg == sb.n_uniform_pg
+    assert 0 < sa.n_uniform_pg < a.npg and sa.n_uniform_pg > 0.8 * a.npg
