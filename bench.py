@@ -281,6 +281,73 @@ def run_conv(args):
     print(json.dumps(out))
 
 
+def run_aux(args):
+    """--aux: the entry points of SURVEY.md 8f (coarse-fine hooks, refinement flags, VL integrator), each timed with
+    CUDA events on blast-wave data after its blast has grown for 40 steps (256^3, PPM+HLLC tiles).  One JSON line;
+    not the headline metric."""
+    import torch
+    from paper_2012_11130_b200 import binding as B
+    from paper_2012_11130_b200 import build as cuda_build
+    from paper_2012_11130_b200.driver import GridStepper
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    cuda_build.build()
+    n = 256 // args.scale
+    prim, dh, bc, _ = make_workload("blast256", scale=args.scale)
+    st = GridStepper(prim.shape[1:], dh, bc, "ppm", "hllc", cfl=0.4).set_prim(prim)
+    for _ in range(40):
+        st.step_async()
+    grid = st.grid.clone()
+    par = st.par
+    tiles = B.grid_gather(grid, par.ghost, bc)
+    npg, ncell = st.npg, st.ncell
+    reps = max(args.steps, 3)
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    out = {}
+    out["refine_flags_D_ms"] = timed(lambda: B.refine_flags(tiles, par, "D", 0.3, 0.0))
+    out["refine_flags_rho_ms"] = timed(lambda: B.refine_flags(tiles, par, "rho", 0.3, 0.0))
+    out["refine_flags_gamma_and_momentum_ms"] = timed(lambda: B.refine_flags(tiles, par, "gamma", 0.3, 1.0))
+    # flux correction: both x faces of every patch, fine flux = coarse flux of the step (so nothing is skipped)
+    smax = B.max_signal_speed(grid.view(5, -1), par)
+    dt = 0.4 * dh / float(smax.cpu())
+    patches, flux, _ = B.fluid_step_fluxes(tiles, dt, dh, par)
+    p5 = patches.reshape(npg * 8, 5, 8, 8, 8).contiguous()
+    fp = torch.arange(npg * 8, dtype=torch.int32, device="cuda").repeat_interleave(2)
+    fi = torch.tensor([0, 1], dtype=torch.int32, device="cuda").repeat(npg * 8)
+    fc = flux.reshape(npg * 8, 6, 5, 8, 8)[:, :2].reshape(-1, 5, 8, 8).contiguous()
+    ff = (fc * 1.001).contiguous()
+    out["flux_correction_ms"] = timed(lambda: B.flux_correction(p5, fc, ff, fp, fi, dt, dh))
+    out["flux_correction_faces"] = int(fp.numel())
+    # ghost-zone interpolation of the central 130^3 block (128^3 coarse cells -> 256^3 fine cells)
+    c0 = n // 2 - min(65, n // 2 - 1)
+    w = min(130, n - 2 * c0)
+    coarse = grid[:, c0:c0 + w, c0:c0 + w, c0:c0 + w].contiguous()
+    out["ghost_interp_ms"] = timed(lambda: B.ghost_interp(coarse, 1.5, par))
+    out["ghost_interp_fine_cells"] = 8 * (w - 2) ** 3
+    # VL integrator on the same state (one more ghost layer)
+    vl = GridStepper(prim.shape[1:], dh, bc, "ppm", "hllc", cfl=0.4, integrator="vl").set_cons(grid)
+    vl.step_async()
+    out["vl_step_ms"] = timed(vl.step_async)
+    mh = GridStepper(prim.shape[1:], dh, bc, "ppm", "hllc", cfl=0.4, fused=False).set_cons(grid)
+    mh.step_async()
+    out["muscl_hancock_step_same_state_ms"] = timed(mh.step_async)
+    print(json.dumps({"aux": True, "what": f"SURVEY 8f entry points on the {n}^3 blast wave after 40 steps (PPM+HLLC tiles, "
+                      f"{npg} patch groups, {ncell} cells); milliseconds per call, CUDA events, {reps} repetitions",
+                      "data": "synthetic", "dtype": "f64", **out}))
+
+
 CONFIG_STEPS = {"blast256": 100, "random512": 50, "jet": 50, "tube": 205}   # BASELINE.json configs: their own step counts
 
 
@@ -566,10 +633,13 @@ def main():
     ap.add_argument("--lib", default="production",
                     help="which in-tree library to time: production (default), exact, or a variant of "
                          "paper_2012_11130_b200/build.py (gamma53, f32, ...); the headline is the production library")
+    ap.add_argument("--aux", action="store_true", help="time the SURVEY 8f entry points instead (one JSON line, not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.aux:
+        return run_aux(args)
     if args.impl == "reference":
         if args.workload == "conv":
             raise SystemExit("--impl reference times the fluid-step workloads only")

@@ -168,39 +168,13 @@ __global__ void __launch_bounds__(kScanThreads) uniform_tiles_kernel(
     real cfl, real min_speed, unsigned char* __restrict__ handled) {
   using P = Plan<G>;
   constexpr int NT = kScanThreads, T3 = P::T3;
-  constexpr int H = T3 / 2;                                  // 16-byte words per component
-  static_assert(T3 % 2 == 0, "tile components must be whole 16-byte words");
   const int tid = threadIdx.x;
   const real* __restrict__ tile = cons_in + (size_t)blockIdx.x * 5 * T3;
   if (tid == 0) handled[blockIdx.x] = 0;
-  const real2* __restrict__ t2 = reinterpret_cast<const real2*>(tile);
-  rbits ref[5];
-#pragma unroll
-  for (int q = 0; q < 5; ++q) ref[q] = real_bits(__ldg(tile + (size_t)q * T3));
-  auto differs = [&](int w, real2 v) {
-    const int q = w / H;
-    const rbits r = (q == 0) ? ref[0] : (q == 1) ? ref[1] : (q == 2) ? ref[2] : (q == 3) ? ref[3] : ref[4];
-    return (real_bits(v.x) != r) || (real_bits(v.y) != r);
-  };
-  if (__syncthreads_or(differs(tid, __ldg(t2 + tid)) ? 1 : 0)) return;      // the first 4 KB settle most tiles
-  for (int base = NT; base < 5 * H; base += 8 * NT) {
-    real2 v[8];
-    int w[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      w[u] = min(base + u * NT + tid, 5 * H - 1);
-      v[u] = __ldg(t2 + w[u]);
-    }
-    bool diff = false;
-#pragma unroll
-    for (int u = 0; u < 8; ++u) diff = diff || differs(w[u], v[u]);
-    if (__syncthreads_or(diff ? 1 : 0)) return;
-  }
+  real U0[5];
+  if (!tile_scan_uniform<T3, NT>(tile, U0)) return;
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);      // as the main kernel (srhd_fluid_step_cfl)
   if (!(fabs(dt / dh) <= kRealMax)) return;                   // U0 - (dt/dh) 0 = U0 needs a finite dt/dh
-  real U0[5];
-#pragma unroll
-  for (int q = 0; q < 5; ++q) U0[q] = bits_real((rbits)ref[q]);
   uniform_write_state(cons_out + (size_t)blockIdx.x * 8 * 5 * 512, U0, tid, NT);   // (rewritten by the march if the verdict is no)
   UniformResult r;
   if (!uniform_eval_by_warp0<RS>(U0, rtol, max_iter, r)) return;      // block-uniform verdict

@@ -43,6 +43,42 @@ SRHD_DEV bool uniform_eval(const real U0in[5], real rtol, int max_iter, UniformR
   return ok;
 }
 
+// Does the tile (5 components x T3 values, 16-byte aligned) hold ONE state?  It is streamed once with 16-byte
+// loads compared as bit patterns with the first cell (U0 receives it); a tile that is not uniform is dropped at
+// its first 4 KB.  NT threads per CTA, all of them call it; the return value is block uniform.
+template <int T3, int NT>
+SRHD_DEV bool tile_scan_uniform(const real* __restrict__ tile, real U0[5]) {
+  constexpr int H = T3 / 2;                                  // 16-byte words per component
+  static_assert(T3 % 2 == 0, "tile components must be whole 16-byte words");
+  const int tid = threadIdx.x;
+  const real2* __restrict__ t2 = reinterpret_cast<const real2*>(tile);
+  rbits ref[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) ref[q] = real_bits(__ldg(tile + (size_t)q * T3));
+  auto differs = [&](int w, real2 v) {
+    const int q = w / H;
+    const rbits r = (q == 0) ? ref[0] : (q == 1) ? ref[1] : (q == 2) ? ref[2] : (q == 3) ? ref[3] : ref[4];
+    return (real_bits(v.x) != r) || (real_bits(v.y) != r);
+  };
+  if (__syncthreads_or(differs(tid, __ldg(t2 + tid)) ? 1 : 0)) return false;   // the first 4 KB settle most tiles
+  for (int base = NT; base < 5 * H; base += 8 * NT) {
+    real2 v[8];
+    int w[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      w[u] = min(base + u * NT + tid, 5 * H - 1);
+      v[u] = __ldg(t2 + w[u]);
+    }
+    bool diff = false;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) diff = diff || differs(w[u], v[u]);
+    if (__syncthreads_or(diff ? 1 : 0)) return false;
+  }
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U0[q] = bits_real(ref[q]);
+  return true;
+}
+
 // the 8 patches of the group, out[patch][component][512] = U0[component]; NT threads, thread tid.  It may be
 // issued BEFORE the verdict of uniform_eval is known: a group that is marched after all has every cell rewritten.
 SRHD_DEV void uniform_write_state(real* __restrict__ out, const real U0[5], int tid, int NT) {

@@ -11,6 +11,7 @@
 // that share it (the solver is a function of its inputs, so both get the same bits).  It is the second
 // integrator of the paper at the same parity bar, not the tuned hot path.
 #include "srhd_common.cuh"
+#include "srhd_uniform.cuh"
 
 namespace srhd {
 
@@ -39,16 +40,18 @@ struct VlScratch {
 template <int G>
 __global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const real* __restrict__ cons_in, VlScratch s,
                                                                long long ncell, real rtol, int max_iter,
-                                                               srhd_stats* __restrict__ stats) {
+                                                               srhd_stats* __restrict__ stats,
+                                                               const unsigned char* __restrict__ handled) {
   constexpr int NXT = 16 + 2 * G, PL = NXT * NXT, T3 = PL * NXT;
   const unsigned lane = threadIdx.x & 31u;
   const long long step = (long long)gridDim.x * blockDim.x;
-  unsigned long long iters = 0, fail = 0;
+  unsigned long long iters = 0, fail = 0, done = 0;
   real umax = real(0.0);
   for (long long i0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; i0 - lane < ncell; i0 += step) {
-    const bool valid = i0 < ncell;
-    const long long i = valid ? i0 : ncell - 1;
+    const long long i = (i0 < ncell) ? i0 : ncell - 1;
     const long long pg = i / T3;
+    const bool valid = (i0 < ncell) && !handled[pg];          // groups the uniform pre-pass has finished are skipped
+    if (!__any_sync(0xffffffffu, valid)) continue;             // (whole warps: the conversion votes)
     const int c = (int)(i - pg * T3);
     const real* t = cons_in + pg * 5 * T3 + c;
     real U[1][5], W[1][5];
@@ -63,6 +66,7 @@ __global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const real* __res
 #pragma unroll
       for (int q = 0; q < 5; ++q) w[(size_t)q * T3] = W[0][q];
       iters += (unsigned)it[0];
+      ++done;
       const int ti = c % NXT, tj = (c / NXT) % NXT, tk = c / PL;
       if (ti >= G && ti < G + 16 && tj >= G && tj < G + 16 && tk >= G && tk < G + 16) {
         fail += phys[0] ? 0u : 1u;
@@ -72,16 +76,17 @@ __global__ void __launch_bounds__(kVlThreads) vl_centre_kernel(const real* __res
   }
   iters = warp_sum(iters);
   fail = warp_sum(fail);
+  done = warp_sum(done);
   umax = warp_max(umax);
   if (lane == 0) {
     atomicMax(s.umax, real_bits(umax));
     if (stats) {
       atomicAdd(&stats->newton_iters, iters);
       atomicAdd(&stats->exec_newton, iters);
+      atomicAdd(&stats->exec_c2p, done);
       if (fail) atomicAdd(&stats->n_c2p_fail, fail);
     }
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0 && stats) atomicAdd(&stats->exec_c2p, (unsigned long long)ncell);
 }
 
 // first-order flux through the face between tile cells cl and cl + stride_d (centre states)
@@ -105,17 +110,19 @@ __global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const real* __
                                                                   long long ncell, real dt, real dh, real rtol,
                                                                   int max_iter, srhd_stats* __restrict__ stats,
                                                                   const real* __restrict__ d_smax, real cfl,
-                                                                  real min_speed) {
+                                                                  real min_speed,
+                                                                  const unsigned char* __restrict__ handled) {
   constexpr int NXT = 16 + 2 * G, PL = NXT * NXT, T3 = PL * NXT, E = NXT - 2, E3 = E * E * E;
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);        // Eq. 28 on the device
   const real hdt = dt / (real(2.0) * dh);
   const unsigned lane = threadIdx.x & 31u;
   const long long step = (long long)gridDim.x * blockDim.x;
-  unsigned long long iters = 0, fail = 0;
+  unsigned long long iters = 0, fail = 0, done = 0;
   for (long long i0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; i0 - lane < ncell; i0 += step) {
-    const bool valid = i0 < ncell;
-    const long long i = valid ? i0 : ncell - 1;
+    const long long i = (i0 < ncell) ? i0 : ncell - 1;
     const long long pg = i / E3;
+    const bool valid = (i0 < ncell) && !handled[pg];
+    if (!__any_sync(0xffffffffu, valid)) continue;
     const int e = (int)(i - pg * E3);
     const int c = ((e / (E * E)) + 1) * PL + (((e / E) % E) + 1) * NXT + (e % E) + 1;   // one layer in from the rim
     const real* t = cons_in + pg * 5 * T3;
@@ -141,19 +148,19 @@ __global__ void __launch_bounds__(kVlThreads) vl_predictor_kernel(const real* __
 #pragma unroll
       for (int q = 0; q < 5; ++q) wh[(size_t)q * T3] = W[0][q];
       iters += (unsigned)it[0];
+      ++done;
       fail += phys[0] ? 0u : 1u;                               // S15 / S18: counted, no rung can cure it
     }
   }
   iters = warp_sum(iters);
   fail = warp_sum(fail);
+  done = warp_sum(done);
   if (lane == 0 && stats) {
     atomicAdd(&stats->newton_iters, iters);
     atomicAdd(&stats->exec_newton, iters);
+    atomicAdd(&stats->exec_c2p, done);
+    atomicAdd(&stats->exec_riemann, 6ull * done);
     if (fail) atomicAdd(&stats->n_c2p_fail, fail);
-  }
-  if (blockIdx.x == 0 && threadIdx.x == 0 && stats) {
-    atomicAdd(&stats->exec_c2p, (unsigned long long)ncell);
-    atomicAdd(&stats->exec_riemann, 6ull * (unsigned long long)ncell);
   }
 }
 
@@ -183,8 +190,10 @@ __global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const real* __
                                                                   real dh, real beta0, int max_retry,
                                                                   srhd_stats* __restrict__ stats,
                                                                   const real* __restrict__ d_smax, real cfl,
-                                                                  real min_speed) {
+                                                                  real min_speed,
+                                                                  const unsigned char* __restrict__ handled) {
   constexpr int NXT = 16 + 2 * G, PL = NXT * NXT, T3 = PL * NXT;
+  if (handled[blockIdx.x]) return;                               // a uniform tile: vl_uniform_tiles_kernel wrote its result
   if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);
   const real dtdh = dt / dh;
   const long long pg = blockIdx.x;
@@ -264,6 +273,76 @@ __global__ void __launch_bounds__(kVlThreads) vl_corrector_kernel(const real* __
   }
 }
 
+// Uniform tiles under the VL integrator (srhd_uniform.cuh; reading S18): W0 = C2P(U0) for every tile cell; the
+// first-order fluxes of equal neighbours cancel, so the predictor state is U0 again and its primitives are W0 (the
+// same conversion, the same bits); every edge state is (W0, U1 = P2C(W0)); every face solves F_d(W0, U1; W0, U1);
+// every update is U0 - dt/dh 0 = U0.  One CTA per group, ahead of the three VL kernels, which skip the groups it
+// has finished.
+template <int RS>
+SRHD_DEV bool uniform_eval_vl(const real U0in[5], real rtol, int max_iter, UniformResult& r) {
+  real U0[1][5], W0[1][5], U1[5], F1[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) U0[0][q] = U0in[q];
+  bool ph0[1];
+  int it0[1];
+  Aux a0[1], a1;
+  cons2prim_multi<1>(U0, W0, a0, rtol, max_iter, ph0, it0);
+  bool ok = ph0[0] && is_physical(U0[0]);
+  prim2cons_aux(W0[0], U1, a1);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    riemann_flux<RS>(d, W0[0], U0[0], aux_of_prim(W0[0]), W0[0], U0[0], aux_of_prim(W0[0]), F1);   // predictor fluxes: must be finite
+    riemann_flux<RS>(d, W0[0], U1, a1, W0[0], U1, a1, r.F[d]);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) ok = ok && (fabs(F1[q]) <= kRealMax) && (fabs(r.F[d][q]) <= kRealMax);
+  }
+  r.it0 = it0[0];
+  r.it1 = 0;
+  r.umax = umax_of_prim(W0[0], a0[0]);
+  return ok;
+}
+
+template <int G, int RS>
+__global__ void __launch_bounds__(kVlThreads) vl_uniform_tiles_kernel(
+    const real* __restrict__ cons_in, real* __restrict__ cons_out, real* __restrict__ flux_out, VlScratch s, real dt,
+    real dh, real rtol, int max_iter, srhd_stats* __restrict__ stats, const real* __restrict__ d_smax, real cfl,
+    real min_speed, unsigned char* __restrict__ handled) {
+  constexpr int NXT = 16 + 2 * G, T3 = NXT * NXT * NXT, E = NXT - 2;
+  const int tid = threadIdx.x;
+  if (tid == 0) handled[blockIdx.x] = 0;
+  real U0[5];
+  if (!tile_scan_uniform<T3, kVlThreads>(cons_in + (size_t)blockIdx.x * 5 * T3, U0)) return;
+  if (d_smax) dt = cfl * dh / fmax(*d_smax, min_speed);
+  if (!(fabs(dt / dh) <= kRealMax)) return;
+  uniform_write_state(cons_out + (size_t)blockIdx.x * 8 * 5 * 512, U0, tid, kVlThreads);
+  __shared__ UniformResult s_r;
+  __shared__ int s_ok;
+  if (tid < 32) {
+    UniformResult t;
+    const bool ok = uniform_eval_vl<RS>(U0, rtol, max_iter, t);
+    if (tid == 0) {
+      s_r = t;
+      s_ok = ok ? 1 : 0;
+    }
+  }
+  __syncthreads();
+  if (!s_ok) return;                                             // block uniform: left to the three VL kernels
+  if (flux_out) uniform_write_flux(flux_out + (size_t)blockIdx.x * 8 * 6 * 5 * 64, s_r, tid, kVlThreads);
+  if (tid == 0) {
+    handled[blockIdx.x] = 1;
+    atomicMax(s.umax, real_bits(s_r.umax));
+    if (stats) {
+      const unsigned long long it = (unsigned long long)(T3 + E * E * E) * (unsigned)s_r.it0;   // V1 + V3 conversions
+      atomicAdd(&stats->newton_iters, it);
+      atomicAdd(&stats->n_passes, 1ull);
+      atomicAdd(&stats->n_uniform_pg, 1ull);
+      atomicAdd(&stats->exec_newton, (unsigned long long)s_r.it0);
+      atomicAdd(&stats->exec_c2p, 1ull);
+      atomicAdd(&stats->exec_riemann, 6ull);
+    }
+  }
+}
+
 __global__ void vl_finish_kernel(VlScratch s, srhd_stats* stats) {
   if (!stats) return;
   const real umax = bits_real((rbits)*s.umax);
@@ -278,9 +357,12 @@ int launch_vl(const real* cons_in, real* cons_out, real* flux_out, int npg, real
   const int chunk = npg < 4096 ? npg : 4096;                      // bounds the scratch: 2 x 4096 x 5 x T3 doubles
   const size_t tile = (size_t)5 * T3;
   real* buf = nullptr;
-  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf), (2 * (size_t)chunk * tile + 2) * sizeof(real), st);
+  // two primitive tiles per group of a chunk, the U_max word, one flag byte per group of a chunk
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&buf),
+                                  (2 * (size_t)chunk * tile + 2) * sizeof(real) + 16 + (size_t)chunk, st);
   if (e != cudaSuccess) return (int)e;
   VlScratch s{buf, buf + (size_t)chunk * tile, reinterpret_cast<unsigned long long*>(buf + 2 * (size_t)chunk * tile)};
+  unsigned char* handled = reinterpret_cast<unsigned char*>(buf + 2 * (size_t)chunk * tile + 2) + 16;
   e = cudaMemsetAsync(s.umax, 0, sizeof(unsigned long long), st);
   const real rtol = newton_stop_rtol(p->newton_rtol);
   for (int g0 = 0; g0 < npg && e == cudaSuccess; g0 += chunk) {
@@ -289,12 +371,15 @@ int launch_vl(const real* cons_in, real* cons_out, real* flux_out, int npg, real
     const long long nc = (long long)n * T3, ne = (long long)n * E * E * E;
     const int gc = (int)((nc + kVlThreads - 1) / kVlThreads), ge = (int)((ne + kVlThreads - 1) / kVlThreads);
     const int cap = num_sms() * 8 * 4;
-    vl_centre_kernel<G><<<gc < cap ? gc : cap, kVlThreads, 0, st>>>(in, s, nc, rtol, p->newton_max_iter, stats);
+    real* const out = cons_out + (size_t)g0 * 8 * 5 * 512;
+    real* const fout = flux_out ? flux_out + (size_t)g0 * 8 * 6 * 5 * 64 : nullptr;
+    vl_uniform_tiles_kernel<G, RS><<<n, kVlThreads, 0, st>>>(in, out, fout, s, dt, dh, rtol, p->newton_max_iter, stats,
+                                                             d_smax, cfl, min_speed, handled);
+    vl_centre_kernel<G><<<gc < cap ? gc : cap, kVlThreads, 0, st>>>(in, s, nc, rtol, p->newton_max_iter, stats, handled);
     vl_predictor_kernel<G, RS><<<ge < cap ? ge : cap, kVlThreads, 0, st>>>(in, s, ne, dt, dh, rtol, p->newton_max_iter,
-                                                                            stats, d_smax, cfl, min_speed);
-    vl_corrector_kernel<G, RS><<<n, kVlThreads, 0, st>>>(in, cons_out + (size_t)g0 * 8 * 5 * 512,
-                                                         flux_out ? flux_out + (size_t)g0 * 8 * 6 * 5 * 64 : nullptr, s, dt,
-                                                         dh, p->minmod_coeff, p->max_retry, stats, d_smax, cfl, min_speed);
+                                                                            stats, d_smax, cfl, min_speed, handled);
+    vl_corrector_kernel<G, RS><<<n, kVlThreads, 0, st>>>(in, out, fout, s, dt, dh, p->minmod_coeff, p->max_retry, stats,
+                                                         d_smax, cfl, min_speed, handled);
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) {
@@ -322,7 +407,7 @@ int vl_step(const real* cons_in, real* cons_out, real* flux_out, int npg, real d
 size_t vl_workspace_bytes(int npg, const srhd_params* p) {
   const int nxt = 16 + 2 * p->ghost;
   const size_t chunk = npg < 4096 ? (size_t)(npg > 0 ? npg : 0) : 4096;
-  return (2 * chunk * 5 * nxt * nxt * nxt + 2) * sizeof(real);
+  return (2 * chunk * 5 * nxt * nxt * nxt + 2) * sizeof(real) + 16 + chunk;
 }
 
 }  // namespace srhd

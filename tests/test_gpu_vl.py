@@ -97,3 +97,36 @@ def test_vl_multi_step_on_the_grid_stepper(ref):
         b.step_async()
     torch.cuda.synchronize()
     assert torch.equal(a.grid, b.grid)
+
+
+@pytest.mark.parametrize("recon,riemann", [("plm", "hllc"), ("ppm", "hlle")])
+def test_vl_uniform_tile_path_parity(ref, recon, riemann):
+    """Tiles that hold ONE state take the VL uniform-tile pre-pass (srhd_stats.n_uniform_pg): output, patch-boundary
+    fluxes and every algorithm counter must be what the oracle's full VL step gives; tiles that differ from uniform in
+    one cell, and a uniform state that fails Eq. 30, go through the three VL kernels and must match too."""
+    po = ref.params(recon, riemann, integrator="vl")
+    nxt, dh = 16 + 2 * po.ghost, 1.0 / 64
+    states = np.array([[0.7, 3.0e2, -1.0e2, 5.0e1, 1e-4], [1.0, 0.0, 0.0, 0.0, 1e-6], [2.5e-3, -0.4, 0.3, 2.0, 40.0]])
+    cons = ref.prim2cons(states.T.copy())
+    npg = 6
+    tiles = np.empty((npg, 5, nxt, nxt, nxt))
+    for pg in range(npg):
+        tiles[pg] = cons[:, pg % 3][:, None, None, None]
+    tiles[3, 0, 0, 0, 0] *= 1.0 + 2.0 ** -52
+    tiles[4, 2, nxt // 2, nxt // 2, nxt // 2] += 1e-3
+    tiles[5, 4] = -1e-9                                           # uniform but unphysical
+    dt = 0.4 * dh
+    want, wflux, st = ref.fluid_step_fluxes(tiles, dt, dh, po)
+    pe = B.params(recon, riemann, exact=True, integrator="vl")
+    got, gflux, sbuf = B.fluid_step_fluxes(dev(tiles), dt, dh, pe, exact=True)
+    s = B.stats_to_host(sbuf)
+    assert s.n_uniform_pg == 3
+    assert np.array_equal(got.cpu().numpy(), want, equal_nan=True)
+    assert np.array_equal(gflux.cpu().numpy(), wflux, equal_nan=True)
+    assert s.algorithm_dict() == st.as_dict()
+    got, sbuf = B.fluid_step(dev(tiles), dt, dh, B.params(recon, riemann, integrator="vl"))
+    s = B.stats_to_host(sbuf)
+    got = got.cpu().numpy()
+    assert s.n_uniform_pg == 3 and np.array_equal(got[:3], want[:3])
+    assert step_err(got[:5], want[:5], 2).max() <= 1e-11
+    assert (s.n_retry_pg, s.n_passes) == (st.n_retry_pg, st.n_passes)
