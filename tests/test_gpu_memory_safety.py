@@ -98,3 +98,63 @@ def test_state_list_kernels_respect_their_bounds(ref):
             torch.cuda.synchronize()
             assert guards_intact(cbuf) and guards_intact(bbuf) and guards_intact(pbuf)
             assert bool(torch.isfinite(d_cons).all()) and bool(torch.isfinite(d_back).all()) and float(s.cpu()) > 0
+
+
+@pytest.mark.parametrize("recon,riemann", [("plm", "hlle"), ("ppm", "hllc")])
+def test_grid_step_guards_and_determinism(recon, riemann):
+    """srhd_grid_step_cfl (own-uniform flags, pre-pass, march) on a grid with both kinds of patch group: the two
+    patch buffers and the tile scratch sit between guard regions, the output is pre-filled with NaN, the tile scratch
+    of a uniform group must stay untouched, and 8 repetitions (every third with another kernel in flight on a second
+    stream) give the same bits.  The tile-based calls with the uniform-tile pre-pass (MUSCL-Hancock and VL) likewise."""
+    shape, dh, bc = (32, 32, 48), 1.0 / 32, ["periodic", "periodic", "outflow", "outflow", "periodic", "periodic"]
+    rng = np.random.default_rng(7)
+    prim = np.empty((5,) + shape)
+    prim[0], prim[1:4], prim[4] = 1.0, 0.0, 1e-6
+    prim[:, 4:12, 6:14, 20:30] = np.stack([0.5 + rng.random((8, 8, 10)), *rng.normal(0, 1.0, (3, 8, 8, 10)),
+                                           10.0 ** rng.uniform(-2, 1, (8, 8, 10))])
+    par = B.params(recon, riemann)
+    npg = (shape[0] // 16) * (shape[1] // 16) * (shape[2] // 16)
+    nxt = 16 + 2 * par.ghost
+    cons = B.prim2cons(torch.from_numpy(prim.reshape(5, -1)).cuda()).reshape(5, *shape).contiguous()
+    tiles0 = B.grid_gather(cons, par.ghost, bc)
+    smax = B.max_signal_speed(cons.view(5, -1), par)
+    p0, _ = B.fluid_step_cfl(tiles0, 0.4, dh, smax, par)              # a state in the patch layout to start from
+    ibuf, p_in = guarded((npg, 8, 5, 8, 8, 8))
+    ibuf[:GUARD] = float("nan")
+    ibuf[-GUARD:] = float("nan")
+    p_in.copy_(p0)
+    side = torch.cuda.Stream()
+    first = None
+    for rep in range(8):
+        obuf, p_out = guarded((npg, 8, 5, 8, 8, 8))
+        tbuf, tiles = guarded((npg, 5, nxt, nxt, nxt))
+        fbuf, flux = guarded((npg, 8, 6, 5, 8, 8))
+        if rep % 3 == 2:
+            with torch.cuda.stream(side):
+                B.cons2prim(cons.view(5, -1))
+        _, sm, stats = B.grid_step_cfl(p_in, p_out, tiles, shape, 0.4, dh, par, bc, flux_out=flux)
+        torch.cuda.synchronize()
+        s = B.stats_to_host(stats)
+        assert guards_intact(obuf) and guards_intact(tbuf) and guards_intact(fbuf)
+        assert torch.equal(p_in, p0)                                    # the input state is read only
+        assert not bool(torch.isnan(p_out).any()) and not bool(torch.isnan(flux).any())
+        assert 0 < s.n_uniform_pg < npg
+        written = ~torch.isnan(tiles).reshape(npg, -1).all(1)          # groups whose tile was materialised
+        assert int(written.sum()) == npg - s.n_uniform_pg
+        res = (p_out.clone(), flux.clone(), sm.clone())
+        if first is None:
+            first = res
+        else:
+            for a, b in zip(first, res):
+                assert torch.equal(a.view(torch.int64), b.view(torch.int64)), (recon, riemann, rep)
+    # tile-based calls on tiles that are partly uniform: MUSCL-Hancock and VL pre-passes
+    for integ in ("mhm", "vl"):
+        pv = B.params(recon, riemann, integrator=integ)
+        tl = B.grid_gather(cons, pv.ghost, bc)
+        obuf, out = guarded((npg, 8, 5, 8, 8, 8))
+        fbuf, flux = guarded((npg, 8, 6, 5, 8, 8))
+        _, _, stats = B.fluid_step_fluxes(tl, 0.1 * dh, dh, pv, cons_out=out, flux_out=flux)
+        torch.cuda.synchronize()
+        assert guards_intact(obuf) and guards_intact(fbuf)
+        assert not bool(torch.isnan(out).any()) and not bool(torch.isnan(flux).any())
+        assert 0 < B.stats_to_host(stats).n_uniform_pg < npg
