@@ -49,6 +49,7 @@ extern "C" {
 #define SRHD_ERR_BAD_STEP      (-4)   /* dt <= 0 or dh <= 0 (or not finite)                         */
 #define SRHD_ERR_ALIAS         (-5)   /* cons_in and cons_out overlap                               */
 #define SRHD_ERR_BAD_ALIGN     (-6)   /* cons_in not 16-byte aligned (TMA bulk copies need it)      */
+#define SRHD_ERR_TOO_LARGE     (-7)   /* srhd_fluid_step_noalloc: npg > SRHD_NOALLOC_MAX_NPG         */
 
 #define SRHD_RECON_PLM   0
 #define SRHD_RECON_PPM   1
@@ -204,6 +205,39 @@ int srhd_ghost_interp(const srhd_real* coarse, int nx, int ny, int nz, srhd_real
  * integrator the two primitive tiles its stages communicate through.  The call allocates and frees them itself
  * in stream order (cudaMallocAsync / cudaFreeAsync on `stream`): informational, nothing for the caller to provide. */
 size_t srhd_workspace_bytes(int npg, const srhd_params* params);
+
+/* srhd_fluid_step for callers that must not allocate.
+ *
+ * Who this is for: srhd_fluid_step obtains its one-byte-per-group flag array (srhd_workspace_bytes) with
+ * cudaMallocAsync / cudaFreeAsync.  Some hosts of this library cannot afford that: a simulation code whose own
+ * allocator already owns every byte of the GPU (a later cudaMalloc* fails or fragments its pool), a step loop
+ * that has promised its scheduler a fixed memory footprint, a process sharing the GPU whose memory budget is
+ * enforced from outside, or a context in which the stream-ordered pool is disabled.  This variant computes
+ * exactly what srhd_fluid_step computes (same kernels, same arguments, same results bit for bit, same stats),
+ * but calls no cudaMalloc / cudaMallocAsync / cudaFree* and no library routine that allocates.
+ *
+ * Where the scratch lives: in a fixed array of SRHD_NOALLOC_MAX_NPG bytes (64 KiB) that is part of the library
+ * image, so every GPU on which this library is used carries those 64 KiB from the moment the library's code is
+ * loaded there until the process exits, whether or not this call is ever made.
+ *
+ * Limits and rules
+ *   - npg <= SRHD_NOALLOC_MAX_NPG (65 536 patch groups = 2.7e8 cells, the size of the largest BASELINE config);
+ *     a larger npg returns SRHD_ERR_TOO_LARGE and launches nothing: split the batch and call again.
+ *   - MUSCL-Hancock only (params->integrator == SRHD_INTEGRATOR_MHM): the VL integrator's scratch is two
+ *     primitive tiles per group, far beyond a fixed array; it returns SRHD_ERR_BAD_PARAMS here.
+ *   - First call per device: the first call made with a given device current looks up the array's device
+ *     address (once per device, then cached; a cudaGetSymbolAddress call, which may make the runtime load the
+ *     library's code onto that device).  Make that first call during set-up, outside any stream capture and
+ *     before the phase in which allocation is forbidden; later calls on that device do no set-up.
+ *   - The array is shared by every call on the device and keeps whatever the last call left in it.  Each call
+ *     re-zeroes the npg bytes it is going to use, in stream order, before its kernels run, so stale flags are
+ *     never read.  Two calls whose kernels can overlap on one GPU (different streams without an ordering
+ *     between them, or two host threads) RACE on the array and give wrong results: keep calls to this entry
+ *     point on one device ordered one after the other.  Calls on different devices do not interact.
+ *   - Every other argument, error code and the asynchrony are those of srhd_fluid_step. */
+#define SRHD_NOALLOC_MAX_NPG 65536
+int srhd_fluid_step_noalloc(const srhd_real* cons_in, srhd_real* cons_out, int npg, double dt, double dh,
+                            const srhd_params* params, srhd_stats* stats, void* stream);
 
 /* Harness helpers for a uniform grid (reading S11, S13; NOT part of the paper's solver: they stand in
  * for the AMR driver's ghost-zone fill).  grid: [5][nz][ny][nx] conserved, extents multiples

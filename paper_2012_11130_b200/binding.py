@@ -45,7 +45,7 @@ class Stats(C.Structure):
 
 
 SYMBOLS = ["srhd_default_params", "srhd_prim2cons", "srhd_cons2prim", "srhd_max_signal_speed",
-           "srhd_fluid_step", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_flux_correction", "srhd_ghost_interp", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed", "srhd_grid_step_cfl",
+           "srhd_fluid_step", "srhd_fluid_step_noalloc", "srhd_fluid_step_fluxes", "srhd_fluid_step_cfl", "srhd_refine_flags", "srhd_flux_correction", "srhd_ghost_interp", "srhd_workspace_bytes", "srhd_grid_gather", "srhd_grid_scatter", "srhd_grid_scatter_speed", "srhd_patch_gather_speed", "srhd_grid_step_cfl",
            "srhd_fp64_peak_probe", "srhd_issue_probe", "srhd_quotient_check", "srhd_error_string", "srhd_build_is_exact", "srhd_build_variant"]
 
 _LIBS = {}
@@ -79,6 +79,8 @@ def load_library(exact=False):
     L.srhd_fluid_step.restype = C.c_int
     L.srhd_fluid_step.argtypes = [_VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_fluid_step_fluxes.restype = C.c_int
+    L.srhd_fluid_step_noalloc.argtypes = [_VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
+    L.srhd_fluid_step_noalloc.restype = C.c_int
     L.srhd_fluid_step_fluxes.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, C.POINTER(Params), _VP, _VP]
     L.srhd_fluid_step_cfl.restype = C.c_int
     L.srhd_fluid_step_cfl.argtypes = [_VP, _VP, _VP, C.c_int, _D, _D, _VP, _D, C.POINTER(Params), _VP, _VP]
@@ -245,6 +247,25 @@ def fluid_step(cons_in, dt, dh, par, cons_out=None, stats=None, exact=False):
     stats = new_stats(cons_in.device) if stats is None else stats
     _check(L.srhd_fluid_step(cons_in.data_ptr(), _shaped(cons_out, (npg, 8, 5, 8, 8, 8), "cons_out").data_ptr(), npg, float(dt),
                              float(dh), C.byref(par), stats.data_ptr(), _stream()), L)
+    return cons_out, stats
+
+
+NOALLOC_MAX_NPG = 65536   # SRHD_NOALLOC_MAX_NPG of include/srhd.h
+
+
+def fluid_step_noalloc(cons_in, dt, dh, par, cons_out, stats, exact=False):
+    """srhd_fluid_step_noalloc: the MUSCL-Hancock step for programs in which this library must not allocate GPU
+    memory (a host code whose pool owns the device, a fixed-footprint step loop).  Same result as fluid_step; the
+    pre-pass flags live in a 64 KiB array inside the library instead of a cudaMallocAsync block.  To keep the
+    promise on the Python side too, `cons_out` (npg,8,5,8,8,8) and `stats` (new_stats()) are REQUIRED here: this
+    wrapper creates no tensor.  At most NOALLOC_MAX_NPG groups per call; calls on one GPU must not overlap (they
+    share the array); make the first call on each device during set-up.  Returns (cons_out, stats)."""
+    L = load_library(exact)
+    cons_in, npg = _tiles(cons_in, par)
+    if cons_out is None or stats is None:
+        raise SrhdError("fluid_step_noalloc allocates nothing: pass cons_out and stats")
+    _check(L.srhd_fluid_step_noalloc(cons_in.data_ptr(), _shaped(cons_out, (npg, 8, 5, 8, 8, 8), "cons_out").data_ptr(),
+                                     npg, float(dt), float(dh), C.byref(par), stats.data_ptr(), _stream()), L)
     return cons_out, stats
 
 

@@ -18,6 +18,8 @@
 // If any face state or updated cell of the group fails Eq. 30 the CTA repeats the march with
 // beta <- 0.75 beta, finally with beta = 0.  Each cell's state crosses HBM once on the way
 // in (plus ghost layers) and once on the way out; the update re-reads its own cell through L2.
+#include <mutex>
+
 #include "srhd_common.cuh"
 #include "srhd_uniform.cuh"
 
@@ -717,4 +719,97 @@ extern "C" int srhd_fluid_step_cfl(const real* cons_in, real* cons_out, real* fl
   // dt is formed on the device; the host-side check of dt is replaced by the one of cfl (dt = 1 passes it)
   return fluid_step_impl(cons_in, cons_out, flux_out, npg, real(1.0), dh, params, stats, stream, d_max_speed, cfl,
                          min_speed);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// srhd_fluid_step_noalloc (include/srhd.h): the MUSCL-Hancock step for hosts that cannot let this library
+// allocate -- codes whose own pool owns the whole GPU, step loops with a fixed memory budget, processes whose
+// footprint is policed from outside.  Same two kernels as srhd_fluid_step; the only difference is where the
+// pre-pass's one-byte-per-group flags live: in the fixed array below instead of a cudaMallocAsync block.
+// ---------------------------------------------------------------------------------------------------------------
+namespace srhd {
+
+// 64 KiB per GPU that runs this library's code, from module load to process exit.  Shared by every call on the
+// device and never cleared behind the caller's back: each call zeroes the bytes it will use (below).
+static __device__ __align__(256) unsigned char g_noalloc_handled[SRHD_NOALLOC_MAX_NPG];
+
+// In host code `g_noalloc_handled` is only a handle for the runtime, not an address a kernel may dereference.
+// The real device address is asked for once per device, with that device current, and cached here.
+constexpr int kNoAllocMaxDevices = 64;
+static std::mutex g_noalloc_mutex;
+static unsigned char* g_noalloc_addr[kNoAllocMaxDevices] = {};
+
+// Returns 0 and the device address of the flag array on the CURRENT device; a cudaError_t if the look-up fails.
+// First use on a device does the look-up (set-up; keep it out of stream capture), later uses read the cache.
+static int noalloc_flags_on_current_device(unsigned char** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return (int)e;
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return (int)cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_handled);
+    if (e != cudaSuccess) return (int)e;
+    if (!p) return (int)cudaErrorInvalidSymbol;
+    g_noalloc_addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return 0;
+}
+
+template <int G, int RS>
+static int launch_fluid_noalloc(const real* cons_in, real* cons_out, int npg, real dt, real dh,
+                                const srhd_params* p, srhd_stats* stats, cudaStream_t st, unsigned char* flags) {
+  // the flags of this call's groups start at zero whatever the previous call left there (stream-ordered, so it
+  // cannot overtake a kernel of an earlier call on the same stream)
+  cudaError_t e = cudaMemsetAsync(flags, 0, (size_t)npg, st);
+  if (e != cudaSuccess) return (int)e;
+  const real rtol = newton_stop_rtol(p->newton_rtol);
+  uniform_tiles_kernel<G, RS><<<npg, kScanThreads, 0, st>>>(cons_in, cons_out, nullptr, dt, dh, rtol,
+                                                            p->newton_max_iter, stats, nullptr, real(0.0), real(0.0),
+                                                            flags);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return (int)e;
+  // with the flags handed in, launch_fluid launches the march only: no allocation on that branch
+  return launch_fluid<G, RS>(cons_in, cons_out, nullptr, npg, dt, dh, p, stats, st, nullptr, real(0.0), real(0.0), flags);
+}
+
+}  // namespace srhd
+
+extern "C" int srhd_fluid_step_noalloc(const real* cons_in, real* cons_out, int npg, double dt_, double dh_,
+                                       const srhd_params* params, srhd_stats* stats, void* stream) {
+  const real dt = (real)dt_, dh = (real)dh_;
+  // the argument checks of srhd_fluid_step, then the two limits of this variant
+  if (npg > 0 && (!cons_in || !cons_out)) return SRHD_ERR_NULL_POINTER;
+  const int pc = check_params(params);
+  if (pc) return pc;
+  if (params->integrator != SRHD_INTEGRATOR_MHM) return SRHD_ERR_BAD_PARAMS;   // VL scratch does not fit a fixed array
+  if (npg < 0) return SRHD_ERR_BAD_SIZE;
+  if (npg > SRHD_NOALLOC_MAX_NPG) return SRHD_ERR_TOO_LARGE;
+  if (!(dt > real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
+  if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & 7u))
+    return SRHD_ERR_BAD_ALIGN;
+  const int nxt = 16 + 2 * params->ghost;
+  const size_t in_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(real);
+  const size_t out_bytes = (size_t)npg * 8 * 5 * 512 * sizeof(real);
+  const uintptr_t a = reinterpret_cast<uintptr_t>(cons_in), b = reinterpret_cast<uintptr_t>(cons_out);
+  if (a < b + out_bytes && b < a + in_bytes) return SRHD_ERR_ALIAS;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (stats) {
+    const cudaError_t e = cudaMemsetAsync(stats, 0, sizeof(srhd_stats), st);
+    if (e != cudaSuccess) return (int)e;
+  }
+  if (npg == 0) return SRHD_OK;
+  unsigned char* flags = nullptr;
+  const int rc = noalloc_flags_on_current_device(&flags);
+  if (rc) return rc;
+  if (params->recon == SRHD_RECON_PLM) {
+    return params->riemann == SRHD_RIEMANN_HLLE
+               ? launch_fluid_noalloc<2, 0>(cons_in, cons_out, npg, dt, dh, params, stats, st, flags)
+               : launch_fluid_noalloc<2, 1>(cons_in, cons_out, npg, dt, dh, params, stats, st, flags);
+  }
+  return params->riemann == SRHD_RIEMANN_HLLE
+             ? launch_fluid_noalloc<3, 0>(cons_in, cons_out, npg, dt, dh, params, stats, st, flags)
+             : launch_fluid_noalloc<3, 1>(cons_in, cons_out, npg, dt, dh, params, stats, st, flags);
 }

@@ -576,6 +576,7 @@ extern "C" const char* srhd_error_string(int code) {
     case SRHD_ERR_BAD_STEP: return "dt and dh must be positive and finite";
     case SRHD_ERR_ALIAS: return "cons_in and cons_out overlap";
     case SRHD_ERR_BAD_ALIGN: return "cons_in must be 16-byte aligned";
+    case SRHD_ERR_TOO_LARGE: return "srhd_fluid_step_noalloc: npg exceeds SRHD_NOALLOC_MAX_NPG (65536); split the batch";
     default: break;
   }
   if (code > 0) return cudaGetErrorString(static_cast<cudaError_t>(code));

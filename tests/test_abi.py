@@ -55,7 +55,7 @@ def test_defaults_and_error_strings():
     assert p.minmod_coeff == 1.5 and p.newton_rtol == 1e-15
     assert b.params("plm", "hlle").ghost == 2
     L = b.load_library()
-    for code in range(-6, 1):
+    for code in range(-7, 1):
         assert len(L.srhd_error_string(code)) > 1
     assert L.srhd_workspace_bytes(10, C.byref(p)) == 10   # MUSCL-Hancock: one flag byte per patch group
 
@@ -75,6 +75,11 @@ def test_argument_errors_without_gpu():
     assert L.srhd_fluid_step(16, 1 << 30, -1, 0.1, 1.0, C.byref(p), None, None) == -3
     assert L.srhd_fluid_step(24, 1 << 30, 1, 0.1, 1.0, C.byref(p), None, None) == -6
     assert L.srhd_fluid_step(1 << 20, (1 << 20) + 64, 1, 0.1, 1.0, C.byref(p), None, None) == -5
+    # the no-allocation variant: srhd_fluid_step's checks plus its own two limits (include/srhd.h)
+    assert L.srhd_fluid_step_noalloc(16, 1 << 30, 1, 0.0, 1.0, C.byref(p), None, None) == -4
+    assert L.srhd_fluid_step_noalloc(24, 1 << 30, 1, 0.1, 1.0, C.byref(p), None, None) == -6
+    assert L.srhd_fluid_step_noalloc(16, 1 << 44, b.NOALLOC_MAX_NPG + 1, 0.1, 1.0, C.byref(p), None, None) == -7
+    assert L.srhd_fluid_step_noalloc(16, 1 << 30, 1, 0.1, 1.0, C.byref(b.params("plm", "hllc", integrator="vl")), None, None) == -2
     # device-side dt variant: needs the speed pointer and a positive Courant number
     assert L.srhd_fluid_step_cfl(16, 1 << 30, None, 1, 0.4, 1.0, None, 0.0, C.byref(p), None, None) == -1
     assert L.srhd_fluid_step_cfl(16, 1 << 30, None, 1, 0.0, 1.0, 64, 0.0, C.byref(p), None, None) == -4
