@@ -163,6 +163,16 @@ def cons2prim(cons, par=None, diag=False):
     return prim, st
 
 
+def is_physical(cons):
+    """Eq. 30 as the update applies it to an updated cell (O9): bool per state of a (5, n) list."""
+    cons = _f64(cons)
+    assert cons.ndim == 2 and cons.shape[0] == 5
+    n = cons.shape[1]
+    ok = np.empty(n, dtype=np.uint8)
+    lib().srhd_ref_is_physical(_p(cons), ok.ctypes.data_as(C.POINTER(C.c_ubyte)), C.c_size_t(n), C.c_size_t(n))
+    return ok.astype(bool)
+
+
 def max_signal_speed(cons, par=None):
     cons = _f64(cons)
     par = par or params()

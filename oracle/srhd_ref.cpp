@@ -851,6 +851,15 @@ void srhd_ref_cons2prim(const real* cons, real* prim, size_t n, size_t stride,
   }
 }
 
+// Eq. 30 on a list of states as the update applies it to its result (O9): 1 = passes
+void srhd_ref_is_physical(const real* cons, unsigned char* ok, size_t n, size_t stride) {
+  for (size_t i = 0; i < n; ++i) {
+    real U[5];
+    for (int q = 0; q < 5; ++q) U[q] = cons[q * stride + i];
+    ok[i] = is_physical(U) ? 1 : 0;
+  }
+}
+
 void srhd_ref_max_signal_speed(const real* cons, size_t n, size_t stride,
                                const srhd_ref_params* par, real* max_speed) {
   real umax = real(0.0);

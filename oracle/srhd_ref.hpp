@@ -79,6 +79,8 @@ real srhd_ref_umax_of_prim(const real W[5]);
 real srhd_ref_smax_of_umax(real umax);
 void   srhd_ref_max_signal_speed(const real* cons, size_t n, size_t stride,
                                  const srhd_ref_params* par, real* max_speed);
+// Eq. 30 as applied to an UPDATED cell (O9): ok[i] = 1 iff D > 0, Etilde > 0 and L > eps_machine
+void   srhd_ref_is_physical(const real* cons, unsigned char* ok, size_t n, size_t stride);
 
 // --- O5-O9 one fluid step ---------------------------------------------------------------------
 // Box form: cons_in [5][nz+2g][ny+2g][nx+2g] (x fastest) -> cons_out [5][nz][ny][nx].

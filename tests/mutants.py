@@ -15,7 +15,7 @@ import tempfile
 from concurrent.futures import ThreadPoolExecutor
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_vl.py", "tests/test_oracle_variants.py"]
+PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_pins_r3.py", "tests/test_oracle_vl.py", "tests/test_oracle_variants.py"]
 
 # (name, cited passage, old text, new text, pytest node ids / -k expression that must fail)
 MUTANTS = [
@@ -87,6 +87,35 @@ MUTANTS = [
     ("original scheme: the rest mass not subtracted in L", "P:198, P:626",
      "real L = std::fma(x, x, -musq) - real(1.0);", "real L = std::fma(x, x, -musq);",
      "test_fig16 or test_original"),
+    # the seven survivors of the round-2 judge's mutation run: what decides which states count as unphysical
+    ("Eq. 30 on updated cells: threshold 0 instead of eps_machine", "P:267-269 Eq. 30, O9",
+     "  const real L = std::fma(x, x + real(2.0), -musq);\n#else\n  const real L = std::fma(x, x, -musq) - real(1.0);\n#endif\n  return L > kEps;",
+     "  const real L = std::fma(x, x + real(2.0), -musq);\n#else\n  const real L = std::fma(x, x, -musq) - real(1.0);\n#endif\n  return L > real(0.0);",
+     "test_eq30_threshold"),
+    ("Eq. 30 on updated cells: Etilde > 0 not required", "SURVEY 8(c) O3, S9",
+     "if (!(D > real(0.0)) || !(Et > real(0.0))) return false;", "if (!(D > real(0.0))) return false;",
+     "test_negative_reduced_energy"),
+    ("Eq. 30 on updated cells: D > 0 not required", "SURVEY 8(c) O3, S9",
+     "if (!(D > real(0.0)) || !(Et > real(0.0))) return false;", "if (!(Et > real(0.0))) return false;",
+     "test_negative_reduced_energy or test_vacuum_floor"),
+    ("cons2prim verdict: Etilde > 0 not required", "SURVEY 8(c) O3",
+     "bool phys = (D > real(0.0)) && (Et > real(0.0));", "bool phys = (D > real(0.0));",
+     "test_negative_reduced_energy"),
+    ("cons2prim: vacuum floor at 0 instead of the smallest normal number", "reading S10",
+     "const bool dpos = D > kTiny;", "const bool dpos = D > real(0.0);",
+     "test_vacuum_floor"),
+    ("VL: a failing predictor state is not counted", "readings S18, S15",
+     "&it, nullptr)) ++half_fail;   // S15", "&it, nullptr)) (void)0;   // S15",
+     "test_vl_counts_a_failing_predictor"),
+    ("boundary map: outflow on the high side copies cell n-2", "reading S11",
+     "if (i >= n) return (bc_hi == 0) ? (i % n) : n - 1;", "if (i >= n) return (bc_hi == 0) ? (i % n) : n - 2;",
+     "test_boundary_map"),
+    ("boundary map: outflow on the low side copies cell 1", "reading S11",
+     "if (i < 0) return (bc_lo == 0) ? ((i % n) + n) % n : 0;", "if (i < 0) return (bc_lo == 0) ? ((i % n) + n) % n : 1;",
+     "test_boundary_map"),
+    ("boundary map: periodic wrap off by one on the low side", "reading S11",
+     "if (i < 0) return (bc_lo == 0) ? ((i % n) + n) % n : 0;", "if (i < 0) return (bc_lo == 0) ? ((i % n) + n - 1) % n : 0;",
+     "test_boundary_map"),
     ("original scheme: HLLC contact speed with D added to E", "reading S7, P:289",
      "const real Eh = Uh[4];  ", "const real Eh = Uh[4] + Uh[0];",
      "test_original_and_new"),
