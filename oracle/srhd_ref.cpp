@@ -1063,7 +1063,13 @@ unsigned long long srhd_ref_flux_correction(real* patches, const real* flux_coar
 // neighbours gives its 2^3 children  Q_child = ((Q + sx dx/4) + sy dy/4) + sz dz/4,  s = -+1, with the limited
 // slopes d of reading S3 (coefficient beta) -- on the CONSERVED variables (conservative: the children average to
 // the parent).  If any child fails Eq. 30, the same interpolation is done on the PRIMITIVE variables of the
-// seven cells and the children are converted back (always physical; "ghost zones do not affect conservation").
+// seven cells and the children are converted back ("ghost zones do not affect conservation").
+// Reading S22: the paper's "Eq. 30 is always satisfied" holds for interpolated primitives only while rho and p of
+// every child stay positive; three quarter-slopes of up to 0.375 (V0 - V_low) each (beta = 1.5) can sum to more than
+// V0 at a steep 3-D corner.  If a child's rho or p is not positive the cell's eight children are copies of the parent
+// state -- the end of the paper's own ladder for interpolation on parent patches ("a vanished minmod
+// coefficient is essentially equivalent to directly copying data from the parent patch") -- and the cell's
+// fallback byte is 2 instead of 1.  The returned count includes those cells.
 //   coarse [5][nz][ny][nx];  fine [5][2(nz-2)][2(ny-2)][2(nx-2)];  fallback (may be null) [nz-2][ny-2][nx-2] bytes.
 unsigned long long srhd_ref_ghost_interp(const real* coarse, int nx, int ny, int nz, real* fine, real beta,
                                          const srhd_ref_params* par, unsigned char* fallback) {
@@ -1085,7 +1091,7 @@ unsigned long long srhd_ref_ghost_interp(const real* coarse, int nx, int ny, int
           }
         }
         real child[8][5];
-        bool ok = true, fell_back = false;
+        bool ok = true, fell_back = false, prim_bad = false;
         for (int pass = 0; pass < 2; ++pass) {                // 0: conserved variables, 1: primitive variables
           real V[7][5];
           for (int m = 0; m < 7; ++m) {
@@ -1105,12 +1111,19 @@ unsigned long long srhd_ref_ghost_interp(const real* coarse, int nx, int ny, int
               v[q] = ((V[0][q] + ax) + ay) + az;
             }
             if (pass == 0) { for (int q = 0; q < 5; ++q) child[ch][q] = v[q]; ok = ok && is_physical(v); }
-            else prim2cons(v, child[ch]);
+            else {
+              if (!(v[0] > real(0.0)) || !(v[4] > real(0.0))) prim_bad = true;      // S22
+              prim2cons(v, child[ch]);
+            }
           }
           if (ok) break;
           if (pass == 0) { ++nfb; fell_back = true; }
         }
-        if (fallback) fallback[((size_t)(k - 1) * (ny - 2) + (j - 1)) * (nx - 2) + (i - 1)] = fell_back ? 1 : 0;
+        if (prim_bad)                                                                // S22: copy the parent
+          for (int ch = 0; ch < 8; ++ch)
+            for (int q = 0; q < 5; ++q) child[ch][q] = Q[0][q];
+        if (fallback)
+          fallback[((size_t)(k - 1) * (ny - 2) + (j - 1)) * (nx - 2) + (i - 1)] = prim_bad ? 2 : (fell_back ? 1 : 0);
         for (int ch = 0; ch < 8; ++ch) {
           const int I = 2 * (i - 1) + (ch & 1), J = 2 * (j - 1) + ((ch >> 1) & 1), Kk = 2 * (k - 1) + (ch >> 2);
           for (int q = 0; q < 5; ++q) fine[q * nf + ((size_t)Kk * fy + J) * fx + I] = child[ch][q];

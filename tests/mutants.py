@@ -15,7 +15,7 @@ import tempfile
 from concurrent.futures import ThreadPoolExecutor
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_pins_r3.py", "tests/test_oracle_vl.py", "tests/test_oracle_variants.py"]
+PINS = ["tests/test_oracle_pins_r2.py", "tests/test_oracle_pins_r3.py", "tests/test_oracle_amr_hooks.py", "tests/test_oracle_vl.py", "tests/test_oracle_variants.py"]
 
 # (name, cited passage, old text, new text, pytest node ids / -k expression that must fail)
 MUTANTS = [
@@ -116,6 +116,9 @@ MUTANTS = [
     ("boundary map: periodic wrap off by one on the low side", "reading S11",
      "if (i < 0) return (bc_lo == 0) ? ((i % n) + n) % n : 0;", "if (i < 0) return (bc_lo == 0) ? ((i % n) + n - 1) % n : 0;",
      "test_boundary_map"),
+    ("ghost interpolation: negative primitive children accepted", "reading S22, P:277",
+     "if (!(v[0] > real(0.0)) || !(v[4] > real(0.0))) prim_bad = true;", "(void)prim_bad;",
+     "test_ghost_interpolation_copies_the_parent"),
     ("original scheme: HLLC contact speed with D added to E", "reading S7, P:289",
      "const real Eh = Uh[4];  ", "const real Eh = Uh[4] + Uh[0];",
      "test_original_and_new"),

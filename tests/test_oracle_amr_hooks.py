@@ -115,7 +115,7 @@ def test_ghost_interpolation_falls_back_to_primitives(ref):
     prim[1:4] *= np.where(z < 3, 0.02, 1.0)                   # ... which is also slow
     coarse = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
     fine, fb, nfb = ref.ghost_interp(coarse, 1.5, par)
-    assert nfb > 0 and fb.sum() == nfb
+    assert nfb > 0 and fb.sum() == nfb and fb.max() == 1          # no cell needed the parent copy (S22)
     F = fine.reshape(5, -1)
     _, _, _, bad = ref.cons2prim(F, par, diag=True)
     assert bad.sum() == 0                                           # every child passes Eq. 30
@@ -128,3 +128,42 @@ def test_ghost_interpolation_falls_back_to_primitives(ref):
     Wf = ref.cons2prim(F, par)[0].reshape(fine.shape)
     assert Wf[0].min() >= prim[0].min() * (1 - 1e-9) and Wf[0].max() <= prim[0].max() * (1 + 1e-9)
     assert fb[:1].sum() == 0 and fb[3:].all()                   # hot planes: conserved interpolation; cold planes: fallback
+
+
+def test_ghost_interpolation_copies_the_parent_at_a_steep_3d_corner(ref):
+    """Reading S22: with density 0.01 / 1 / 3.97 along ALL three axes and beta = 1.5 each quarter-slope
+    is 1.5 * 0.99 / 4 = 0.371, so the child at the low corner would get rho = 1 - 3 * 0.371 < 0 from the primitive
+    interpolation: "Eq. 30 is always satisfied" does not cover it.  Such a cell's children are copies of the
+    parent (vanished coefficient = copy from the parent patch) and its flag is 2; every child passes Eq. 30
+    and the children trivially average to the parent."""
+    par = ref.params()
+    prof = np.array([0.01, 1.0, 3.97])
+    z, y, x = np.meshgrid(np.arange(3), np.arange(3), np.arange(3), indexing="ij")
+    prim = np.zeros((5, 3, 3, 3))
+    # separable would give 0.01^3 at the corner; the recipe wants the centre cell's SIX neighbours at 0.01 / 3.97
+    prim[0] = 1.0
+    for ax, idx in ((2, x), (1, y), (0, z)):
+        prim[0] = np.where((idx != 1) & ((x == 1).astype(int) + (y == 1).astype(int) + (z == 1).astype(int) == 2),
+                           prof[idx], prim[0])
+    assert prim[0][1, 1, 0] == 0.01 and prim[0][1, 1, 2] == 3.97 and prim[0][0, 1, 1] == 0.01 and prim[0][1, 1, 1] == 1.0
+    prim[4] = 1e-8 * prim[0]                          # cold: the conserved interpolation fails Eq. 30 first
+    prim[1] = 5.0                                     # moving, so that L sits on the boundary of Eq. 30 (L = O(T))
+    coarse = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    # the arithmetic of the premise, from the limiter's definition (S3): min(2|ab|/|a+b|, beta min(|a|,|b|)) / 4
+    a, b = 1.0 - 0.01, 3.97 - 1.0
+    q = min(2 * a * b / (a + b), 1.5 * min(a, b)) / 4
+    assert 1.0 - 3 * q < 0.0
+    fine, fb, nfb = ref.ghost_interp(coarse, 1.5, par)
+    assert fb.shape == (1, 1, 1) and fb[0, 0, 0] == 2 and nfb == 1
+    kids = fine.reshape(5, 8)
+    assert np.array_equal(kids, np.repeat(coarse[:, 1, 1, 1][:, None], 8, axis=1))
+    assert ref.is_physical(kids).all()
+    # a milder corner (slopes sum to less than the cell value) keeps the primitive interpolation: flag 1
+    prim2 = prim.copy()
+    prim2[0] = np.where(prim[0] == 0.01, 0.5, prim[0])
+    prim2[4] = 1e-8 * prim2[0]
+    c2 = ref.prim2cons(prim2.reshape(5, -1)).reshape(prim2.shape)
+    f2, fb2, n2 = ref.ghost_interp(c2, 1.5, par)
+    assert fb2[0, 0, 0] in (0, 1)
+    W = ref.cons2prim(f2.reshape(5, 8), par)[0]
+    assert W[0].min() > 0 and W[4].min() > 0
