@@ -21,7 +21,10 @@ VARIANTS = {"": ["-ffp-contract=off"], "fma": ["-ffp-contract=fast", "-mfma"],
             "gamma43": ["-ffp-contract=off", "-DSRHD_REF_EOS=1", "-DSRHD_REF_GAMMA_NUM=4", "-DSRHD_REF_GAMMA_DEN=3"],
             "orig": ["-ffp-contract=off", "-DSRHD_REF_SCHEME=1"],
             # "f32": every array and every operation in single precision (the precision of the paper's performance runs)
-            "f32": ["-ffp-contract=off", "-DSRHD_REF_F32"]}
+            "f32": ["-ffp-contract=off", "-DSRHD_REF_F32"],
+            # "ext": the fp64 algorithm (same thresholds) evaluated in x87 extended precision (long double, eps 1.1e-19):
+            # the "truth" both the fp64 oracle and the fp64 CUDA build are measured against; never the parity reference
+            "ext": ["-ffp-contract=off", "-DSRHD_REF_EXT"]}
 
 
 def lib_path(variant=""):

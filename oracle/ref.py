@@ -19,13 +19,16 @@ def _is_f32():
 
 
 def rdtype():
-    """numpy dtype of the oracle's `real` in the current variant (float32 for "f32", else float64)."""
+    """numpy dtype of the oracle's `real` in the current variant (float32 for "f32", x87 long double for "ext",
+    else float64)."""
+    if _VARIANT == "ext":
+        return np.longdouble
     return np.float32 if _is_f32() else np.float64
 
 
 def _D(x=None):
     """ctypes type of `real` (called without an argument) or a `real` scalar argument."""
-    t = C.c_float if _is_f32() else C.c_double
+    t = C.c_longdouble if _VARIANT == "ext" else (C.c_float if _is_f32() else C.c_double)
     return t if x is None else t(x)
 
 

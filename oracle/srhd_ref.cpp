@@ -45,8 +45,14 @@
 
 namespace {
 
+#ifdef SRHD_REF_EXT
+// extended-precision evaluation of the DOUBLE-precision algorithm: the thresholds are the algorithm's, not the type's
+constexpr real kEps = DBL_EPSILON;
+constexpr real kTiny = DBL_MIN;
+#else
 constexpr real kEps = std::numeric_limits<real>::epsilon();  // eps_machine of Eq. 30: 2.2e-16 (double), 1.2e-7 (single)
 constexpr real kTiny = std::numeric_limits<real>::min();     // smallest positive normal number (reading S10)
+#endif
 #if SRHD_REF_EOS == 1
 constexpr real kGnum = SRHD_REF_GAMMA_NUM, kGden = SRHD_REF_GAMMA_DEN;   // Gamma = kGnum / kGden
 constexpr real kG1 = kGnum / (kGnum - kGden);                             // Gamma / (Gamma - 1): 2.5 or 4, exact

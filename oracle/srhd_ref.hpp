@@ -26,8 +26,14 @@
 
 // every state array and every scalar of the arithmetic is a `real`: double, or float in the SRHD_REF_F32 variant
 // (the run-time parameters and the counters keep their types)
-#ifdef SRHD_REF_F32
+// SRHD_REF_EXT: x87 extended precision (64-bit significand, eps = 1.1e-19): the SAME algorithm with the SAME
+// thresholds (Eq. 30 and the S10 floor stay at double's eps_machine / DBL_MIN) evaluated 2048 times more finely --
+// the stand-in for "the true update" against which the fp64 oracle and the fp64 CUDA build are both measured
+// (tests/test_gpu_truth.py); never the parity reference
+#if defined(SRHD_REF_F32)
 typedef float real;
+#elif defined(SRHD_REF_EXT)
+typedef long double real;
 #else
 typedef double real;
 #endif

@@ -148,3 +148,49 @@ def test_boundary_map_against_hand_tables(ref, g):
         assert np.array_equal(ref.grid_pad(grid, g, bc), want), bc
         tiles = ref.grid_gather(grid, g, bc)                     # one patch group: the tile IS the padded grid
         assert tiles.shape[0] == 1 and np.array_equal(tiles[0], want), bc
+
+
+# ---- the extended-precision variant of the oracle ("ext": the stand-in for the true update) --------------------
+def test_extended_precision_variant_is_the_same_algorithm_evaluated_more_finely(ref):
+    """oracle/build.py "ext" (long double, eps = 1.1e-19) is what tests/test_gpu_truth.py measures both the fp64 oracle
+    and the CUDA build against.  Pinned here: (1) its prim->cons agrees with the 40-digit evaluation of the
+    DEFINITIONS (tests/mp_defs.py) to 1e-17 where fp64 cannot do better than 1e-16; (2) the thresholds are the fp64
+    algorithm's: Eq. 30 still switches at 2^-52 and the S10 floor at DBL_MIN; (3) one fluid step makes the same
+    retry decisions as the fp64 oracle and differs from it by fp64 round-off only."""
+    import mpmath as mp
+    from paper_2012_11130_b200 import workloads as wl
+    from tests import mp_defs
+    from tests.gpu_util import step_err
+    prim = wl.conversion_states(n=64, seed=9)
+    with ref.variant("ext"):
+        assert ref.rdtype() == np.longdouble and np.finfo(np.longdouble).eps < 2e-19
+        cons = ref.prim2cons(prim.astype(np.longdouble))
+    c64 = ref.prim2cons(prim)
+    worst_ext = worst_64 = 0.0
+    for k in range(prim.shape[1]):
+        want = mp_defs.prim2cons([float(v) for v in prim[:, k]])
+        for q in (0, 4):
+            w = mp.mpf(want[q])
+            worst_ext = max(worst_ext, float(abs(mp.mpf(str(np.format_float_scientific(cons[q, k], precision=25))) - w) / abs(w)))
+            worst_64 = max(worst_64, float(abs(mp.mpf(float(c64[q, k])) - w) / abs(w)))
+    assert worst_ext <= 2e-18 and worst_64 >= 5e-17, (worst_ext, worst_64)
+    # (2) thresholds
+    states = _threshold_states()
+    cons = np.array([[D, M[0], M[1], M[2], E] for D, M, E, _ in states]).T.copy()
+    want = np.array([c > 1.0 for *_, c in states])
+    tiny = np.array([[0.5 * DBL_MIN, 0.5 * DBL_MIN, 0.0, 0.0, DBL_MIN]]).T.copy()
+    with ref.variant("ext"):
+        assert np.array_equal(ref.is_physical(cons.astype(np.longdouble)), want)
+        prim_t, _, _, bad = ref.cons2prim(tiny.astype(np.longdouble), diag=True)
+    assert bad[0] == 1 and prim_t[0, 0] == np.longdouble(DBL_MIN) and prim_t[1, 0] == 0
+    # (3) one step on rough data with retries
+    par = ref.params("plm", "hllc", max_retry=3)
+    box = _rough_box(ref, 4, par.ghost)
+    dh = 1.0 / 64
+    dt = 0.4 * dh / ref.max_signal_speed(box.reshape(5, -1))
+    o64, st64, p64 = ref.step_box(box, dt, dh, par)
+    with ref.variant("ext"):
+        oe, ste, pe = ref.step_box(box.astype(np.longdouble), dt, dh, par)
+    assert pe == p64 and (ste.n_retry_pg, ste.n_unphys_final) == (st64.n_retry_pg, st64.n_unphys_final)
+    e = step_err(o64.astype(np.longdouble), oe, 0)
+    assert 0 < float(e.max()) <= 1e-11, float(e.max())
