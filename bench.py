@@ -362,6 +362,16 @@ def ncu_traffic(workload):
         return None
 
 
+def ncu_traffic_source(workload):
+    """Which committed capture roofline.traffic was copied from (it is a citation, not a measurement of this run)."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        e = t.get(workload)
+        return None if not e else f'{e["capture"]} ({e["kernel"]}); copied into profiles/ncu_traffic.json, not measured in this run'
+    except Exception:
+        return None
+
+
 def time_workload(name, steps, warmup, scale, world, local, rank, from_start=False, e2e_steps=0, fused=True, lib=False):
     """Time `steps` steps of one workload after `warmup` untimed ones (from_start: the config's own run from
     its initial condition, warm-up on a second instance).  Returns a dict of measured figures."""
@@ -416,15 +426,19 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
     ms = ev0.elapsed_time(ev1)
     k_each = [a.elapsed_time(b) for a, b in kev]
     k_ms = sum(k_each) / len(k_each)
+    passes_each = []
     for row in log.cpu():
         s = B.Stats.from_buffer_copy(row.numpy().tobytes())
+        passes_each.append(s.n_passes / st.npg)
         for k in tot:
             tot[k] += getattr(s, k)
+    i_max = int(np.argmax(k_each))
     value, ms_max = aggregate_value(ncell, steps, ms, world, "cuda")
     nxt = 16 + 2 * st.par.ghost
     nconv = steps * st.npg * (nxt ** 3 + 2 * 3 * 17 * 256)        # conversions the algorithm defines
     k_mean = tot["newton_iters"] / nconv
     flops_alg = ncell * fm.fluid_step_flops_per_cell(recon, riemann, k_mean)          # per step
+    flops_survey = ncell * fm.fluid_step_flops_per_cell_survey(recon, riemann, k_mean)
     flops_exe = fm.fluid_step_flops_executed(recon, riemann, ncell * steps, tot["exec_c2p"], tot["exec_newton"],
                                              tot["exec_riemann"], tot["exec_hancock"]) / steps
     res = {
@@ -440,7 +454,13 @@ def time_workload(name, steps, warmup, scale, world, local, rank, from_start=Fal
         "exec_riemann_per_cell": tot["exec_riemann"] / (ncell * steps),
         "state_mb": st.grid.numel() * 8 / 1e6, "tiles_mb": st.tiles.numel() * 8 / 1e6,
         "launches_per_step": st.launches_per_step,
-        "call_ms": {"min": min(k_each), "median": float(np.median(k_each)), "max": max(k_each)},
+        # the work of a step depends on the state (retry passes, uniform groups): the slowest call is named with
+        # the number of marches per patch group it made, next to the median step's
+        "call_ms": {"min": min(k_each), "median": float(np.median(k_each)), "max": max(k_each),
+                    "max_at_timed_step": i_max + 1, "passes_per_patch_group_at_max": passes_each[i_max],
+                    "passes_per_patch_group_median": float(np.median(passes_each))},
+        "flops_survey_per_step": flops_survey,
+        "value_median_step": ncell * world / (float(np.median(k_each)) * 1e-3),
         # algorithmic bytes per cell update (5 reals in, 5 out) / step time
         "hbm_gbs": ncell * 10.0 * st.patches.element_size() / (ms_max / steps * 1e-3) / 1e9,
     }
@@ -506,7 +526,13 @@ def roofline_of(r, peak, peak_meas, hbm_peak, have_peaks):
         "kernel_share_of_step": r["kernel_ms"] / r["ms_per_step"],
         "flops_per_cell": r["flops_alg_per_step"] / r["ncell"],
         "flops_executed_per_cell": r["flops_exec_per_step"] / r["ncell"],
-        "traffic": ncu_traffic(r["name"]),
+        "traffic": ncu_traffic(r["name"]), "traffic_source": ncu_traffic_source(r["name"]),
+        "flop_count": "frac uses paper_2012_11130_b200/flopmodel.py's hand count of the formulas as written (68 flops per "
+                      "Newton iteration); *_survey_count uses SURVEY.md section 8(a)'s counts (43 per iteration)",
+        "flops_per_cell_survey_count": r["flops_survey_per_step"] / r["ncell"],
+        "frac_survey_count": r["flops_survey_per_step"] / t / 1e12 / peak,
+        "value_at_median_call": r["value_median_step"],
+        "value_at_median_call_note": "cells / median duration of the timed call (call_ms.median): the whole step for a fused run, the fluid-step call alone when the roofline kernel is timed through the separate calls",
         "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
                 "peak_source": "MEASURED_PEAKS.json" if have_peaks else "fallback 6650 GB/s (B200_PROFILING.md)"},
     }
@@ -596,6 +622,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if "f32" in str(args.lib) else "f64", "data": "synthetic",
         "config": {"workload": args.workload, "library": B.load_library(lib).srhd_build_variant().decode(),
+                   "scheme_override": args.scheme,
                    "what": head["desc"], "grid": head["shape"], "patch_groups": head["npg"],
                    "scheme": f'{head["recon"]}+{head["riemann"]}', "cfl": head["cfl"],
                    "parallelism": "replicas only" if world > 1 else "1 gpu",
@@ -608,6 +635,14 @@ def run_ours(args):
                    "uniform_patch_group_fraction": head["uniform_fraction"],
                    "step_call_ms": head["call_ms"],
                    "per_workload": {k: summary_of(v) for k, v in per.items()}},
+        # what `value` is and is not: on the jet 99.97 % of the patch groups are undisturbed ambient
+        # gas that the pre-pass proves uniform and copies, so `value` is an HBM-bound figure; the solver's own
+        # throughput is the general path's, on data with no uniform region
+        "solver_path": {"workload": general["name"], "scheme": f'{general["recon"]}+{general["riemann"]}',
+                        "value": general["value"], "unit": UNIT, "ms_per_step": general["ms_per_step"],
+                        "uniform_patch_group_fraction": general["uniform_fraction"],
+                        "note": "throughput of the SRHD solver proper (no uniform patch groups: every group is marched); "
+                                "the headline `value` is dominated by uniform groups finished by the pre-pass"},
         "clocks": head["clocks"],
         "roofline": roof,
         "gpu_launches": head["launches_per_step"] * args.steps,
@@ -633,11 +668,21 @@ def main():
     ap.add_argument("--lib", default="production",
                     help="which in-tree library to time: production (default), exact, or a variant of "
                          "paper_2012_11130_b200/build.py (gamma53, f32, ...); the headline is the production library")
+    ap.add_argument("--scheme", default=None, choices=["plm+hlle", "plm+hllc", "ppm+hlle", "ppm+hllc"],
+                    help="DIAGNOSTIC: run --workload's data with another reconstruction / Riemann solver than its config "
+                         "names (e.g. --workload random512 --scheme ppm+hllc: the PPM+HLLC kernel on data with no uniform "
+                         "region); the line says so in config.scheme_override and is not a headline")
     ap.add_argument("--aux", action="store_true", help="time the SURVEY 8f entry points instead (one JSON line, not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.scheme:
+        if args.workload == "conv":
+            raise SystemExit("--scheme applies to the fluid-step workloads")
+        rc, rs = args.scheme.split("+")
+        _, _, cfl, desc = WORKLOADS[args.workload]
+        WORKLOADS[args.workload] = (rc, rs, cfl, desc + f" -- DIAGNOSTIC: run with {args.scheme.upper()} instead of the config's scheme")
     if args.aux:
         return run_aux(args)
     if args.impl == "reference":

@@ -45,10 +45,14 @@ extern "C" {
 #define SRHD_OK                 0
 #define SRHD_ERR_NULL_POINTER  (-1)
 #define SRHD_ERR_BAD_PARAMS    (-2)   /* recon/riemann out of range, ghost != 2 (PLM) / 3 (PPM), ... */
-#define SRHD_ERR_BAD_SIZE      (-3)   /* stride < n, negative npg, grid extent not a multiple of 16 */
+#define SRHD_ERR_BAD_SIZE      (-3)   /* stride < n, negative npg, grid extent not a multiple of 16, */
+                                      /* or (nx/16)*(ny/16) > 104857 (32-bit in-plane offsets)      */
 #define SRHD_ERR_BAD_STEP      (-4)   /* dt <= 0 or dh <= 0 (or not finite)                         */
-#define SRHD_ERR_ALIAS         (-5)   /* cons_in and cons_out overlap                               */
-#define SRHD_ERR_BAD_ALIGN     (-6)   /* cons_in not 16-byte aligned (TMA bulk copies need it)      */
+#define SRHD_ERR_ALIAS         (-5)   /* cons_in and cons_out (srhd_grid_step_cfl: any two of       */
+                                      /* patches_in, patches_out, cons_in) overlap                  */
+#define SRHD_ERR_BAD_ALIGN     (-6)   /* cons_in not 16-byte aligned (TMA bulk copies), or cons_out */
+                                      /* / patches_in / patches_out not aligned to 2*sizeof(srhd_real) */
+                                      /* (16 bytes in the fp64 builds: pair loads and stores)       */
 #define SRHD_ERR_TOO_LARGE     (-7)   /* srhd_fluid_step_noalloc: npg > SRHD_NOALLOC_MAX_NPG         */
 
 #define SRHD_RECON_PLM   0
@@ -154,7 +158,7 @@ int srhd_fluid_step_fluxes(const srhd_real* cons_in, srhd_real* cons_out, srhd_r
 /* The same step with the time step formed ON THE DEVICE from a signal speed that is already there
  * (srhd_max_signal_speed / srhd_grid_scatter_speed wrote it): dt = cfl * dh / max(*d_max_speed, min_speed)
  * (Eq. 28).  No host round trip for dt, so a sequence of steps can be enqueued without a
- * synchronisation.  d_max_speed: device, one double, read by every CTA at kernel start; min_speed >= 0
+ * synchronisation.  d_max_speed: device, one srhd_real, read by every CTA at kernel start; min_speed >= 0
  * bounds the speed from below (e.g. the signal speed of a fixed-inflow state that is not in the
  * grid yet); the caller guarantees max(*d_max_speed, min_speed) > 0.  flux_out may be NULL. */
 int srhd_fluid_step_cfl(const srhd_real* cons_in, srhd_real* cons_out, srhd_real* flux_out, int npg, double cfl,
@@ -183,7 +187,10 @@ int srhd_refine_flags(const srhd_real* cons_in, int npg, int quantity, double c_
  *   face_patch, face_id    : device, [nf] ints: patch index, face 0 x-lo .. 5 z-hi
  *   d_n_skipped : device, one unsigned long long (zeroed by the call): cells whose correction was ignored
  * Faces are processed class by class (x-lo, x-hi, y-lo, ...), so a cell on a patch edge is corrected through
- * one face after the other, in that order; within a class a (patch, face) pair may appear once. */
+ * one face after the other, in that order; within a class a (patch, face) pair may appear once.
+ * The two index arrays are TRUSTED (the call does not know how many patches `patches` holds): a face_id outside
+ * 0..5 is silently never applied and a face_patch beyond the array is an out-of-bounds access -- validate them
+ * where they are built (binding.py checks both before the call). */
 int srhd_flux_correction(srhd_real* patches, const srhd_real* flux_coarse, const srhd_real* flux_fine,
                          const int* face_patch, const int* face_id, int nf, double dt, double dh,
                          unsigned long long* d_n_skipped, void* stream);
@@ -192,10 +199,13 @@ int srhd_flux_correction(srhd_real* patches, const srhd_real* flux_coarse, const
  * neighbours gives its 2^3 children Q -+ d_x/4 -+ d_y/4 -+ d_z/4 with the limited slopes of reading S3
  * (coefficient minmod_coeff) on the CONSERVED variables (conservative); where a child fails Eq. 30 the
  * same interpolation is done on the PRIMITIVE variables of the seven cells and converted back ("Eq. 30 is
- * always satisfied ... ghost zones do not affect conservation").
+ * always satisfied ... ghost zones do not affect conservation").  That holds while every child's rho and p stay
+ * positive; where the primitive interpolation would give a child rho <= 0 or p <= 0 (a steep 3-D corner) the eight
+ * children are copies of the parent state (vanished minmod coefficient = copy from the parent; reading S22).
  *   coarse: device, [5][nz][ny][nx];  fine: device, [5][2(nz-2)][2(ny-2)][2(nx-2)]
- *   fallback: device, (nz-2)(ny-2)(nx-2) bytes, 1 where the fallback was used (may be NULL)
- *   d_n_fallback: device, one unsigned long long (zeroed by the call) */
+ *   fallback: device, (nz-2)(ny-2)(nx-2) bytes: 0 conserved interpolation, 1 primitive interpolation, 2 parent
+ *             copied (may be NULL)
+ *   d_n_fallback: device, one unsigned long long (zeroed by the call): cells with fallback != 0 */
 int srhd_ghost_interp(const srhd_real* coarse, int nx, int ny, int nz, srhd_real* fine, double minmod_coeff,
                       const srhd_params* params, unsigned char* fallback, unsigned long long* d_n_fallback,
                       void* stream);
@@ -273,7 +283,7 @@ int srhd_patch_gather_speed(const srhd_real* patches, srhd_real* cons_in, int nx
  *   cons_in    : device scratch for the ghosted tiles, [npg][5][nxt]^3, nxt = 16 + 2*params->ghost; only the
  *                tiles of groups that are not uniform are written
  *   flux_out   : as srhd_fluid_step_fluxes, may be NULL
- *   d_max_speed: device, one double: receives S_max of the CURRENT state (Eq. 26-27); the step then uses
+ *   d_max_speed: device, one srhd_real: receives S_max of the CURRENT state (Eq. 26-27); the step then uses
  *                dt = cfl * dh / max(S_max, min_speed) (Eq. 28) without a host round trip
  * A patch group whose whole tile (ghost zones after the boundary mapping included) holds one state bit for bit is
  * finished by the first kernel: its new patches are its old ones (srhd_stats.n_uniform_pg counts them), so its

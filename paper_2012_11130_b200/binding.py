@@ -193,7 +193,7 @@ def _inflow(inflow, ny, nx):
 
 
 def new_stats(device="cuda"):
-    """Device buffer holding one srhd_stats (40 bytes)."""
+    """Device buffer holding one srhd_stats (sizeof(Stats) = 88 bytes), zeroed."""
     return torch.zeros(C.sizeof(Stats), dtype=torch.uint8, device=device)
 
 

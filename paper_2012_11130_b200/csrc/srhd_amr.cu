@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const real* __restric
     }
     real sl[3][5], child[8][5];
     quarter_slopes(Q, beta, sl);
-    bool ok = true;
+    bool ok = true, prim_bad = false;
 #pragma unroll
     for (int ch = 0; ch < 8; ++ch) {
       child_of(Q[0], sl, ch, child[ch]);
@@ -115,13 +115,22 @@ __global__ void __launch_bounds__(128) ghost_interp_kernel(const real* __restric
         for (int ch = 0; ch < 8; ++ch) {
           real v[5];
           child_of(W[0], sl, ch, v);
+          // S22: interpolated primitives pass Eq. 30 only while rho and p stay positive (a steep 3-D corner can
+          // take three quarter-slopes off the cell value)
+          prim_bad = prim_bad || !(v[0] > real(0.0)) || !(v[4] > real(0.0));
           prim2cons(v, child[ch]);
+        }
+        if (prim_bad) {                         // copy the parent: the vanished-coefficient end of the ladder
+#pragma unroll
+          for (int ch = 0; ch < 8; ++ch)
+#pragma unroll
+            for (int q = 0; q < 5; ++q) child[ch][q] = Q[0][q];
         }
         if (valid) ++nfb;
       }
     }
     if (valid) {
-      if (fallback) fallback[e] = ok ? 0 : 1;
+      if (fallback) fallback[e] = ok ? 0 : (prim_bad ? 2 : 1);
 #pragma unroll
       for (int ch = 0; ch < 8; ++ch) {
         const int I = 2 * (i - 1) + (ch & 1), J = 2 * (j - 1) + ((ch >> 1) & 1), K = 2 * (k - 1) + (ch >> 2);

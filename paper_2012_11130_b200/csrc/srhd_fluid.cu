@@ -682,7 +682,9 @@ static int fluid_step_impl(const real* cons_in, real* cons_out, real* flux_out, 
   if (pc) return pc;
   if (npg < 0) return SRHD_ERR_BAD_SIZE;
   if (!(dt > real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
-  if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & 7u))
+  // cons_in: TMA bulk copies (16 bytes) and the pair loads of the uniform-tile scan; cons_out: the uniform-tile
+  // path stores pairs of srhd_real (flux_out is written one value at a time)
+  if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & (sizeof(real2) - 1)))
     return SRHD_ERR_BAD_ALIGN;
   const int nxt = 16 + 2 * params->ghost;
   const size_t in_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(real);
@@ -788,7 +790,7 @@ extern "C" int srhd_fluid_step_noalloc(const real* cons_in, real* cons_out, int 
   if (npg < 0) return SRHD_ERR_BAD_SIZE;
   if (npg > SRHD_NOALLOC_MAX_NPG) return SRHD_ERR_TOO_LARGE;
   if (!(dt > real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dt) || !std::isfinite(dh)) return SRHD_ERR_BAD_STEP;
-  if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & 7u))
+  if ((reinterpret_cast<uintptr_t>(cons_in) & 15u) || (reinterpret_cast<uintptr_t>(cons_out) & (sizeof(real2) - 1)))
     return SRHD_ERR_BAD_ALIGN;
   const int nxt = 16 + 2 * params->ghost;
   const size_t in_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(real);

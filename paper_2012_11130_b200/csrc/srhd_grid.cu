@@ -393,6 +393,10 @@ using namespace srhd;
 
 static int check_extents(int nx, int ny, int nz) {
   if (nx <= 0 || ny <= 0 || nz <= 0 || nx % 16 || ny % 16 || nz % 16) return SRHD_ERR_BAD_SIZE;
+  // the gather kernels keep the in-plane patch offsets (up to (ny/16)(nx/16) * 20480 values) in 32-bit integers:
+  // a very flat grid (e.g. 8192 x 4096 x 16) would overflow them, so it is refused rather than read out of bounds
+  if ((long long)(nx / 16) * (ny / 16) * 20480 > 2147483647LL) return SRHD_ERR_BAD_SIZE;
+  if ((long long)(nx / 16) * (ny / 16) * (nz / 16) > 2147483647LL / 8) return SRHD_ERR_BAD_SIZE;   // npg * 8 patches in an int
   return SRHD_OK;
 }
 
@@ -506,9 +510,24 @@ extern "C" int srhd_grid_step_cfl(const real* patches_in, real* patches_out, rea
   if (ce) return ce;
   if (!(cfl > real(0.0)) || !std::isfinite(cfl) || !(min_speed >= real(0.0)) || !(dh > real(0.0)) || !std::isfinite(dh))
     return SRHD_ERR_BAD_STEP;
-  if (patches_in == patches_out) return SRHD_ERR_ALIAS;
-  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  // patches_in / patches_out are read and written as pairs of srhd_real (own-uniform scan, uniform-tile stores);
+  // cons_in is the target of the ghost-zone fill and the source of the march's 16-byte TMA bulk copies
+  if ((reinterpret_cast<uintptr_t>(patches_in) & (sizeof(real2) - 1)) ||
+      (reinterpret_cast<uintptr_t>(patches_out) & (sizeof(real2) - 1)) || (reinterpret_cast<uintptr_t>(cons_in) & 15u))
+    return SRHD_ERR_BAD_ALIGN;
   const int npg = (nx / 16) * (ny / 16) * (nz / 16);
+  {
+    // the three state buffers must be pairwise disjoint (the pre-pass reads patches_in while it writes the other two)
+    const int nxt = 16 + 2 * params->ghost;
+    const size_t patch_bytes = (size_t)npg * 8 * 5 * 512 * sizeof(real);
+    const size_t tile_bytes = (size_t)npg * 5 * nxt * nxt * nxt * sizeof(real);
+    const uintptr_t a = reinterpret_cast<uintptr_t>(patches_in), b = reinterpret_cast<uintptr_t>(patches_out),
+                    c = reinterpret_cast<uintptr_t>(cons_in);
+    if ((a < b + patch_bytes && b < a + patch_bytes) || (a < c + tile_bytes && c < a + patch_bytes) ||
+        (b < c + tile_bytes && c < b + patch_bytes))
+      return SRHD_ERR_ALIAS;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (params->integrator != SRHD_INTEGRATOR_MHM) {           // no pre-pass for the VL kernels: the two plain calls
     const int e = srhd_patch_gather_speed(patches_in, cons_in, nx, ny, nz, bc, inflow_mask, inflow_cons, params,
                                           d_max_speed, stream);
@@ -574,8 +593,8 @@ extern "C" const char* srhd_error_string(int code) {
     case SRHD_ERR_BAD_PARAMS: return "bad srhd_params (recon / riemann / ghost / coefficients)";
     case SRHD_ERR_BAD_SIZE: return "bad size (stride < n, negative count, extent not a multiple of 16)";
     case SRHD_ERR_BAD_STEP: return "dt and dh must be positive and finite";
-    case SRHD_ERR_ALIAS: return "cons_in and cons_out overlap";
-    case SRHD_ERR_BAD_ALIGN: return "cons_in must be 16-byte aligned";
+    case SRHD_ERR_ALIAS: return "state buffers overlap (cons_in / cons_out; patches_in / patches_out / cons_in)";
+    case SRHD_ERR_BAD_ALIGN: return "cons_in must be 16-byte aligned; cons_out, patches_in and patches_out aligned to two srhd_real";
     case SRHD_ERR_TOO_LARGE: return "srhd_fluid_step_noalloc: npg exceeds SRHD_NOALLOC_MAX_NPG (65536); split the batch";
     default: break;
   }

@@ -73,3 +73,15 @@ def fluid_step_flops_executed(recon, riemann, ncell, exec_c2p, exec_newton, exec
     hancock = rec + 2 * (P2C + PHYS_FLUX) + 5 + 10 + 10       # per (cell, direction): dF, share of the sum, two adds
     return (exec_c2p * C2P_FIXED + exec_newton * NEWTON_ITER + exec_riemann * (2 * SIDE_SETUP + solver) +
             exec_hancock * hancock + ncell * (UPDATE + EQ30_CHECK + UMAX))
+
+
+def fluid_step_flops_per_cell_survey(recon, riemann, k_mean):
+    """The same quantity with SURVEY.md section 8(a)'s own per-step counts (simple / div / sqrt operations, each
+    counted as ONE flop): A1 cons->prim (40+38k)/(5+4k)/(2.5+k); A2 16/1/2; A3 PLM 210/15/0 or PPM 420/15/0;
+    A4 282/30/18; A5 = 6 x A1; A6 per face HLLC 123/9/5 or HLLE 85/7/4, three faces per cell; A7 30; A8 10/1/0.
+    It charges 43 flops per Newton iteration where the count above charges 68 (it shares T and dT/dhtilde between f
+    and f'), so it comes out about 15-20 % lower; bench.py prints both and says which one `frac` uses."""
+    a1 = 47.5 + 43.0 * k_mean
+    a3 = 225.0 if recon in (0, "plm") else 435.0
+    a6 = 3 * (96.0 if riemann in (0, "hlle") else 137.0)
+    return a1 + 19.0 + a3 + 330.0 + 6 * a1 + a6 + 30.0 + 11.0

@@ -75,6 +75,9 @@ def test_argument_errors_without_gpu():
     assert L.srhd_fluid_step(16, 1 << 30, -1, 0.1, 1.0, C.byref(p), None, None) == -3
     assert L.srhd_fluid_step(24, 1 << 30, 1, 0.1, 1.0, C.byref(p), None, None) == -6
     assert L.srhd_fluid_step(1 << 20, (1 << 20) + 64, 1, 0.1, 1.0, C.byref(p), None, None) == -5
+    # vector accesses: cons_out on an 8-byte boundary (a view one double into a buffer) is refused, not faulted on
+    assert L.srhd_fluid_step(16, (1 << 30) + 8, 1, 0.1, 1.0, C.byref(p), None, None) == -6
+    assert L.srhd_fluid_step_noalloc(16, (1 << 30) + 8, 1, 0.1, 1.0, C.byref(p), None, None) == -6
     # the no-allocation variant: srhd_fluid_step's checks plus its own two limits (include/srhd.h)
     assert L.srhd_fluid_step_noalloc(16, 1 << 30, 1, 0.0, 1.0, C.byref(p), None, None) == -4
     assert L.srhd_fluid_step_noalloc(24, 1 << 30, 1, 0.1, 1.0, C.byref(p), None, None) == -6
@@ -100,6 +103,14 @@ def test_argument_errors_without_gpu():
     assert L.srhd_grid_step_cfl(16, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.0, 1.0, 0.0, C.byref(p), None, 64, None) == -4
     assert L.srhd_grid_step_cfl(16, 16, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -5
     assert L.srhd_grid_step_cfl(16, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(bad), None, 64, None) == -2
+    # round 3 (ADVICE): alignment of the three state buffers, range overlap (not only pointer equality), flat-grid overflow
+    assert L.srhd_grid_step_cfl(24, 1 << 30, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -6
+    assert L.srhd_grid_step_cfl(16, (1 << 30) + 8, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -6
+    assert L.srhd_grid_step_cfl(16, 1 << 30, (1 << 31) + 8, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -6
+    assert L.srhd_grid_step_cfl(1 << 30, (1 << 30) + 4096, 1 << 31, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -5
+    assert L.srhd_grid_step_cfl(1 << 30, 1 << 31, (1 << 30) + 4096, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -5
+    assert L.srhd_grid_step_cfl(1 << 30, 1 << 31, (1 << 31) - 4096, None, 16, 16, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -5
+    assert L.srhd_grid_step_cfl(1 << 30, 1 << 31, 1 << 32, None, 8192, 4096, 16, bc, None, None, 0.4, 1.0, 0.0, C.byref(p), None, 64, None) == -3
     # every variant library answers the same way and says what it is
     for key in ("gamma53", "gamma53_exact", "gamma43_exact", "orig_exact", "f32", "f32_exact", True):
         V = b.load_library(key)

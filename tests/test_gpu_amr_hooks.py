@@ -63,3 +63,37 @@ def test_ghost_interp_parity_with_fallback(ref):
             scale = np.abs(want).reshape(5, -1).max(1)
             scale[1:4] = scale[1:4].max()
             assert (np.abs(g - want) / scale[:, None, None, None]).max() <= 1e-13
+
+
+def test_ghost_interp_copies_the_parent_at_a_steep_corner(ref):
+    """Reading S22: where the primitive fallback would give a child rho <= 0 (density 0.01 / 1 / 3.97 along all three
+    axes, beta = 1.5) the CUDA kernel, like the oracle, copies the parent and flags the cell 2; a grid holding such
+    corners next to ordinary cold gradients reproduces the oracle's flags and children."""
+    n = 9
+    z, y, x = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    prim = np.zeros((5, n, n, n))
+    prim[0] = 1.0
+    for c in ((1, 1, 1), (4, 4, 4), (7, 4, 1)):          # corners: the six neighbours of c at 0.01 (low) / 3.97 (high)
+        for ax in range(3):
+            lo, hi = list(c), list(c)
+            lo[ax] -= 1
+            hi[ax] += 1
+            prim[0][tuple(lo)], prim[0][tuple(hi)] = 0.01, 3.97
+    prim[4] = 1e-8 * prim[0]
+    prim[1] = 5.0 + 0.1 * x
+    coarse = ref.prim2cons(prim.reshape(5, -1)).reshape(prim.shape)
+    par = ref.params()
+    want, wfb, wn = ref.ghost_interp(coarse, 1.5, par)
+    assert (wfb == 2).sum() >= 3 and (wfb == 1).sum() > 0
+    for exact in (True, False):
+        fine, fb, cnt = B.ghost_interp(dev(coarse), 1.5, B.params(exact=exact), exact=exact)
+        assert int(cnt.cpu()) == wn and np.array_equal(fb.cpu().numpy(), wfb)
+        g = fine.cpu().numpy()
+        copied = np.repeat(np.repeat(np.repeat(wfb == 2, 2, 0), 2, 1), 2, 2)
+        assert np.array_equal(g[:, copied], want[:, copied])            # copies of the parent: exact in every build
+        if exact:
+            assert np.array_equal(g, want)
+        else:
+            scale = np.abs(want).reshape(5, -1).max(1)
+            scale[1:4] = scale[1:4].max()
+            assert (np.abs(g - want) / scale[:, None, None, None]).max() <= 1e-13
